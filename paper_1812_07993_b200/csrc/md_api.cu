@@ -1,0 +1,623 @@
+// md_api.cu -- C ABI (include/md.h) over the kernels in md_kernels.cuh.
+// Host logic only: validation, workspace carving, launch order, CUDA graphs.
+#include "../../include/md.h"
+#include "md_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+namespace {
+
+thread_local std::string g_create_error;
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// Bump allocator over the caller's workspace; base == nullptr only measures.
+struct Carver {
+    char* base;
+    size_t off = 0;
+    explicit Carver(void* b) : base((char*)b) {}
+    template <typename U>
+    U* take(size_t n)
+    {
+        off = align_up(off, 256);
+        U* p = base ? (U*)(base + off) : nullptr;
+        off += n * sizeof(U);
+        return p;
+    }
+};
+
+struct GridSpec {
+    int nc[3];
+    long long ncell;
+    bool cells_ok;
+};
+
+GridSpec make_grid(const md_box& box, double rc)
+{
+    GridSpec g;
+    g.cells_ok = true;
+    g.ncell = 1;
+    for (int a = 0; a < 3; ++a) {
+        g.nc[a] = 1;
+        if (a < box.dim) {
+            int k = (int)std::floor(box.len[a] / rc);
+            if (k < 1) k = 1;
+            if (box.bc[a] == MD_BC_PERIODIC && k < 3) g.cells_ok = false;
+            g.nc[a] = k;
+        }
+        g.ncell *= g.nc[a];
+    }
+    if (g.ncell > (1ll << 30)) g.cells_ok = false;
+    return g;
+}
+
+const char* validate(const md_box* box, const md_lj* lj, const md_opts* o, long long nv, long long nw)
+{
+    if (!box || !lj || !o) return "null parameter struct";
+    if (box->dim != 2 && box->dim != 3) return "dim must be 2 or 3";
+    if (nv < 1 || nv > (1ll << 30)) return "n_vapor must be in [1, 2^30]";
+    if (nw < 0 || nw > (1ll << 30)) return "n_wall must be in [0, 2^30]";
+    if (!(o->dt > 0) || !std::isfinite(o->dt)) return "dt must be > 0";
+    if (!(o->mass > 0) || !std::isfinite(o->mass)) return "mass must be > 0";
+    if (o->precision != 64 && o->precision != 32) return "precision must be 64 or 32";
+    if (o->force_algo < MD_FORCE_AUTO || o->force_algo > MD_FORCE_CELLS) return "unknown force_algo";
+    if (!(lj->r_cut > 0) || !std::isfinite(lj->r_cut)) return "r_cut must be > 0";
+    if (!(lj->sigma > 0) || !(lj->sigma_w > 0)) return "sigma, sigma_w must be > 0";
+    if (!std::isfinite(lj->eps) || !std::isfinite(lj->eps_w)) return "eps, eps_w must be finite";
+    for (int a = 0; a < box->dim; ++a) {
+        if (!(box->len[a] > 0) || !std::isfinite(box->len[a])) return "box length must be > 0";
+        if (box->bc[a] != MD_BC_PERIODIC && box->bc[a] != MD_BC_REFLECT) return "unknown boundary condition";
+        if (box->bc[a] == MD_BC_PERIODIC && box->len[a] < 2.0 * lj->r_cut)
+            return "periodic box length < 2 r_cut (minimum image undefined)";
+    }
+    return nullptr;
+}
+
+int pick_algo(const md_opts& o, const GridSpec& g, long long nv)
+{
+    if (o.force_algo == MD_FORCE_ALLPAIRS) return MD_FORCE_ALLPAIRS;
+    if (o.force_algo == MD_FORCE_CELLS) return g.cells_ok ? MD_FORCE_CELLS : -1;
+    return (g.cells_ok && nv >= 2048) ? MD_FORCE_CELLS : MD_FORCE_ALLPAIRS;
+}
+
+template <typename T>
+struct Layout {
+    md::State<T> st[2];
+    md::Force<T> f;
+    int *cell, *slot, *count, *start, *tile_sum;
+    T *wx, *wy, *wz, *wtx, *wty, *wtz;
+    int *wcell, *wslot, *wstart;
+    uint8_t* wnear;
+    md::EnergyOut eo;
+    double *part, *eout;
+    int* err;
+    unsigned long long* tests;
+    double *stage0, *stage1, *wstage;
+    int red_blocks;
+    size_t bytes;
+};
+
+template <typename T>
+Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell, bool cells)
+{
+    Layout<T> l;
+    Carver c(base);
+    size_t n = (size_t)align_up((size_t)nv, 64);
+    size_t m = (size_t)align_up((size_t)(nw > 0 ? nw : 1), 64);
+    for (int b = 0; b < (cells ? 2 : 1); ++b) {
+        l.st[b].x = c.take<T>(n); l.st[b].y = c.take<T>(n); l.st[b].z = c.take<T>(n);
+        l.st[b].vx = c.take<T>(n); l.st[b].vy = c.take<T>(n); l.st[b].vz = c.take<T>(n);
+        l.st[b].id = c.take<int>(n);
+    }
+    if (!cells) l.st[1] = l.st[0];
+    l.f.fx = c.take<T>(n); l.f.fy = c.take<T>(n); l.f.fz = c.take<T>(n);
+    l.cell = c.take<int>(n > m ? n : m);
+    l.slot = c.take<int>(n > m ? n : m);
+    size_t nc = cells ? (size_t)ncell : 1;
+    l.count = c.take<int>(nc);
+    l.start = c.take<int>(nc + 1);
+    l.tile_sum = c.take<int>((size_t)cdiv((long long)nc, md::SCAN_TILE) + 1);
+    l.wx = c.take<T>(m); l.wy = c.take<T>(m); l.wz = c.take<T>(m);
+    l.wtx = c.take<T>(m); l.wty = c.take<T>(m); l.wtz = c.take<T>(m);
+    l.wcell = l.cell; l.wslot = l.slot;   // wall binning runs once, before the vapor's
+    l.wstart = c.take<int>(nc + 1);
+    l.wnear = c.take<uint8_t>(nc);
+    l.eo.pe = c.take<double>(n); l.eo.pew = c.take<double>(n); l.eo.vir = c.take<double>(n);
+    l.eo.cvv = c.take<int>(n); l.eo.cvw = c.take<int>(n);
+    l.red_blocks = (int)std::min<long long>(cdiv(nv, md::RED_THREADS), 1024);
+    l.part = c.take<double>(6 * (size_t)l.red_blocks);
+    l.eout = c.take<double>(8);
+    l.err = c.take<int>(4);
+    l.tests = c.take<unsigned long long>(2);
+    l.stage0 = c.take<double>(n * dim);
+    l.stage1 = c.take<double>(n * dim);
+    l.wstage = c.take<double>(m * dim);
+    l.bytes = align_up(c.off, 256);
+    return l;
+}
+
+} // namespace
+
+struct md_sim {
+    std::string err;
+    virtual ~md_sim() {}
+    virtual int step(long long n) = 0;
+    virtual int get_state(double* pos, double* vel, double* force, double* pe, long long* step) = 0;
+    virtual int energy(md_energy_out* out) = 0;
+    virtual int profile(long long n, md_kernel_times* out) = 0;
+    virtual int pair_tests(long long* tests) = 0;
+    virtual void info(int* algo, int nc[3], int* kps) const = 0;
+};
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            err = std::string(#call) + ": " + cudaGetErrorString(e_);                              \
+            return MD_ERR_CUDA;                                                                    \
+        }                                                                                          \
+    } while (0)
+
+namespace {
+
+template <typename T>
+struct Sim : md_sim {
+    md::Params<T> p;
+    Layout<T> l;
+    md::Walls<T> walls;
+    int dim = 3, algo = MD_FORCE_CELLS, cur = 0;
+    long long step_no = 0, energy_step = -1;
+    cudaStream_t stream = nullptr;
+    cudaGraphExec_t g1[2] = {nullptr, nullptr}, gN[2] = {nullptr, nullptr};
+    static constexpr int CHUNK = 16;
+    cudaEvent_t ev[5] = {};
+    double e_host[6];
+
+    ~Sim() override
+    {
+        for (int k = 0; k < 2; ++k) {
+            if (g1[k]) cudaGraphExecDestroy(g1[k]);
+            if (gN[k]) cudaGraphExecDestroy(gN[k]);
+        }
+        for (auto& e : ev) if (e) cudaEventDestroy(e);
+    }
+
+    int blocks(int threads) const { return cdiv(p.nv, threads); }
+
+    // ---- a2: bin `n` particles of state s into cell order (count -> scan -> caller scatters)
+    void launch_scan(int* count, int* start)
+    {
+        int tiles = cdiv(p.ncell, md::SCAN_TILE);
+        md::k_scan_reduce<<<tiles, md::SCAN_THREADS, 0, stream>>>(count, p.ncell, l.tile_sum);
+        md::k_scan_apply<<<tiles, md::SCAN_THREADS, 0, stream>>>(count, p.ncell, l.tile_sum, start);
+    }
+
+    template <bool ENERGY, bool KICK, bool COUNT>
+    void launch_force()
+    {
+        if (algo == MD_FORCE_CELLS)
+            md::k_force_cells<T, ENERGY, KICK, COUNT><<<blocks(128), 128, 0, stream>>>(p, l.st[cur], l.start, walls, l.f,
+                                                                                        l.eo, l.tests);
+        else
+            md::k_force_allpairs<T, ENERGY, KICK><<<blocks(md::AP_THREADS), md::AP_THREADS, 0, stream>>>(
+                p, l.st[cur], l.wtx, l.wty, l.wtz, l.f, l.eo);
+    }
+
+    // One velocity-Verlet step: a1 -> a2 -> a3 + a4. `t` (optional) = events around each kernel.
+    void enqueue_step(cudaEvent_t* t)
+    {
+        if (t) cudaEventRecord(t[0], stream);
+        if (algo == MD_FORCE_CELLS) {
+            md::k_kick_drift_bin<T, true, true><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, l.count, l.cell,
+                                                                                l.slot, l.err);
+            if (t) cudaEventRecord(t[1], stream);
+            launch_scan(l.count, l.start);
+            if (t) cudaEventRecord(t[2], stream);
+            md::k_scatter<T><<<blocks(256), 256, 0, stream>>>(p.nv, l.st[cur], l.st[cur ^ 1], l.f, l.f, l.cell, l.slot,
+                                                              l.start, 0);
+            cur ^= 1;
+            if (t) cudaEventRecord(t[3], stream);
+        } else {
+            md::k_kick_drift_bin<T, true, false><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, nullptr, nullptr,
+                                                                                 nullptr, l.err);
+            if (t) { cudaEventRecord(t[1], stream); cudaEventRecord(t[2], stream); cudaEventRecord(t[3], stream); }
+        }
+        launch_force<false, true, false>();
+        if (t) cudaEventRecord(t[4], stream);
+    }
+
+    int capture(int nsteps, cudaGraphExec_t* out)
+    {
+        cudaGraph_t g = nullptr;
+        CK(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
+        for (int k = 0; k < nsteps; ++k) enqueue_step(nullptr);
+        CK(cudaStreamEndCapture(stream, &g));
+        cudaError_t e = cudaGraphInstantiate(out, g, 0);
+        cudaGraphDestroy(g);
+        if (e != cudaSuccess) { err = std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e); return MD_ERR_CUDA; }
+        return MD_OK;
+    }
+
+    int step(long long n) override
+    {
+        if (n < 0) { err = "n_steps < 0"; return MD_ERR_INVALID_ARG; }
+        if (stream == nullptr || stream == cudaStreamLegacy || stream == cudaStreamPerThread) {
+            // the default streams cannot be captured: plain launches
+            for (long long k = 0; k < n; ++k) enqueue_step(nullptr);
+            step_no += n;
+            CK(cudaGetLastError());
+            return MD_OK;
+        }
+        while (n > 0) {
+            const int par = algo == MD_FORCE_CELLS ? cur : 0;
+            if (n >= CHUNK) {
+                if (!gN[par]) { int c0 = cur; int rc = capture(CHUNK, &gN[par]); cur = c0; if (rc) return rc; }
+                CK(cudaGraphLaunch(gN[par], stream));
+                n -= CHUNK; step_no += CHUNK;       // CHUNK is even: buffer parity unchanged
+            } else {
+                if (!g1[par]) { int c0 = cur; int rc = capture(1, &g1[par]); cur = c0; if (rc) return rc; }
+                CK(cudaGraphLaunch(g1[par], stream));
+                if (algo == MD_FORCE_CELLS) cur ^= 1;
+                n -= 1; step_no += 1;
+            }
+        }
+        return MD_OK;
+    }
+
+    int profile(long long n, md_kernel_times* out) override
+    {
+        if (!out || n < 0) { err = "bad arguments"; return MD_ERR_INVALID_ARG; }
+        memset(out, 0, sizeof(*out));
+        for (auto& e : ev) if (!e) CK(cudaEventCreate(&e));
+        for (long long k = 0; k < n; ++k) {
+            enqueue_step(ev);
+            CK(cudaStreamSynchronize(stream));
+            for (int q = 0; q < 4; ++q) {
+                float ms = 0.f;
+                CK(cudaEventElapsedTime(&ms, ev[q], ev[q + 1]));
+                out->ms[q] += ms;
+            }
+            float tot = 0.f;
+            CK(cudaEventElapsedTime(&tot, ev[0], ev[4]));
+            out->total_ms += tot;
+            ++step_no;
+        }
+        const bool cells = algo == MD_FORCE_CELLS;
+        out->launches[0] = n; out->launches[1] = cells ? 2 * n : 0; out->launches[2] = cells ? n : 0;
+        out->launches[3] = n; out->steps = n;
+        return MD_OK;
+    }
+
+    int check_err_flag()
+    {
+        int h = 0;
+        CK(cudaMemcpyAsync(&h, l.err, sizeof(int), cudaMemcpyDeviceToHost, stream));
+        CK(cudaStreamSynchronize(stream));
+        if (h) { err = "a particle left a reflecting box (more than one bounce in a step)"; return MD_ERR_STATE; }
+        return MD_OK;
+    }
+
+    int energy_pass()
+    {
+        if (energy_step == step_no) return MD_OK;
+        launch_force<true, false, false>();
+        md::k_energy_partial<T><<<l.red_blocks, md::RED_THREADS, 0, stream>>>(p.nv, p.mass, l.st[cur], l.eo, l.part);
+        md::k_energy_final<<<1, md::RED_THREADS, 0, stream>>>(l.red_blocks, l.part, l.eout);
+        CK(cudaMemcpyAsync(e_host, l.eout, 6 * sizeof(double), cudaMemcpyDeviceToHost, stream));
+        CK(cudaStreamSynchronize(stream));
+        CK(cudaGetLastError());
+        energy_step = step_no;
+        return MD_OK;
+    }
+
+    int energy(md_energy_out* out) override
+    {
+        if (!out) { err = "out is NULL"; return MD_ERR_INVALID_ARG; }
+        int rc = check_err_flag();
+        if (rc) return rc;
+        rc = energy_pass();
+        if (rc) return rc;
+        out->kinetic = e_host[0];
+        out->potential = e_host[1];
+        out->potential_vw = e_host[2];
+        out->potential_vv = e_host[1] - e_host[2];
+        out->virial = e_host[3];
+        out->pairs_vv = (long long)llround(e_host[4]) / 2;
+        out->pairs_vw = (long long)llround(e_host[5]);
+        out->step = step_no;
+        if (!std::isfinite(out->kinetic) || !std::isfinite(out->potential)) {
+            err = "non-finite energy";
+            return MD_ERR_NONFINITE;
+        }
+        return MD_OK;
+    }
+
+    int export3(const T* a, const T* b, const T* c, double* host)
+    {
+        md::k_export3<T><<<blocks(256), 256, 0, stream>>>(p.nv, dim, l.st[cur].id, a, b, c, l.stage0);
+        CK(cudaMemcpyAsync(host, l.stage0, sizeof(double) * (size_t)p.nv * dim, cudaMemcpyDeviceToHost, stream));
+        CK(cudaStreamSynchronize(stream));
+        return MD_OK;
+    }
+
+    int get_state(double* pos, double* vel, double* force, double* pe, long long* step) override
+    {
+        int rc = check_err_flag();
+        if (rc) return rc;
+        const md::State<T>& s = l.st[cur];
+        if (pos && (rc = export3(s.x, s.y, s.z, pos))) return rc;
+        if (vel && (rc = export3(s.vx, s.vy, s.vz, vel))) return rc;
+        if (force && (rc = export3(l.f.fx, l.f.fy, l.f.fz, force))) return rc;
+        if (pe) {
+            if ((rc = energy_pass())) return rc;
+            md::k_export1<<<blocks(256), 256, 0, stream>>>(p.nv, s.id, l.eo.pe, l.stage0);
+            CK(cudaMemcpyAsync(pe, l.stage0, sizeof(double) * (size_t)p.nv, cudaMemcpyDeviceToHost, stream));
+            CK(cudaStreamSynchronize(stream));
+        }
+        if (step) *step = step_no;
+        CK(cudaGetLastError());
+        return MD_OK;
+    }
+
+    int pair_tests(long long* tests) override
+    {
+        if (!tests) { err = "tests is NULL"; return MD_ERR_INVALID_ARG; }
+        if (algo == MD_FORCE_ALLPAIRS) {
+            *tests = (long long)p.nv * ((long long)p.nv - 1 + p.nw);
+            return MD_OK;
+        }
+        CK(cudaMemsetAsync(l.tests, 0, sizeof(unsigned long long), stream));
+        launch_force<false, false, true>();
+        unsigned long long h = 0;
+        CK(cudaMemcpyAsync(&h, l.tests, sizeof(h), cudaMemcpyDeviceToHost, stream));
+        CK(cudaStreamSynchronize(stream));
+        *tests = (long long)h;
+        return MD_OK;
+    }
+
+    void info(int* a, int nc[3], int* kps) const override
+    {
+        if (a) *a = algo;
+        if (nc) for (int k = 0; k < 3; ++k) nc[k] = p.nc[k];
+        if (kps) *kps = algo == MD_FORCE_CELLS ? 5 : 2;
+    }
+
+    int init(const md_box& box, const md_lj& lj, const md_opts& o, long long nv, const double* pos, const double* vel,
+             long long nw, const double* wall);
+};
+
+} // namespace
+
+namespace {
+
+template <typename T>
+__global__ void k_scatter_wall(int n, const T* sx, const T* sy, const T* sz, T* dx, T* dy, T* dz, const int* cell,
+                               const int* slot, const int* start)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int d = start[cell[i]] + slot[i];
+    dx[d] = sx[i]; dy[d] = sy[i]; dz[d] = sz[i];
+}
+
+template <typename T>
+int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long nv, const double* pos,
+                 const double* vel, long long nw, const double* wall)
+{
+    // wall particles: upload, convert, and (cell mode) bin once -- they are never integrated
+    if (nw > 0) {
+        CK(cudaMemcpyAsync(l.wstage, wall, sizeof(double) * (size_t)nw * dim, cudaMemcpyHostToDevice, stream));
+        md::State<T> ws = {l.wtx, l.wty, l.wtz, nullptr, nullptr, nullptr, nullptr};
+        md::k_import<T><<<cdiv(nw, 256), 256, 0, stream>>>((int)nw, dim, l.wstage, nullptr, ws);
+    }
+    CK(cudaMemsetAsync(l.err, 0, 4 * sizeof(int), stream));
+    if (algo == MD_FORCE_CELLS) {
+        CK(cudaMemsetAsync(l.count, 0, sizeof(int) * (size_t)p.ncell, stream));
+        md::Params<T> pw = p;
+        pw.nv = (int)nw;
+        if (nw > 0) {
+            md::State<T> ws = {l.wtx, l.wty, l.wtz, nullptr, nullptr, nullptr, nullptr};
+            md::k_kick_drift_bin<T, false, true><<<cdiv(nw, 256), 256, 0, stream>>>(pw, ws, l.f, l.count, l.wcell,
+                                                                                    l.wslot, l.err);
+        }
+        launch_scan(l.count, l.wstart);
+        if (nw > 0)
+            k_scatter_wall<T><<<cdiv(nw, 256), 256, 0, stream>>>((int)nw, l.wtx, l.wty, l.wtz, l.wx, l.wy, l.wz,
+                                                                 l.wcell, l.wslot, l.wstart);
+        md::k_wall_near<T><<<cdiv(p.ncell, 256), 256, 0, stream>>>(p, l.wstart, l.wnear);
+    }
+    walls.x = l.wx; walls.y = l.wy; walls.z = l.wz; walls.start = l.wstart; walls.near = l.wnear;
+    // vapor: upload, AoS -> SoA
+    CK(cudaMemcpyAsync(l.stage0, pos, sizeof(double) * (size_t)nv * dim, cudaMemcpyHostToDevice, stream));
+    CK(cudaMemcpyAsync(l.stage1, vel, sizeof(double) * (size_t)nv * dim, cudaMemcpyHostToDevice, stream));
+    md::k_import<T><<<blocks(256), 256, 0, stream>>>((int)nv, dim, l.stage0, l.stage1, l.st[0]);
+    cur = 0;
+    if (algo == MD_FORCE_CELLS) {
+        md::k_kick_drift_bin<T, false, true><<<blocks(256), 256, 0, stream>>>(p, l.st[0], l.f, l.count, l.cell, l.slot,
+                                                                             l.err);
+        launch_scan(l.count, l.start);
+        md::k_scatter<T><<<blocks(256), 256, 0, stream>>>(p.nv, l.st[0], l.st[1], l.f, l.f, l.cell, l.slot, l.start, 0);
+        cur = 1;
+    }
+    launch_force<false, false, false>();   // f(0)
+    CK(cudaStreamSynchronize(stream));
+    CK(cudaGetLastError());
+    return MD_OK;
+}
+
+template <typename T>
+int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o, long long nv, const double* pos,
+             const double* vel, long long nw, const double* wall, void* ws, size_t ws_bytes, void* stream,
+             const GridSpec& g, int algo)
+{
+    Sim<T>* s = new Sim<T>();
+    const bool cells = algo == MD_FORCE_CELLS;
+    s->dim = box.dim;
+    s->algo = algo;
+    s->stream = (cudaStream_t)stream;
+    s->l = carve<T>(ws, box.dim, nv, nw, g.ncell, cells);
+    if (s->l.bytes > ws_bytes) {
+        g_create_error = "workspace too small";
+        delete s;
+        return MD_ERR_WORKSPACE;
+    }
+    md::Params<T>& p = s->p;
+    p.nv = (int)nv; p.nw = (int)nw;
+    p.ncell = cells ? (int)g.ncell : 1;
+    for (int a = 0; a < 3; ++a) {
+        const bool on = a < box.dim;
+        p.L[a] = on ? (T)box.len[a] : T(1);
+        p.invL[a] = on ? (T)(1.0 / box.len[a]) : T(1);
+        p.bc[a] = on ? box.bc[a] : md::BC_NONE;
+        p.nc[a] = cells ? g.nc[a] : 1;
+        p.inv_c[a] = on ? (T)((double)g.nc[a] / box.len[a]) : T(1);
+    }
+    auto ucut = [&](double eps, double sig) {
+        double q = (sig * sig) / (lj.r_cut * lj.r_cut), q3 = q * q * q;
+        return lj.shift_energy ? 4.0 * eps * (q3 * q3 - q3) : 0.0;
+    };
+    p.rc2 = (T)(lj.r_cut * lj.r_cut);
+    p.sig2_vv = (T)(lj.sigma * lj.sigma); p.e24_vv = (T)(24.0 * lj.eps); p.e4_vv = (T)(4.0 * lj.eps);
+    p.uc_vv = (T)ucut(lj.eps, lj.sigma);
+    p.sig2_vw = (T)(lj.sigma_w * lj.sigma_w); p.e24_vw = (T)(24.0 * lj.eps_w); p.e4_vw = (T)(4.0 * lj.eps_w);
+    p.uc_vw = (T)ucut(lj.eps_w, lj.sigma_w);
+    p.dt = (T)o.dt; p.hk = (T)(o.dt / (2.0 * o.mass)); p.mass = o.mass;
+    int rc = s->init(box, lj, o, nv, pos, vel, nw, wall);
+    if (rc != MD_OK) {
+        g_create_error = s->err;
+        delete s;
+        return rc;
+    }
+    *out = s;
+    return MD_OK;
+}
+
+template <typename T>
+double time_fma(cudaStream_t st, T* out, cudaEvent_t a, cudaEvent_t b)
+{
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int grid = sms * 8, iters = 1 << 14;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(a, st);
+        md::k_fma_chain<T><<<grid, 256, 0, st>>>(iters, T(1), out);
+        cudaEventRecord(b, st);
+        cudaEventSynchronize(b);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        double tf = 2.0 * 8.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    return best;
+}
+
+} // namespace
+
+extern "C" {
+
+size_t md_workspace_bytes(const md_box* box, const md_lj* lj, const md_opts* o, long long nv, long long nw)
+{
+    if (validate(box, lj, o, nv, nw)) return 0;
+    GridSpec g = make_grid(*box, lj->r_cut);
+    int algo = pick_algo(*o, g, nv);
+    if (algo < 0) return 0;
+    const bool cells = algo == MD_FORCE_CELLS;
+    return o->precision == 64 ? carve<double>(nullptr, box->dim, nv, nw, g.ncell, cells).bytes
+                              : carve<float>(nullptr, box->dim, nv, nw, g.ncell, cells).bytes;
+}
+
+int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj* lj, const md_opts* o, long long nv,
+              const double* pos, const double* vel, long long nw, const double* wall, void* ws, size_t ws_bytes,
+              void* stream)
+{
+    (void)pore;
+    if (!out) { g_create_error = "out is NULL"; return MD_ERR_INVALID_ARG; }
+    *out = nullptr;
+    const char* why = validate(box, lj, o, nv, nw);
+    if (!why && (!pos || !vel)) why = "pos / vel is NULL";
+    if (!why && nw > 0 && !wall) why = "wall_pos is NULL with n_wall > 0";
+    if (!why && (!ws || ((uintptr_t)ws & 255))) why = "device_workspace is NULL or not 256-byte aligned";
+    if (why) { g_create_error = why; return MD_ERR_INVALID_ARG; }
+    const int dim = box->dim;
+    auto inside = [&](const double* r, long long n) {
+        for (long long i = 0; i < n; ++i)
+            for (int a = 0; a < dim; ++a) {
+                double v = r[i * dim + a];
+                if (!(v >= 0.0 && v <= box->len[a])) return false;   // also rejects NaN
+            }
+        return true;
+    };
+    if (!inside(pos, nv) || !inside(wall, nw)) { g_create_error = "position non-finite or outside [0, L]"; return MD_ERR_INVALID_ARG; }
+    for (long long i = 0; i < nv * dim; ++i)
+        if (!std::isfinite(vel[i])) { g_create_error = "velocity non-finite"; return MD_ERR_INVALID_ARG; }
+    GridSpec g = make_grid(*box, lj->r_cut);
+    int algo = pick_algo(*o, g, nv);
+    if (algo < 0) { g_create_error = "cell list needs >= 3 cells in every periodic dimension"; return MD_ERR_UNSUPPORTED; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        g_create_error = "no CUDA device (there is no CPU fallback)";
+        return MD_ERR_CUDA;
+    }
+    return o->precision == 64
+               ? create_t<double>(out, *box, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo)
+               : create_t<float>(out, *box, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo);
+}
+
+int md_step(md_sim* s, long long n) { return s ? s->step(n) : MD_ERR_INVALID_ARG; }
+int md_get_state(md_sim* s, double* pos, double* vel, double* force, double* pe, long long* step)
+{
+    return s ? s->get_state(pos, vel, force, pe, step) : MD_ERR_INVALID_ARG;
+}
+int md_energy(md_sim* s, md_energy_out* out) { return s ? s->energy(out) : MD_ERR_INVALID_ARG; }
+int md_profile_step(md_sim* s, long long n, md_kernel_times* out) { return s ? s->profile(n, out) : MD_ERR_INVALID_ARG; }
+int md_pair_tests(md_sim* s, long long* t) { return s ? s->pair_tests(t) : MD_ERR_INVALID_ARG; }
+int md_info(const md_sim* s, int* algo, int nc[3], int* kps)
+{
+    if (!s) return MD_ERR_INVALID_ARG;
+    s->info(algo, nc, kps);
+    return MD_OK;
+}
+int md_destroy(md_sim* s)
+{
+    delete s;
+    return MD_OK;
+}
+const char* md_last_error(const md_sim* s) { return s ? s->err.c_str() : g_create_error.c_str(); }
+
+int md_measure_peaks(void* scratch, size_t bytes, void* stream, md_peaks* out)
+{
+    if (!scratch || !out || bytes < (1u << 20)) return MD_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return MD_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return MD_ERR_CUDA;
+    out->fp64_tflops = time_fma<double>(st, (double*)scratch, a, b);
+    out->fp32_tflops = time_fma<float>(st, (float*)scratch, a, b);
+    size_t n16 = bytes / 32;   // double2 elements per half
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(a, st);
+        md::k_copy<<<148 * 16, 256, 0, st>>>((const double2*)scratch, (double2*)scratch + n16, n16);
+        cudaEventRecord(b, st);
+        cudaEventSynchronize(b);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        double gbs = 2.0 * 16.0 * (double)n16 / (ms * 1e-3) * 1e-9;
+        if (rep > 0 && gbs > best) best = gbs;
+    }
+    out->copy_gbs = best;
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    return cudaGetLastError() == cudaSuccess ? MD_OK : MD_ERR_CUDA;
+}
+
+} // extern "C"
