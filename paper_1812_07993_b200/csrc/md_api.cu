@@ -90,7 +90,7 @@ struct Layout {
     md::State<T> st[2];
     md::Force<T> f;
     int *cell, *slot, *count, *start, *tile_sum;
-    T *wx, *wy, *wz, *wtx, *wty, *wtz;
+    md::Vec4<T> *wr, *wtr;      // wall positions: cell order / caller's order
     int *wcell, *wslot, *wstart;
     uint8_t* wnear;
     md::EnergyOut eo;
@@ -110,7 +110,7 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     size_t n = (size_t)align_up((size_t)nv, 64);
     size_t m = (size_t)align_up((size_t)(nw > 0 ? nw : 1), 64);
     for (int b = 0; b < (cells ? 2 : 1); ++b) {
-        l.st[b].x = c.take<T>(n); l.st[b].y = c.take<T>(n); l.st[b].z = c.take<T>(n);
+        l.st[b].r = c.take<md::Vec4<T>>(n);
         l.st[b].vx = c.take<T>(n); l.st[b].vy = c.take<T>(n); l.st[b].vz = c.take<T>(n);
         l.st[b].id = c.take<int>(n);
     }
@@ -122,8 +122,8 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.count = c.take<int>(nc);
     l.start = c.take<int>(nc + 1);
     l.tile_sum = c.take<int>((size_t)cdiv((long long)nc, md::SCAN_TILE) + 1);
-    l.wx = c.take<T>(m); l.wy = c.take<T>(m); l.wz = c.take<T>(m);
-    l.wtx = c.take<T>(m); l.wty = c.take<T>(m); l.wtz = c.take<T>(m);
+    l.wr = c.take<md::Vec4<T>>(m);
+    l.wtr = c.take<md::Vec4<T>>(m);
     l.wcell = l.cell; l.wslot = l.slot;   // wall binning runs once, before the vapor's
     l.wstart = c.take<int>(nc + 1);
     l.wnear = c.take<uint8_t>(nc);
@@ -200,12 +200,17 @@ struct Sim : md_sim {
     template <bool ENERGY, bool KICK, bool COUNT>
     void launch_force()
     {
-        if (algo == MD_FORCE_CELLS)
-            md::k_force_cells<T, ENERGY, KICK, COUNT><<<blocks(128), 128, 0, stream>>>(p, l.st[cur], l.start, walls, l.f,
-                                                                                        l.eo, l.tests);
-        else
+        if (algo == MD_FORCE_CELLS) {
+            // ROWS lanes per particle: 9 in 3D (3 particles per warp), 3 in 2D (10 per warp)
+            if (dim == 3)
+                md::k_force_cells<T, 9, ENERGY, KICK, COUNT><<<cdiv(cdiv(p.nv, 3), 4), 128, 0, stream>>>(
+                    p, l.st[cur], l.start, walls, l.f, l.eo, l.tests);
+            else
+                md::k_force_cells<T, 3, ENERGY, KICK, COUNT><<<cdiv(cdiv(p.nv, 10), 4), 128, 0, stream>>>(
+                    p, l.st[cur], l.start, walls, l.f, l.eo, l.tests);
+        } else
             md::k_force_allpairs<T, ENERGY, KICK><<<blocks(md::AP_THREADS), md::AP_THREADS, 0, stream>>>(
-                p, l.st[cur], l.wtx, l.wty, l.wtz, l.f, l.eo);
+                p, l.st[cur], l.wtr, l.f, l.eo);
     }
 
     // One velocity-Verlet step: a1 -> a2 -> a3 + a4. `t` (optional) = events around each kernel.
@@ -350,7 +355,11 @@ struct Sim : md_sim {
         int rc = check_err_flag();
         if (rc) return rc;
         const md::State<T>& s = l.st[cur];
-        if (pos && (rc = export3(s.x, s.y, s.z, pos))) return rc;
+        if (pos) {
+            md::k_export_pos<T><<<blocks(256), 256, 0, stream>>>(p.nv, dim, s.id, s.r, l.stage0);
+            CK(cudaMemcpyAsync(pos, l.stage0, sizeof(double) * (size_t)p.nv * dim, cudaMemcpyDeviceToHost, stream));
+            CK(cudaStreamSynchronize(stream));
+        }
         if (vel && (rc = export3(s.vx, s.vy, s.vz, vel))) return rc;
         if (force && (rc = export3(l.f.fx, l.f.fy, l.f.fz, force))) return rc;
         if (pe) {
@@ -396,13 +405,12 @@ struct Sim : md_sim {
 namespace {
 
 template <typename T>
-__global__ void k_scatter_wall(int n, const T* sx, const T* sy, const T* sz, T* dx, T* dy, T* dz, const int* cell,
-                               const int* slot, const int* start)
+__global__ void k_scatter_wall(int n, const md::Vec4<T>* src, md::Vec4<T>* dst, const int* cell, const int* slot,
+                               const int* start)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    int d = start[cell[i]] + slot[i];
-    dx[d] = sx[i]; dy[d] = sy[i]; dz[d] = sz[i];
+    dst[start[cell[i]] + slot[i]] = src[i];
 }
 
 template <typename T>
@@ -412,7 +420,7 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
     // wall particles: upload, convert, and (cell mode) bin once -- they are never integrated
     if (nw > 0) {
         CK(cudaMemcpyAsync(l.wstage, wall, sizeof(double) * (size_t)nw * dim, cudaMemcpyHostToDevice, stream));
-        md::State<T> ws = {l.wtx, l.wty, l.wtz, nullptr, nullptr, nullptr, nullptr};
+        md::State<T> ws = {l.wtr, nullptr, nullptr, nullptr, nullptr};
         md::k_import<T><<<cdiv(nw, 256), 256, 0, stream>>>((int)nw, dim, l.wstage, nullptr, ws);
     }
     CK(cudaMemsetAsync(l.err, 0, 4 * sizeof(int), stream));
@@ -421,17 +429,16 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
         md::Params<T> pw = p;
         pw.nv = (int)nw;
         if (nw > 0) {
-            md::State<T> ws = {l.wtx, l.wty, l.wtz, nullptr, nullptr, nullptr, nullptr};
+            md::State<T> ws = {l.wtr, nullptr, nullptr, nullptr, nullptr};
             md::k_kick_drift_bin<T, false, true><<<cdiv(nw, 256), 256, 0, stream>>>(pw, ws, l.f, l.count, l.wcell,
                                                                                     l.wslot, l.err);
         }
         launch_scan(l.count, l.wstart);
         if (nw > 0)
-            k_scatter_wall<T><<<cdiv(nw, 256), 256, 0, stream>>>((int)nw, l.wtx, l.wty, l.wtz, l.wx, l.wy, l.wz,
-                                                                 l.wcell, l.wslot, l.wstart);
+            k_scatter_wall<T><<<cdiv(nw, 256), 256, 0, stream>>>((int)nw, l.wtr, l.wr, l.wcell, l.wslot, l.wstart);
         md::k_wall_near<T><<<cdiv(p.ncell, 256), 256, 0, stream>>>(p, l.wstart, l.wnear);
     }
-    walls.x = l.wx; walls.y = l.wy; walls.z = l.wz; walls.start = l.wstart; walls.near = l.wnear;
+    walls.r = l.wr; walls.start = l.wstart; walls.near = l.wnear;
     // vapor: upload, AoS -> SoA
     CK(cudaMemcpyAsync(l.stage0, pos, sizeof(double) * (size_t)nv * dim, cudaMemcpyHostToDevice, stream));
     CK(cudaMemcpyAsync(l.stage1, vel, sizeof(double) * (size_t)nv * dim, cudaMemcpyHostToDevice, stream));

@@ -25,10 +25,19 @@ struct Params {
     double mass;
 };
 
-// SoA particle state (a0). One of two ping-pong buffers; id = caller's original index.
+// Packed position: one 4-wide vector load per neighbour (w is spare; the cell path keeps the
+// path length since the last re-bin there).
+template <typename T>
+struct alignas(4 * sizeof(T)) Vec4 {
+    T x, y, z, w;
+};
+
+// Particle state (a0): positions packed (x, y, z, w), velocities SoA. One of two ping-pong
+// buffers; id = caller's original index.
 template <typename T>
 struct State {
-    T *x, *y, *z, *vx, *vy, *vz;
+    Vec4<T>* r;
+    T *vx, *vy, *vz;
     int* id;
 };
 
@@ -45,7 +54,7 @@ struct EnergyOut {
 
 template <typename T>
 struct Walls {
-    const T *x, *y, *z;       // sorted by cell
+    const Vec4<T>* r;         // sorted by cell
     const int* start;         // [ncell + 1]
     const uint8_t* near;      // [ncell]: any wall particle in the 3^d neighbourhood
 };
@@ -97,7 +106,8 @@ __global__ void __launch_bounds__(256) k_kick_drift_bin(Params<T> p, State<T> s,
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= p.nv) return;
-    T x = s.x[i], y = s.y[i], z = s.z[i];
+    Vec4<T> ri = s.r[i];
+    T x = ri.x, y = ri.y, z = ri.z;
     if (MOVE) {
         T vx = s.vx[i] + p.hk * f.fx[i];
         T vy = s.vy[i] + p.hk * f.fy[i];
@@ -108,7 +118,8 @@ __global__ void __launch_bounds__(256) k_kick_drift_bin(Params<T> p, State<T> s,
         boundary(x, vx, p.L[0], p.bc[0], err);
         boundary(y, vy, p.L[1], p.bc[1], err);
         boundary(z, vz, p.L[2], p.bc[2], err);
-        s.x[i] = x; s.y[i] = y; s.z[i] = z;
+        ri.x = x; ri.y = y; ri.z = z;
+        s.r[i] = ri;
         s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz;
     }
     if (BIN) {
@@ -218,7 +229,7 @@ __global__ void __launch_bounds__(256) k_scatter(int nv, State<T> src, State<T> 
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= nv) return;
     int d = start[cell[i]] + slot[i];
-    dst.x[d] = src.x[i]; dst.y[d] = src.y[i]; dst.z[d] = src.z[i];
+    dst.r[d] = src.r[i];
     dst.vx[d] = src.vx[i]; dst.vy[d] = src.vy[i]; dst.vz[d] = src.vz[i];
     dst.id[d] = src.id[i];
     if (with_force) { fdst.fx[d] = fsrc.fx[i]; fdst.fy[d] = fsrc.fy[i]; fdst.fz[d] = fsrc.fz[i]; }
@@ -257,77 +268,117 @@ __device__ __forceinline__ void pair_term(T dx, T dy, T dz, T rc2, T sig2, T e24
     }
 }
 
-// Variant B: cell-list traversal, one thread per particle in cell order.  The three cells
-// (cx-1, cx, cx+1) of one (cy+ky, cz+kz) row are contiguous in cell order, so a row is ONE
-// contiguous j range (plus one wrapped cell at a periodic x face); images are applied by
-// shifting r_i once per row/segment instead of a per-pair rint.
-template <typename T, bool ENERGY, bool KICK, bool COUNT>
+// Variant B: cell-list traversal.  ROWS = 3^(d-1) lanes cooperate on one particle: lane `row` walks the
+// cell row (cy+ky, cz+kz), whose three cells (cx-1, cx, cx+1) are contiguous in cell order, so a row is
+// ONE contiguous j range (plus one wrapped cell at a periodic x face).  Images are applied by shifting
+// r_i once per row/segment instead of a per-pair rint.  The ROWS partial sums are combined with warp
+// shuffles in a fixed tree and the leader lane stores f_i and applies the second half-kick (a4).
+// A warp holds 32 / ROWS particles (3 in 3D, 10 in 2D); short dependent chains and 9x the warps of a
+// thread-per-particle walk are what hide the L2 latency at N ~ 1e5 (profiles/r01_v1_cfg2.md).
+template <typename T, bool ENERGY>
+__device__ __forceinline__ void row_range(const Vec4<T>* __restrict__ r, int jb, int je, int skip, T xe, T ye, T ze,
+                                          T xj0, T yjs, T zjs, T rc2, T sig2, T e24, T e4, T uc, Acc<T, ENERGY>& a)
+{
+    constexpr bool TWO_SIDED = sizeof(T) == 4;
+    for (int j = jb; j < je; j += 2) {
+        const int j1 = min(j + 1, je - 1);
+        const Vec4<T> a0 = r[j], a1 = r[j1];           // two independent loads in flight
+        if (j != skip) {
+            if (TWO_SIDED) pair_term<T, ENERGY>(xe - (a0.x - xj0), ye - (a0.y - yjs), ze - (a0.z - zjs), rc2, sig2, e24, e4, uc, a);
+            else pair_term<T, ENERGY>(xe - a0.x, ye - a0.y, ze - a0.z, rc2, sig2, e24, e4, uc, a);
+        }
+        if (j1 != j && j1 != skip) {
+            if (TWO_SIDED) pair_term<T, ENERGY>(xe - (a1.x - xj0), ye - (a1.y - yjs), ze - (a1.z - zjs), rc2, sig2, e24, e4, uc, a);
+            else pair_term<T, ENERGY>(xe - a1.x, ye - a1.y, ze - a1.z, rc2, sig2, e24, e4, uc, a);
+        }
+    }
+}
+
+template <int ROWS, typename V>
+__device__ __forceinline__ V rows_sum(V v, int row)
+{
+    constexpr int TOP = ROWS > 4 ? 8 : 2;    // largest power of two below ROWS (9 -> 8, 3 -> 2)
+#pragma unroll
+    for (int off = TOP; off > 0; off >>= 1) {
+        V o = __shfl_down_sync(0xffffffffu, v, off);
+        if (row < off && row + off < ROWS) v += o;
+    }
+    return v;
+}
+
+template <typename T, int ROWS, bool ENERGY, bool KICK, bool COUNT>
 __global__ void __launch_bounds__(128) k_force_cells(Params<T> p, State<T> s, const int* __restrict__ start,
                                                      Walls<T> w, Force<T> f, EnergyOut eo,
                                                      unsigned long long* __restrict__ tests)
 {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= p.nv) return;
-    const T xi = s.x[i], yi = s.y[i], zi = s.z[i];
-    int cx, cy, cz;
-    const int ci = cell_index(p, xi, yi, zi, cx, cy, cz);
-    Acc<T, ENERGY> av, aw;
-    const bool do_wall = p.nw > 0 && w.near[ci];
-    const int nx = p.nc[0], ny = p.nc[1], nz = p.nc[2];
-    const int x0 = max(cx - 1, 0), x1 = min(cx + 1, nx - 1);
-    // Image shifts.  fp64: r_i is shifted (+-L) once per row.  fp32: the shift is put on whichever side
-    // sits at the top of the box (r - L is exact there), so that d keeps full relative precision.
+    constexpr int PPW = 32 / ROWS;
     constexpr bool TWO_SIDED = sizeof(T) == 4;
-    int xw = -1;          // wrapped extra cell in x
-    T xs = T(0), xjs = T(0);
-    if (p.bc[0] == BC_PERIODIC) {
-        if (cx == 0) { xw = nx - 1; if (TWO_SIDED) xjs = p.L[0]; else xs = p.L[0]; }
-        else if (cx == nx - 1) { xw = 0; xs = -p.L[0]; }
-    }
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int pl = lane / ROWS, row = lane - pl * ROWS;
+    const int i = warp * PPW + pl;
+    const bool active = pl < PPW && i < p.nv;
+    Acc<T, ENERGY> av, aw;
     long long nt = 0;
-    for (int kz = -1; kz <= 1; ++kz) {
-        int qz = cz + kz;
-        T ze = zi, zjs = T(0);
-        if (qz < 0) { if (p.bc[2] != BC_PERIODIC) continue; qz += nz; if (TWO_SIDED) zjs = p.L[2]; else ze = zi + p.L[2]; }
-        else if (qz >= nz) { if (p.bc[2] != BC_PERIODIC) continue; qz -= nz; ze = zi - p.L[2]; }
-        for (int ky = -1; ky <= 1; ++ky) {
-            int qy = cy + ky;
-            T ye = yi, yjs = T(0);
-            if (qy < 0) { if (p.bc[1] != BC_PERIODIC) continue; qy += ny; if (TWO_SIDED) yjs = p.L[1]; else ye = yi + p.L[1]; }
-            else if (qy >= ny) { if (p.bc[1] != BC_PERIODIC) continue; qy -= ny; ye = yi - p.L[1]; }
-            const int row = (qz * ny + qy) * nx;
-            for (int seg = 0; seg < 2; ++seg) {
-                int c0, c1;
-                T xe, xj0 = T(0);
-                if (seg == 0) { c0 = row + x0; c1 = row + x1; xe = xi; }
-                else { if (xw < 0) break; c0 = c1 = row + xw; xe = xi + xs; xj0 = xjs; }
-                int jb = start[c0], je = start[c1 + 1];
-                for (int j = jb; j < je; ++j) {
-                    if (j == i) continue;
-                    if (TWO_SIDED)
-                        pair_term<T, ENERGY>(xe - (s.x[j] - xj0), ye - (s.y[j] - yjs), ze - (s.z[j] - zjs), p.rc2,
-                                             p.sig2_vv, p.e24_vv, p.e4_vv, p.uc_vv, av);
-                    else
-                        pair_term<T, ENERGY>(xe - s.x[j], ye - s.y[j], ze - s.z[j], p.rc2, p.sig2_vv, p.e24_vv,
-                                             p.e4_vv, p.uc_vv, av);
-                }
-                if (COUNT) nt += (je - jb) - ((i >= jb && i < je) ? 1 : 0);
-                if (do_wall) {
-                    int wb = w.start[c0], we = w.start[c1 + 1];
-                    for (int j = wb; j < we; ++j) {
-                        if (TWO_SIDED)
-                            pair_term<T, ENERGY>(xe - (w.x[j] - xj0), ye - (w.y[j] - yjs), ze - (w.z[j] - zjs), p.rc2,
-                                                 p.sig2_vw, p.e24_vw, p.e4_vw, p.uc_vw, aw);
-                        else
-                            pair_term<T, ENERGY>(xe - w.x[j], ye - w.y[j], ze - w.z[j], p.rc2, p.sig2_vw, p.e24_vw,
-                                                 p.e4_vw, p.uc_vw, aw);
-                    }
-                    if (COUNT) nt += we - wb;
-                }
+    if (active) {
+        const Vec4<T> ri = s.r[i];
+        int cx, cy, cz;
+        const int ci = cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
+        const int nx = p.nc[0], ny = p.nc[1], nz = p.nc[2];
+        const int ky = row % 3 - 1, kz = ROWS == 9 ? row / 3 - 1 : 0;
+        int qy = cy + ky, qz = cz + kz;
+        T ye = ri.y, ze = ri.z, yjs = T(0), zjs = T(0);
+        bool ok = true;
+        // image shifts: fp64 shifts r_i by +-L; fp32 puts the shift on whichever side sits at the top of
+        // the box (r - L is exact there) so that d keeps full relative precision
+        if (qz < 0) { ok = p.bc[2] == BC_PERIODIC; qz += nz; if (TWO_SIDED) zjs = p.L[2]; else ze += p.L[2]; }
+        else if (qz >= nz) { ok = p.bc[2] == BC_PERIODIC; qz -= nz; ze -= p.L[2]; }
+        if (qy < 0) { ok = ok && p.bc[1] == BC_PERIODIC; qy += ny; if (TWO_SIDED) yjs = p.L[1]; else ye += p.L[1]; }
+        else if (qy >= ny) { ok = ok && p.bc[1] == BC_PERIODIC; qy -= ny; ye -= p.L[1]; }
+        if (ok) {
+            const int rowc = (qz * ny + qy) * nx;
+            const int x0 = max(cx - 1, 0), x1 = min(cx + 1, nx - 1);
+            int xw = -1;
+            T xs = T(0), xjs = T(0);
+            if (p.bc[0] == BC_PERIODIC) {
+                if (cx == 0) { xw = nx - 1; if (TWO_SIDED) xjs = p.L[0]; else xs = p.L[0]; }
+                else if (cx == nx - 1) { xw = 0; xs = -p.L[0]; }
+            }
+            const bool do_wall = p.nw > 0 && w.near[ci];
+            // all cell-start loads first (independent), then the particle loops
+            const int jb = start[rowc + x0], je = start[rowc + x1 + 1];
+            int jb2 = 0, je2 = 0, wb = 0, we = 0, wb2 = 0, we2 = 0;
+            if (xw >= 0) { jb2 = start[rowc + xw]; je2 = start[rowc + xw + 1]; }
+            if (do_wall) {
+                wb = w.start[rowc + x0]; we = w.start[rowc + x1 + 1];
+                if (xw >= 0) { wb2 = w.start[rowc + xw]; we2 = w.start[rowc + xw + 1]; }
+            }
+            row_range<T, ENERGY>(s.r, jb, je, i, ri.x, ye, ze, T(0), yjs, zjs, p.rc2, p.sig2_vv, p.e24_vv, p.e4_vv,
+                                 p.uc_vv, av);
+            row_range<T, ENERGY>(s.r, jb2, je2, i, ri.x + xs, ye, ze, xjs, yjs, zjs, p.rc2, p.sig2_vv, p.e24_vv,
+                                 p.e4_vv, p.uc_vv, av);
+            row_range<T, ENERGY>(w.r, wb, we, -1, ri.x, ye, ze, T(0), yjs, zjs, p.rc2, p.sig2_vw, p.e24_vw, p.e4_vw,
+                                 p.uc_vw, aw);
+            row_range<T, ENERGY>(w.r, wb2, we2, -1, ri.x + xs, ye, ze, xjs, yjs, zjs, p.rc2, p.sig2_vw, p.e24_vw,
+                                 p.e4_vw, p.uc_vw, aw);
+            if (COUNT) {
+                nt = (je - jb) + (je2 - jb2) + (we - wb) + (we2 - wb2);
+                if ((i >= jb && i < je) || (i >= jb2 && i < je2)) nt -= 1;
             }
         }
     }
-    const T fx = av.fx + aw.fx, fy = av.fy + aw.fy, fz = av.fz + aw.fz;
+    const T fx = rows_sum<ROWS>(av.fx + aw.fx, row);
+    const T fy = rows_sum<ROWS>(av.fy + aw.fy, row);
+    const T fz = rows_sum<ROWS>(av.fz + aw.fz, row);
+    double uv = 0, uw = 0, wv = 0, ww = 0;
+    int cv = 0, cw = 0;
+    if (ENERGY) {
+        uv = rows_sum<ROWS>(av.u, row); uw = rows_sum<ROWS>(aw.u, row);
+        wv = rows_sum<ROWS>(av.w, row); ww = rows_sum<ROWS>(aw.w, row);
+        cv = rows_sum<ROWS>(av.c, row); cw = rows_sum<ROWS>(aw.c, row);
+    }
+    if (COUNT) nt = rows_sum<ROWS>(nt, row);
+    if (!active || row != 0) return;
     f.fx[i] = fx; f.fy[i] = fy; f.fz[i] = fz;
     if (KICK) {   // a4: second half-kick (paper's F3)
         s.vx[i] = s.vx[i] + p.hk * fx;
@@ -335,11 +386,11 @@ __global__ void __launch_bounds__(128) k_force_cells(Params<T> p, State<T> s, co
         s.vz[i] = s.vz[i] + p.hk * fz;
     }
     if (ENERGY) {
-        eo.pe[i] = 0.5 * av.u + aw.u;
-        eo.pew[i] = aw.u;
-        eo.vir[i] = 0.5 * av.w + aw.w;
-        eo.cvv[i] = av.c;
-        eo.cvw[i] = aw.c;
+        eo.pe[i] = 0.5 * uv + uw;
+        eo.pew[i] = uw;
+        eo.vir[i] = 0.5 * wv + ww;
+        eo.cvv[i] = cv;
+        eo.cvw[i] = cw;
     }
     if (COUNT) atomicAdd(tests, (unsigned long long)nt);
 }
@@ -361,25 +412,25 @@ __device__ __forceinline__ float min_image(float a, float b, float d, float L, f
 constexpr int AP_THREADS = 128;
 
 template <typename T, bool ENERGY, bool KICK>
-__global__ void __launch_bounds__(AP_THREADS) k_force_allpairs(Params<T> p, State<T> s, const T* __restrict__ wx,
-                                                               const T* __restrict__ wy, const T* __restrict__ wz,
-                                                               Force<T> f, EnergyOut eo)
+__global__ void __launch_bounds__(AP_THREADS) k_force_allpairs(Params<T> p, State<T> s,
+                                                               const Vec4<T>* __restrict__ wr, Force<T> f,
+                                                               EnergyOut eo)
 {
     __shared__ T sx[AP_THREADS], sy[AP_THREADS], sz[AP_THREADS];
     const int i = blockIdx.x * AP_THREADS + threadIdx.x;
     const bool live = i < p.nv;
-    const T xi = live ? s.x[i] : T(0), yi = live ? s.y[i] : T(0), zi = live ? s.z[i] : T(0);
+    Vec4<T> ri = {T(0), T(0), T(0), T(0)};
+    if (live) ri = s.r[i];
+    const T xi = ri.x, yi = ri.y, zi = ri.z;
     const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
     Acc<T, ENERGY> av, aw;
     for (int pass = 0; pass < 2; ++pass) {
         const int n = pass == 0 ? p.nv : p.nw;
-        const T* jx = pass == 0 ? s.x : wx;
-        const T* jy = pass == 0 ? s.y : wy;
-        const T* jz = pass == 0 ? s.z : wz;
+        const Vec4<T>* jr = pass == 0 ? s.r : wr;
         for (int t0 = 0; t0 < n; t0 += AP_THREADS) {
             int j = t0 + threadIdx.x;
             __syncthreads();
-            if (j < n) { sx[threadIdx.x] = jx[j]; sy[threadIdx.x] = jy[j]; sz[threadIdx.x] = jz[j]; }
+            if (j < n) { Vec4<T> q = jr[j]; sx[threadIdx.x] = q.x; sy[threadIdx.x] = q.y; sz[threadIdx.x] = q.z; }
             __syncthreads();
             const int m = min(AP_THREADS, n - t0);
 #pragma unroll 4
@@ -421,9 +472,12 @@ __global__ void k_import(int n, int dim, const double* __restrict__ pos, const d
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    s.x[i] = (T)pos[i * dim];
-    s.y[i] = (T)pos[i * dim + 1];
-    s.z[i] = dim == 3 ? (T)pos[i * dim + 2] : T(0);
+    Vec4<T> r;
+    r.x = (T)pos[i * dim];
+    r.y = (T)pos[i * dim + 1];
+    r.z = dim == 3 ? (T)pos[i * dim + 2] : T(0);
+    r.w = T(0);
+    s.r[i] = r;
     if (vel) {
         s.vx[i] = (T)vel[i * dim];
         s.vy[i] = (T)vel[i * dim + 1];
@@ -449,6 +503,20 @@ __global__ void k_export1(int n, const int* __restrict__ id, const double* __res
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) out[id[i]] = a[i];
+}
+
+// out[id[i]][0..dim) = r[i].xyz
+template <typename T>
+__global__ void k_export_pos(int n, int dim, const int* __restrict__ id, const Vec4<T>* __restrict__ r,
+                             double* __restrict__ out)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    size_t o = (size_t)id[i] * dim;
+    Vec4<T> v = r[i];
+    out[o] = (double)v.x;
+    out[o + 1] = (double)v.y;
+    if (dim == 3) out[o + 2] = (double)v.z;
 }
 
 // near[c] = 1 if any of the 3^d neighbour cells of c (same wrap / drop rule as the force
