@@ -26,6 +26,7 @@ sys.path.insert(0, ROOT)
 
 METRIC = "pair-interactions/s"
 WORKLOAD = "cfg2_cyl3d_64k: 3D cylindrical pore, 65536 vapor + 1240 wall particles, 110^3 box, fp64, cell list"
+ALGO = "auto"      # resolves to the persistent Verlet-list kernel on this workload (md.h: MD_FORCE_AUTO)
 
 
 def peaks_file():
@@ -160,7 +161,7 @@ def run_ours(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
     # ---------------- device-resident arm -------------------------------------------------
-    sim = md.Simulation(cfg, algo="cells", device=dev)
+    sim = md.Simulation(cfg, algo=ALGO, device=dev)
     info = sim.info()
     for _ in range(args.warmup):
         sim.step(inner)
@@ -185,7 +186,8 @@ def run_ours(args):
     inter_all = sum_over_ranks(inter)
     value = inter_all / t_dev
     steps_per_s = args.steps * inner / t_dev                        # per replica (all replicas advance together)
-    launches = args.steps * (inner * info["kernels_per_step"] + 3)
+    persistent = info["algo"] == "verlet"
+    launches = args.steps * ((1 if persistent else inner * info["kernels_per_step"]) + 3)
 
     # ---------------- end-to-end arm: host arrays in, host arrays out, through the C ABI ----
     host = {k: torch.from_numpy(np.ascontiguousarray(cfg[k])).pin_memory().numpy() for k in ("pos", "vel", "wall")}
@@ -193,11 +195,11 @@ def run_ours(args):
     ecfg.update(host)
     stream = torch.cuda.Stream(device=dev)
     e2e_inter = 0.0
-    md.Simulation(ecfg, algo="cells", device=dev, stream=stream).close()
+    md.Simulation(ecfg, algo=ALGO, device=dev, stream=stream).close()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        s2 = md.Simulation(ecfg, algo="cells", device=dev, stream=stream)    # H2D of pos, vel, wall
+        s2 = md.Simulation(ecfg, algo=ALGO, device=dev, stream=stream)    # H2D of pos, vel, wall
         s2.step(inner)
         st = s2.get_state(force=False, pe=False)                              # D2H of pos, vel
         e = s2.energy()
@@ -215,25 +217,52 @@ def run_ours(args):
         return
 
     # ---------------- roofline of the dominant kernel, measured live (rank 0) --------------
-    prof_steps = 200
-    sim.profile_step(20)
-    kt = sim.profile_step(prof_steps)
-    names = ["kick_drift_bin", "scan", "scatter", "force_kick"]
-    shares = {n: kt["ms"][k] / max(kt["total_ms"], 1e-12) for k, n in enumerate(names)}
-    top = max(range(4), key=lambda k: kt["ms"][k])
-    ncell = int(np.prod(info["n_cells"]))
-    # algorithmic bytes per launch: fp64, 3D
-    alg_bytes = {0: 120 * nv + 8 * nv, 1: 12 * ncell, 2: (52 + 52 + 8) * nv + 4 * ncell, 3: 96 * nv + 4 * (ncell + 1)}
-    t_top = kt["ms"][top] * 1e-3 / kt["launches"][top]
     pk, pk_src = peaks_file()
-    achieved = alg_bytes[top] / t_top * 1e-9
-    roofline = {"kernel": names[top], "bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / pk["hbm_gbs"], "traffic": None, "peak_source": pk_src + " (MEASURED_PEAKS.json hbm_gbs)",
-                "algorithmic_bytes_per_launch": alg_bytes[top], "us_per_launch": t_top * 1e6,
-                "kernel_share_of_step": shares, "note": "state (4.7 MB) is L2-resident: the kernel is latency/L2 "
-                "bound, far below the HBM roofline by construction (DESIGN.md)"}
     tests = sim.pair_tests()
+    ncell = int(np.prod(info["n_cells"]))
+    if persistent:
+        # one launch = prof_steps time steps of k_md_run (force from the list + both half-kicks + drift, and the
+        # in-kernel re-bin / list rebuilds); algorithmic bytes per particle-step, fp64:
+        # r 32 + v 24 read, r' 32 + v' 24 + f 24 written, list count 4 + 4 per list entry read
+        prof_steps = 2000
+        sim.profile_step(200)
+        kt = sim.profile_step(prof_steps)
+        per_step = nv * (136 + 4) + 4 * tests
+        top_name, t_top, alg = "k_md_run (persistent: %d time steps per launch)" % prof_steps, kt["ms"][3] * 1e-3, per_step * prof_steps
+        shares = {"k_md_run": 1.0}
+        extra = {"time_steps_per_launch": prof_steps, "rebuilds_in_launch": kt["rebuilds"],
+                 "us_per_time_step": kt["ms"][3] * 1e3 / prof_steps}
+    else:
+        prof_steps = 200
+        sim.profile_step(20)
+        kt = sim.profile_step(prof_steps)
+        names = ["kick_drift_bin", "scan", "scatter", "force_kick"]
+        shares = {n: kt["ms"][k] / max(kt["total_ms"], 1e-12) for k, n in enumerate(names)}
+        top = max(range(4), key=lambda k: kt["ms"][k])
+        alg_bytes = {0: 144 * nv, 1: 12 * ncell, 2: 128 * nv + 4 * ncell, 3: 104 * nv + 4 * (ncell + 1)}
+        top_name, t_top, alg = names[top], kt["ms"][top] * 1e-3 / kt["launches"][top], alg_bytes[top]
+        extra = {}
+    achieved = alg / t_top * 1e-9
+    roofline = {"kernel": top_name, "bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / pk["hbm_gbs"], "traffic": None, "peak_source": pk_src + " (MEASURED_PEAKS.json hbm_gbs)",
+                "algorithmic_bytes_per_launch": alg, "us_per_launch": t_top * 1e6, "kernel_share_of_step": shares,
+                "note": "the 4.7 MB state is L2-resident across time steps, so the step is bound by L2 latency and the "
+                        "grid barrier, not by HBM: a low fraction here is expected (DESIGN.md)"}
+    roofline.update(extra)
     sim.close()
+
+    # the counting-sort cell path rebuilt every step (MD_FORCE_CELLS), same workload, for comparison
+    sim_c = md.Simulation(cfg, algo="cells", device=dev)
+    sim_c.step(64)
+    sim_c.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(sim_c.stream)
+    sim_c.step(512)
+    e1.record(sim_c.stream)
+    sim_c.synchronize()
+    cells_path = {"md_steps_per_s": 512 / (e0.elapsed_time(e1) * 1e-3), "pair_tests_per_timestep": sim_c.pair_tests(),
+                  "kernels_per_step": sim_c.info()["kernels_per_step"]}
+    sim_c.close()
 
     # FP64 roofline of the all-pairs force kernel at the same N (north_star: % of FP64 peak, measured in the same run)
     peaks = md.measure_peaks(device=dev)
@@ -267,7 +296,8 @@ def run_ours(args):
             "pair_tests_per_s": tests * steps_per_s * world, "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": 1e3 * t_e2e / args.steps},
-            "gpu_launches": launches, "roofline": roofline, "roofline_allpairs_fp64": allpairs,
+            "gpu_launches": launches, "roofline": roofline, "cells_every_step_path": cells_path,
+            "roofline_allpairs_fp64": allpairs,
             "measured_peaks_this_run": peaks, "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:

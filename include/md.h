@@ -44,7 +44,7 @@ typedef struct md_sim md_sim; /* opaque */
 enum { MD_OK = 0, MD_ERR_INVALID_ARG = -1, MD_ERR_UNSUPPORTED = -2, MD_ERR_CUDA = -3,
        MD_ERR_WORKSPACE = -4, MD_ERR_NONFINITE = -5, MD_ERR_STATE = -6 };
 enum { MD_BC_PERIODIC = 0, MD_BC_REFLECT = 1 };
-enum { MD_FORCE_AUTO = 0, MD_FORCE_ALLPAIRS = 1, MD_FORCE_CELLS = 2 };
+enum { MD_FORCE_AUTO = 0, MD_FORCE_ALLPAIRS = 1, MD_FORCE_CELLS = 2, MD_FORCE_VERLET = 3 };
 enum { MD_PORE_NONE = 0, MD_PORE_SLIT, MD_PORE_CYLINDER, MD_PORE_CONE, MD_PORE_INKBOTTLE, MD_PORE_PRISM };
 
 /* Simulation box [0, len[d]] per dimension; dim = 2 or 3 (len[2], bc[2] ignored in 2D).
@@ -61,8 +61,15 @@ typedef struct { int kind, axis; double center[3], length, r0, r1, neck_len, wid
 typedef struct { double eps, sigma, eps_w, sigma_w, r_cut; int shift_energy; } md_lj;
 
 /* dt > 0, mass > 0 (one mass for all vapor particles); precision 64 or 32 (state and pair
- * arithmetic type; K and U are always reduced in fp64); force_algo one of MD_FORCE_*. */
-typedef struct { double dt, mass; int precision, force_algo; } md_opts;
+ * arithmetic type; K and U are always reduced in fp64); force_algo one of MD_FORCE_*:
+ *   ALLPAIRS  shared-memory-tiled all-pairs (small N);
+ *   CELLS     counting-sort cell list rebuilt every step, neighbour-cell traversal;
+ *   VERLET    the same cell list, rebuilt only when a particle's path since the last rebuild exceeds
+ *             skin/2, cached as a neighbour list of all pairs within r_cut + skin (exact: no pair
+ *             within r_cut is ever missed); the whole md_step batch is one persistent launch;
+ *   AUTO      VERLET when the grid allows it and n_vapor >= 2048, else CELLS, else ALLPAIRS.
+ * skin >= 0 is the VERLET list margin in length units; 0 selects the default 0.16 r_cut. */
+typedef struct { double dt, mass; int precision, force_algo; double skin; } md_opts;
 
 /* potential = potential_vv + potential_vw = sum_i pe_i; virial = sum over unordered vv pairs and
  * vw pairs of g.d (g = force on the vapor particle, d = r_i - r_j); pairs_* = pairs with r < r_cut. */
@@ -70,8 +77,9 @@ typedef struct { double kinetic, potential, potential_vv, potential_vw, virial;
                  long long pairs_vv, pairs_vw; long long step; } md_energy_out;
 
 /* Per-kernel device times of md_profile_step, milliseconds summed over the profiled steps, and
- * launch counts.  Index: 0 kick+drift(+bin count), 1 scan, 2 scatter, 3 force(+half-kick). */
-typedef struct { double ms[4]; long long launches[4]; double total_ms; long long steps; } md_kernel_times;
+ * launch counts.  Index: 0 kick+drift(+bin count), 1 scan, 2 scatter, 3 force(+half-kick).  VERLET: the
+ * whole batch is one launch, reported in slot 3; rebuilds = cell-list + neighbour-list rebuilds in it. */
+typedef struct { double ms[4]; long long launches[4]; double total_ms; long long steps, rebuilds; } md_kernel_times;
 
 /* Peak micro-benchmarks run on the caller's stream (TFLOP/s count FMA = 2 flops; GB/s = read+write). */
 typedef struct { double fp64_tflops, fp32_tflops, copy_gbs; } md_peaks;
@@ -96,7 +104,8 @@ int md_step(md_sim*, long long n_steps);
 
 /* Copies the state at the current step to host buffers (each may be NULL = skip):
  * pos, vel, force [n_vapor][dim]; pe [n_vapor] (pe_i = 1/2 sum_j u_vv + sum_w u_vw); *step.
- * MD_ERR_STATE if a particle left a reflecting box (more than one bounce in a step). */
+ * MD_ERR_STATE if a particle left a reflecting box (more than one bounce in a step);
+ * MD_ERR_WORKSPACE if a VERLET neighbour list overflowed its 128 entries per particle. */
 int md_get_state(md_sim*, double* pos, double* vel, double* force, double* pe, long long* step);
 
 /* Kinetic / potential energies, virial and pair counts at the current step (host struct).

@@ -2,6 +2,7 @@
 // Host logic only: validation, workspace carving, launch order, CUDA graphs.
 #include "../../include/md.h"
 #include "md_kernels.cuh"
+#include "md_verlet.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -65,7 +66,8 @@ const char* validate(const md_box* box, const md_lj* lj, const md_opts* o, long 
     if (!(o->dt > 0) || !std::isfinite(o->dt)) return "dt must be > 0";
     if (!(o->mass > 0) || !std::isfinite(o->mass)) return "mass must be > 0";
     if (o->precision != 64 && o->precision != 32) return "precision must be 64 or 32";
-    if (o->force_algo < MD_FORCE_AUTO || o->force_algo > MD_FORCE_CELLS) return "unknown force_algo";
+    if (o->force_algo < MD_FORCE_AUTO || o->force_algo > MD_FORCE_VERLET) return "unknown force_algo";
+    if (!(o->skin >= 0) || !std::isfinite(o->skin)) return "skin must be >= 0";
     if (!(lj->r_cut > 0) || !std::isfinite(lj->r_cut)) return "r_cut must be > 0";
     if (!(lj->sigma > 0) || !(lj->sigma_w > 0)) return "sigma, sigma_w must be > 0";
     if (!std::isfinite(lj->eps) || !std::isfinite(lj->eps_w)) return "eps, eps_w must be finite";
@@ -78,11 +80,30 @@ const char* validate(const md_box* box, const md_lj* lj, const md_opts* o, long 
     return nullptr;
 }
 
-int pick_algo(const md_opts& o, const GridSpec& g, long long nv)
+double list_skin(const md_lj& lj, const md_opts& o) { return o.skin > 0 ? o.skin : 0.16 * lj.r_cut; }
+
+// Grid the handle uses: cells of side >= r_cut (CELLS) or >= r_cut + skin (VERLET).
+GridSpec grid_for(const md_box& box, const md_lj& lj, const md_opts& o, int algo)
 {
+    return make_grid(box, algo == MD_FORCE_VERLET ? lj.r_cut + list_skin(lj, o) : lj.r_cut);
+}
+
+bool verlet_ok(const md_box& box, const md_lj& lj, const md_opts& o, long long nv, long long nw)
+{
+    const double rl = lj.r_cut + list_skin(lj, o);
+    for (int a = 0; a < box.dim; ++a)
+        if (box.bc[a] == MD_BC_PERIODIC && box.len[a] <= 2.0 * rl) return false;
+    return make_grid(box, rl).cells_ok && nv + nw < (1ll << 30);
+}
+
+int pick_algo(const md_box& box, const md_lj& lj, const md_opts& o, long long nv, long long nw)
+{
+    const bool cells_ok = make_grid(box, lj.r_cut).cells_ok;
     if (o.force_algo == MD_FORCE_ALLPAIRS) return MD_FORCE_ALLPAIRS;
-    if (o.force_algo == MD_FORCE_CELLS) return g.cells_ok ? MD_FORCE_CELLS : -1;
-    return (g.cells_ok && nv >= 2048) ? MD_FORCE_CELLS : MD_FORCE_ALLPAIRS;
+    if (o.force_algo == MD_FORCE_CELLS) return cells_ok ? MD_FORCE_CELLS : -1;
+    if (o.force_algo == MD_FORCE_VERLET) return verlet_ok(box, lj, o, nv, nw) ? MD_FORCE_VERLET : -1;
+    if (nv >= 2048 && verlet_ok(box, lj, o, nv, nw)) return MD_FORCE_VERLET;
+    return (cells_ok && nv >= 2048) ? MD_FORCE_CELLS : MD_FORCE_ALLPAIRS;
 }
 
 template <typename T>
@@ -98,19 +119,21 @@ struct Layout {
     int* err;
     unsigned long long* tests;
     double *stage0, *stage1, *wstage;
+    int *nbr, *ncnt, *vflags;   // VERLET: neighbour list, counts, flags
     int red_blocks;
     size_t bytes;
 };
 
 template <typename T>
-Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell, bool cells)
+Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell, int algo)
 {
     Layout<T> l;
     Carver c(base);
+    const bool cells = algo != MD_FORCE_ALLPAIRS, verlet = algo == MD_FORCE_VERLET;
     size_t n = (size_t)align_up((size_t)nv, 64);
     size_t m = (size_t)align_up((size_t)(nw > 0 ? nw : 1), 64);
     for (int b = 0; b < (cells ? 2 : 1); ++b) {
-        l.st[b].r = c.take<md::Vec4<T>>(n);
+        l.st[b].r = c.take<md::Vec4<T>>(verlet ? n + m : n);   // VERLET: walls appended at [nv, nv + nw)
         l.st[b].vx = c.take<T>(n); l.st[b].vy = c.take<T>(n); l.st[b].vz = c.take<T>(n);
         l.st[b].id = c.take<int>(n);
     }
@@ -134,6 +157,9 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.eout = c.take<double>(8);
     l.err = c.take<int>(4);
     l.tests = c.take<unsigned long long>(2);
+    l.nbr = c.take<int>(verlet ? (size_t)nv * md::VL_MAXN : 1);
+    l.ncnt = c.take<int>(verlet ? n : 1);
+    l.vflags = c.take<int>(md::VF_COUNT);
     l.stage0 = c.take<double>(n * dim);
     l.stage1 = c.take<double>(n * dim);
     l.wstage = c.take<double>(m * dim);
@@ -177,6 +203,54 @@ struct Sim : md_sim {
     static constexpr int CHUNK = 16;
     cudaEvent_t ev[5] = {};
     double e_host[6];
+    // VERLET (persistent kernel): device-side buffer parities are mirrored here by refresh()
+    md::Verlet<T> vl;
+    int curv = 0, coop_grid = 0;
+    long long rebuilds_seen = 0;
+
+    bool verlet() const { return algo == MD_FORCE_VERLET; }
+
+    // Particle state as the post-processing kernels see it (positions from `cur`, the rest from `curv`).
+    md::State<T> view() const
+    {
+        md::State<T> s = l.st[verlet() ? curv : cur];
+        s.r = l.st[cur].r;
+        return s;
+    }
+
+    int launch_run(long long n, int force_rebuild)
+    {
+        void* kernel = dim == 3 ? (void*)md::k_md_run<T, 9> : (void*)md::k_md_run<T, 3>;
+        if (!coop_grid) {
+            int dev = 0, sms = 0, coop = 0, nb = 0;
+            CK(cudaGetDevice(&dev));
+            CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+            if (!coop) { err = "device does not support cooperative launches"; return MD_ERR_UNSUPPORTED; }
+            CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, md::VL_THREADS, 0));
+            if (nb < 1) { err = "persistent kernel does not fit on an SM"; return MD_ERR_CUDA; }
+            const int want = cdiv((long long)p.nv * md::VL_G, md::VL_THREADS);
+            coop_grid = std::max(1, std::min(nb * sms, want));
+        }
+        CK(cudaMemsetAsync(l.vflags + md::VF_REQ0, 0, 3 * sizeof(int), stream));   // rebuild-request slots
+        void* args[] = {(void*)&p, (void*)&vl, (void*)&n, (void*)&force_rebuild};
+        CK(cudaLaunchCooperativeKernel(kernel, dim3(coop_grid), dim3(md::VL_THREADS), args, 0, stream));
+        return MD_OK;
+    }
+
+    // Synchronises and mirrors the persistent kernel's flags; reports its error flags.
+    int refresh()
+    {
+        if (!verlet()) return MD_OK;
+        int h[md::VF_COUNT];
+        CK(cudaMemcpyAsync(h, l.vflags, sizeof(h), cudaMemcpyDeviceToHost, stream));
+        CK(cudaStreamSynchronize(stream));
+        CK(cudaGetLastError());
+        cur = h[md::VF_CUR]; curv = h[md::VF_CURV]; rebuilds_seen = h[md::VF_NREBUILD];
+        if (h[md::VF_ESCAPE]) { err = "a particle left a reflecting box (more than one bounce in a step)"; return MD_ERR_STATE; }
+        if (h[md::VF_OVERFLOW]) { err = "neighbour list overflow (> 128 neighbours within r_cut + skin)"; return MD_ERR_WORKSPACE; }
+        return MD_OK;
+    }
 
     ~Sim() override
     {
@@ -200,7 +274,11 @@ struct Sim : md_sim {
     template <bool ENERGY, bool KICK, bool COUNT>
     void launch_force()
     {
-        if (algo == MD_FORCE_CELLS) {
+        if (verlet()) {
+            if (ENERGY)
+                md::k_verlet_energy<T><<<cdiv((long long)p.nv * md::VL_G, md::VL_THREADS), md::VL_THREADS, 0, stream>>>(
+                    p, vl, cur, l.eo);
+        } else if (algo == MD_FORCE_CELLS) {
             // ROWS lanes per particle: 9 in 3D (3 particles per warp), 3 in 2D (10 per warp)
             if (dim == 3)
                 md::k_force_cells<T, 9, ENERGY, KICK, COUNT><<<cdiv(cdiv(p.nv, 3), 4), 128, 0, stream>>>(
@@ -251,6 +329,12 @@ struct Sim : md_sim {
     int step(long long n) override
     {
         if (n < 0) { err = "n_steps < 0"; return MD_ERR_INVALID_ARG; }
+        if (verlet()) {
+            if (n == 0) return MD_OK;
+            int rc = launch_run(n, 0);
+            if (rc == MD_OK) step_no += n;
+            return rc;
+        }
         if (stream == nullptr || stream == cudaStreamLegacy || stream == cudaStreamPerThread) {
             // the default streams cannot be captured: plain launches
             for (long long k = 0; k < n; ++k) enqueue_step(nullptr);
@@ -279,6 +363,22 @@ struct Sim : md_sim {
         if (!out || n < 0) { err = "bad arguments"; return MD_ERR_INVALID_ARG; }
         memset(out, 0, sizeof(*out));
         for (auto& e : ev) if (!e) CK(cudaEventCreate(&e));
+        if (verlet()) {
+            int rc = refresh();
+            if (rc) return rc;
+            const long long r0 = rebuilds_seen;
+            CK(cudaEventRecord(ev[0], stream));
+            if (n > 0 && (rc = launch_run(n, 0))) return rc;
+            CK(cudaEventRecord(ev[1], stream));
+            if ((rc = refresh())) return rc;
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, ev[0], ev[1]));
+            out->ms[3] = out->total_ms = ms;
+            out->launches[3] = n > 0 ? 1 : 0;
+            out->steps = n; out->rebuilds = rebuilds_seen - r0;
+            step_no += n;
+            return MD_OK;
+        }
         for (long long k = 0; k < n; ++k) {
             enqueue_step(ev);
             CK(cudaStreamSynchronize(stream));
@@ -300,6 +400,7 @@ struct Sim : md_sim {
 
     int check_err_flag()
     {
+        if (verlet()) return refresh();
         int h = 0;
         CK(cudaMemcpyAsync(&h, l.err, sizeof(int), cudaMemcpyDeviceToHost, stream));
         CK(cudaStreamSynchronize(stream));
@@ -311,7 +412,7 @@ struct Sim : md_sim {
     {
         if (energy_step == step_no) return MD_OK;
         launch_force<true, false, false>();
-        md::k_energy_partial<T><<<l.red_blocks, md::RED_THREADS, 0, stream>>>(p.nv, p.mass, l.st[cur], l.eo, l.part);
+        md::k_energy_partial<T><<<l.red_blocks, md::RED_THREADS, 0, stream>>>(p.nv, p.mass, view(), l.eo, l.part);
         md::k_energy_final<<<1, md::RED_THREADS, 0, stream>>>(l.red_blocks, l.part, l.eout);
         CK(cudaMemcpyAsync(e_host, l.eout, 6 * sizeof(double), cudaMemcpyDeviceToHost, stream));
         CK(cudaStreamSynchronize(stream));
@@ -344,7 +445,7 @@ struct Sim : md_sim {
 
     int export3(const T* a, const T* b, const T* c, double* host)
     {
-        md::k_export3<T><<<blocks(256), 256, 0, stream>>>(p.nv, dim, l.st[cur].id, a, b, c, l.stage0);
+        md::k_export3<T><<<blocks(256), 256, 0, stream>>>(p.nv, dim, view().id, a, b, c, l.stage0);
         CK(cudaMemcpyAsync(host, l.stage0, sizeof(double) * (size_t)p.nv * dim, cudaMemcpyDeviceToHost, stream));
         CK(cudaStreamSynchronize(stream));
         return MD_OK;
@@ -354,9 +455,10 @@ struct Sim : md_sim {
     {
         int rc = check_err_flag();
         if (rc) return rc;
-        const md::State<T>& s = l.st[cur];
+        const md::State<T> s = view();
         if (pos) {
-            md::k_export_pos<T><<<blocks(256), 256, 0, stream>>>(p.nv, dim, s.id, s.r, l.stage0);
+            if (verlet()) md::k_export_pos_wrapped<T><<<blocks(256), 256, 0, stream>>>(p, dim, s.id, s.r, l.stage0);
+            else md::k_export_pos<T><<<blocks(256), 256, 0, stream>>>(p.nv, dim, s.id, s.r, l.stage0);
             CK(cudaMemcpyAsync(pos, l.stage0, sizeof(double) * (size_t)p.nv * dim, cudaMemcpyDeviceToHost, stream));
             CK(cudaStreamSynchronize(stream));
         }
@@ -380,6 +482,17 @@ struct Sim : md_sim {
             *tests = (long long)p.nv * ((long long)p.nv - 1 + p.nw);
             return MD_OK;
         }
+        if (verlet()) {   // one test per neighbour-list entry
+            int rc = refresh();
+            if (rc) return rc;
+            std::vector<int> h((size_t)p.nv);
+            CK(cudaMemcpyAsync(h.data(), l.ncnt, sizeof(int) * h.size(), cudaMemcpyDeviceToHost, stream));
+            CK(cudaStreamSynchronize(stream));
+            long long t = 0;
+            for (int c : h) t += c;
+            *tests = t;
+            return MD_OK;
+        }
         CK(cudaMemsetAsync(l.tests, 0, sizeof(unsigned long long), stream));
         launch_force<false, false, true>();
         unsigned long long h = 0;
@@ -393,7 +506,7 @@ struct Sim : md_sim {
     {
         if (a) *a = algo;
         if (nc) for (int k = 0; k < 3; ++k) nc[k] = p.nc[k];
-        if (kps) *kps = algo == MD_FORCE_CELLS ? 5 : 2;
+        if (kps) *kps = algo == MD_FORCE_CELLS ? 5 : (verlet() ? 1 : 2);
     }
 
     int init(const md_box& box, const md_lj& lj, const md_opts& o, long long nv, const double* pos, const double* vel,
@@ -424,7 +537,7 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
         md::k_import<T><<<cdiv(nw, 256), 256, 0, stream>>>((int)nw, dim, l.wstage, nullptr, ws);
     }
     CK(cudaMemsetAsync(l.err, 0, 4 * sizeof(int), stream));
-    if (algo == MD_FORCE_CELLS) {
+    if (algo != MD_FORCE_ALLPAIRS) {
         CK(cudaMemsetAsync(l.count, 0, sizeof(int) * (size_t)p.ncell, stream));
         md::Params<T> pw = p;
         pw.nv = (int)nw;
@@ -444,6 +557,17 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
     CK(cudaMemcpyAsync(l.stage1, vel, sizeof(double) * (size_t)nv * dim, cudaMemcpyHostToDevice, stream));
     md::k_import<T><<<blocks(256), 256, 0, stream>>>((int)nv, dim, l.stage0, l.stage1, l.st[0]);
     cur = 0;
+    if (verlet()) {
+        // walls (cell order) appended to both position buffers; then bin + list + f(0) in one persistent launch
+        CK(cudaMemsetAsync(l.vflags, 0, sizeof(int) * md::VF_COUNT, stream));
+        if (nw > 0)
+            for (int b = 0; b < 2; ++b)
+                CK(cudaMemcpyAsync(l.st[b].r + nv, l.wr, sizeof(md::Vec4<T>) * (size_t)nw, cudaMemcpyDeviceToDevice,
+                                   stream));
+        int rc = launch_run(0, 1);
+        if (rc) return rc;
+        return refresh();
+    }
     if (algo == MD_FORCE_CELLS) {
         md::k_kick_drift_bin<T, false, true><<<blocks(256), 256, 0, stream>>>(p, l.st[0], l.f, l.count, l.cell, l.slot,
                                                                              l.err);
@@ -463,11 +587,11 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
              const GridSpec& g, int algo)
 {
     Sim<T>* s = new Sim<T>();
-    const bool cells = algo == MD_FORCE_CELLS;
+    const bool cells = algo != MD_FORCE_ALLPAIRS;
     s->dim = box.dim;
     s->algo = algo;
     s->stream = (cudaStream_t)stream;
-    s->l = carve<T>(ws, box.dim, nv, nw, g.ncell, cells);
+    s->l = carve<T>(ws, box.dim, nv, nw, g.ncell, algo);
     if (s->l.bytes > ws_bytes) {
         g_create_error = "workspace too small";
         delete s;
@@ -494,6 +618,15 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
     p.sig2_vw = (T)(lj.sigma_w * lj.sigma_w); p.e24_vw = (T)(24.0 * lj.eps_w); p.e4_vw = (T)(4.0 * lj.eps_w);
     p.uc_vw = (T)ucut(lj.eps_w, lj.sigma_w);
     p.dt = (T)o.dt; p.hk = (T)(o.dt / (2.0 * o.mass)); p.mass = o.mass;
+    if (algo == MD_FORCE_VERLET) {
+        const double skin = list_skin(lj, o), rl = lj.r_cut + skin;
+        md::Verlet<T>& v = s->vl;
+        v.st[0] = s->l.st[0]; v.st[1] = s->l.st[1]; v.f = s->l.f;
+        v.nbr = s->l.nbr; v.ncnt = s->l.ncnt;
+        v.cell = s->l.cell; v.slot = s->l.slot; v.count = s->l.count; v.start = s->l.start; v.tile_sum = s->l.tile_sum;
+        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags;
+        v.rl2 = (T)(rl * rl); v.half_skin = (T)(0.5 * skin);
+    }
     int rc = s->init(box, lj, o, nv, pos, vel, nw, wall);
     if (rc != MD_OK) {
         g_create_error = s->err;
@@ -532,12 +665,11 @@ extern "C" {
 size_t md_workspace_bytes(const md_box* box, const md_lj* lj, const md_opts* o, long long nv, long long nw)
 {
     if (validate(box, lj, o, nv, nw)) return 0;
-    GridSpec g = make_grid(*box, lj->r_cut);
-    int algo = pick_algo(*o, g, nv);
+    int algo = pick_algo(*box, *lj, *o, nv, nw);
     if (algo < 0) return 0;
-    const bool cells = algo == MD_FORCE_CELLS;
-    return o->precision == 64 ? carve<double>(nullptr, box->dim, nv, nw, g.ncell, cells).bytes
-                              : carve<float>(nullptr, box->dim, nv, nw, g.ncell, cells).bytes;
+    GridSpec g = grid_for(*box, *lj, *o, algo);
+    return o->precision == 64 ? carve<double>(nullptr, box->dim, nv, nw, g.ncell, algo).bytes
+                              : carve<float>(nullptr, box->dim, nv, nw, g.ncell, algo).bytes;
 }
 
 int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj* lj, const md_opts* o, long long nv,
@@ -564,9 +696,9 @@ int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj*
     if (!inside(pos, nv) || !inside(wall, nw)) { g_create_error = "position non-finite or outside [0, L]"; return MD_ERR_INVALID_ARG; }
     for (long long i = 0; i < nv * dim; ++i)
         if (!std::isfinite(vel[i])) { g_create_error = "velocity non-finite"; return MD_ERR_INVALID_ARG; }
-    GridSpec g = make_grid(*box, lj->r_cut);
-    int algo = pick_algo(*o, g, nv);
+    int algo = pick_algo(*box, *lj, *o, nv, nw);
     if (algo < 0) { g_create_error = "cell list needs >= 3 cells in every periodic dimension"; return MD_ERR_UNSUPPORTED; }
+    GridSpec g = grid_for(*box, *lj, *o, algo);
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         cudaGetLastError();

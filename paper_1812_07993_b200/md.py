@@ -17,8 +17,8 @@ LIB_PATH = os.path.join(HERE, "libmd_b200.so")
 MD_OK = 0
 MD_ERR_INVALID_ARG, MD_ERR_UNSUPPORTED, MD_ERR_CUDA, MD_ERR_WORKSPACE, MD_ERR_NONFINITE, MD_ERR_STATE = -1, -2, -3, -4, -5, -6
 MD_BC_PERIODIC, MD_BC_REFLECT = 0, 1
-MD_FORCE_AUTO, MD_FORCE_ALLPAIRS, MD_FORCE_CELLS = 0, 1, 2
-_ALGO = {"auto": MD_FORCE_AUTO, "allpairs": MD_FORCE_ALLPAIRS, "cells": MD_FORCE_CELLS}
+MD_FORCE_AUTO, MD_FORCE_ALLPAIRS, MD_FORCE_CELLS, MD_FORCE_VERLET = 0, 1, 2, 3
+_ALGO = {"auto": MD_FORCE_AUTO, "allpairs": MD_FORCE_ALLPAIRS, "cells": MD_FORCE_CELLS, "verlet": MD_FORCE_VERLET}
 
 EXPORTS = ["md_workspace_bytes", "md_create", "md_step", "md_get_state", "md_energy", "md_profile_step",
            "md_pair_tests", "md_info", "md_measure_peaks", "md_destroy", "md_last_error"]
@@ -39,7 +39,8 @@ class md_lj(C.Structure):
 
 
 class md_opts(C.Structure):
-    _fields_ = [("dt", C.c_double), ("mass", C.c_double), ("precision", C.c_int), ("force_algo", C.c_int)]
+    _fields_ = [("dt", C.c_double), ("mass", C.c_double), ("precision", C.c_int), ("force_algo", C.c_int),
+                ("skin", C.c_double)]
 
 
 class md_energy_out(C.Structure):
@@ -50,7 +51,7 @@ class md_energy_out(C.Structure):
 
 class md_kernel_times(C.Structure):
     _fields_ = [("ms", C.c_double * 4), ("launches", C.c_longlong * 4), ("total_ms", C.c_double),
-                ("steps", C.c_longlong)]
+                ("steps", C.c_longlong), ("rebuilds", C.c_longlong)]
 
 
 class md_peaks(C.Structure):
@@ -114,6 +115,7 @@ def _structs(cfg, precision=64, algo=None):
     lj.r_cut, lj.shift_energy = float(cfg["r_cut"]), int(cfg.get("shift_energy", 1))
     opts.dt, opts.mass, opts.precision = float(cfg["dt"]), float(cfg["mass"]), int(precision)
     opts.force_algo = _ALGO[algo if algo is not None else cfg.get("algo", "auto")]
+    opts.skin = float(cfg.get("skin", 0.0))
     return box, lj, opts
 
 
@@ -185,7 +187,7 @@ class Simulation:
     def profile_step(self, n_steps: int):
         t = md_kernel_times()
         self._check(self._lib.md_profile_step(self._h, int(n_steps), C.byref(t)))
-        return dict(ms=list(t.ms), launches=list(t.launches), total_ms=t.total_ms, steps=t.steps)
+        return dict(ms=list(t.ms), launches=list(t.launches), total_ms=t.total_ms, steps=t.steps, rebuilds=t.rebuilds)
 
     def pair_tests(self) -> int:
         v = C.c_longlong()
@@ -195,7 +197,7 @@ class Simulation:
     def info(self):
         algo, nc, kps = C.c_int(), (C.c_int * 3)(), C.c_int()
         self._check(self._lib.md_info(self._h, C.byref(algo), C.byref(nc), C.byref(kps)))
-        return dict(algo={1: "allpairs", 2: "cells"}[algo.value], n_cells=list(nc), kernels_per_step=kps.value)
+        return dict(algo={1: "allpairs", 2: "cells", 3: "verlet"}[algo.value], n_cells=list(nc), kernels_per_step=kps.value)
 
     def synchronize(self):
         self.stream.synchronize()

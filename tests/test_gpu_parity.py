@@ -24,9 +24,18 @@ def _need_gpu():
     md.load_library()
 
 
+def make_sim(cfg, algo, precision=64):
+    try:
+        return md.Simulation(cfg, precision=precision, algo=algo)
+    except md.MDError as e:
+        if e.code == md.MD_ERR_UNSUPPORTED and algo in ("verlet", "cells"):
+            pytest.skip("%s needs >= 3 cells per periodic dimension in this box" % algo)
+        raise
+
+
 def check_step0(cfg, algo, ref=None, precision=64, ftol=FTOL):
+    sim = make_sim(cfg, algo, precision)
     ref = ref if ref is not None else O.forces(cfg, cells=cfg["n_vapor"] > 20000)
-    sim = md.Simulation(cfg, precision=precision, algo=algo)
     st = sim.get_state()
     en = sim.energy()
     assert sim.info()["algo"] == algo
@@ -45,8 +54,8 @@ def check_step0(cfg, algo, ref=None, precision=64, ftol=FTOL):
 
 
 def check_traj(cfg, algo, n_steps=100, cells_oracle=False, chunks=(37, 63)):
+    sim = make_sim(cfg, algo)
     ref = O.run(cfg, n_steps, cells=cells_oracle)
-    sim = md.Simulation(cfg, algo=algo)
     assert sum(chunks) == n_steps
     for c in chunks:                      # odd + odd chunk sizes exercise both graph parities
         sim.step(c)
@@ -61,7 +70,10 @@ def check_traj(cfg, algo, n_steps=100, cells_oracle=False, chunks=(37, 63)):
     sim.close()
 
 
-@pytest.mark.parametrize("algo", ["allpairs", "cells"])
+ALGOS = ["allpairs", "cells", "verlet"]
+
+
+@pytest.mark.parametrize("algo", ALGOS)
 def test_config0_forces_and_trajectory(algo):
     cfg = I.config0()
     check_step0(cfg, algo)
@@ -72,8 +84,9 @@ def test_config0_forces_and_trajectory(algo):
 @pytest.mark.parametrize("dim,box,bc,nw,seed", [
     (3, (8.0, 9.3, 7.6), (0, 0, 0), 40, 1), (3, (8.1, 7.5, 5.2), (0, 0, 1), 40, 2), (3, (4.0, 8.0, 8.0), (1, 0, 0), 0, 3),
     (2, (13.7, 9.9), (0, 1), 12, 4), (2, (7.5, 7.5), (0, 0), 12, 5), (2, (2.6, 30.0), (1, 0), 5, 6),
-    (3, (3.0, 3.0, 3.0), (1, 1, 1), 2, 7)])
-@pytest.mark.parametrize("algo", ["allpairs", "cells"])
+    (3, (3.0, 3.0, 3.0), (1, 1, 1), 2, 7), (3, (9.0, 10.5, 9.3), (0, 0, 0), 30, 8), (3, (9.5, 9.0, 5.2), (0, 0, 1), 30, 9),
+    (2, (12.0, 9.0), (0, 0), 10, 10)])
+@pytest.mark.parametrize("algo", ALGOS)
 def test_small_ragged_cases(dim, box, bc, nw, seed, algo):
     vol = float(np.prod(box))
     nv = min(300, int((0.5 if dim == 3 else 0.45) * vol) - nw)
@@ -88,7 +101,7 @@ def test_small_ragged_cases(dim, box, bc, nw, seed, algo):
 
 def test_single_particle_and_no_walls():
     cfg = I.small_case(3, 1, (9.0, 9.0, 9.0), (0, 1, 0), seed=3)
-    for algo in ("allpairs", "cells"):
+    for algo in ALGOS:
         sim = md.Simulation(cfg, algo=algo)
         sim.step(10)
         st = sim.get_state()
@@ -103,7 +116,7 @@ def test_two_particle_closed_form_on_gpu():
     cfg = I.small_case(3, 2, (20.0, 20.0, 20.0), (0, 0, 0), seed=3)
     cfg["pos"] = np.array([[1.5, 7.0, 7.0], [0.0, 7.0, 7.0]])
     cfg["shift_energy"] = 0
-    for algo in ("allpairs", "cells"):
+    for algo in ALGOS:
         sim = md.Simulation(cfg, algo=algo)
         st, en = sim.get_state(), sim.energy()
         assert abs(en["U"] + 0.3203365942785745) < 1e-14
@@ -114,17 +127,20 @@ def test_two_particle_closed_form_on_gpu():
 def test_reflecting_escape_is_reported():
     cfg = I.small_case(3, 4, (9.0, 9.0, 9.0), (1, 1, 1), seed=3)
     cfg["vel"][0, 0] = 9.0 * 3 / cfg["dt"]           # crosses the box three times in one step
-    sim = md.Simulation(cfg, algo="allpairs")
-    sim.step(1)
-    with pytest.raises(md.MDError) as e:
-        sim.get_state()
-    assert e.value.code == md.MD_ERR_STATE
+    for algo in ALGOS:
+        sim = md.Simulation(cfg, algo=algo)
+        sim.step(1)
+        with pytest.raises(md.MDError) as e:
+            sim.get_state()
+        assert e.value.code == md.MD_ERR_STATE
 
 
 def test_config1_step0_and_100_steps():
     cfg = I.config1()
-    check_step0(cfg, "cells", ref=O.forces(cfg))          # brute-force oracle, 3.4e8 tests
-    check_traj(cfg, "cells", 100, cells_oracle=True)
+    ref = O.forces(cfg)                                   # brute-force oracle, 3.4e8 tests
+    for algo in ("cells", "verlet"):
+        check_step0(cfg, algo, ref=ref)
+        check_traj(cfg, algo, 100, cells_oracle=True)
 
 
 def test_config2_step0_brute_sample_and_cells():
@@ -140,13 +156,17 @@ def test_config2_step0_brute_sample_and_cells():
     assert force_error(st["f"][idx], ref["f"][idx]) <= FTOL
     assert sim.energy()["pairs_vv"] == ref["pairs_vv"]
     sim.close()
+    check_step0(cfg, "verlet", ref=ref)
     check_traj(cfg, "cells", 100, cells_oracle=True)
+    check_traj(cfg, "verlet", 100, cells_oracle=True)
 
 
 @pytest.mark.parametrize("shape", ["cone", "inkbottle", "slit"])
 def test_config3_shapes_step0(shape):
     cfg = I.config3(shape)
-    check_step0(cfg, "cells", ref=O.forces(cfg, cells=True))
+    ref = O.forces(cfg, cells=True)
+    check_step0(cfg, "cells", ref=ref)
+    check_step0(cfg, "verlet", ref=ref)
 
 
 @pytest.mark.parametrize("log2n", [10, 12, 14])
@@ -155,12 +175,16 @@ def test_config4_sizes_both_kernels(log2n):
     ref = O.forces(cfg)
     check_step0(cfg, "cells", ref=ref)
     check_step0(cfg, "allpairs", ref=ref)
+    check_step0(cfg, "verlet", ref=ref)
     check_traj(cfg, "cells", 100, cells_oracle=True)
+    check_traj(cfg, "verlet", 100, cells_oracle=True)
 
 
 def test_config4_2p20_cells_step0():
     cfg = I.config4(20)
-    check_step0(cfg, "cells", ref=O.forces(cfg, cells=True))
+    ref = O.forces(cfg, cells=True)
+    check_step0(cfg, "cells", ref=ref)
+    check_step0(cfg, "verlet", ref=ref)
 
 
 def test_fp32_mode_forces():
@@ -171,27 +195,35 @@ def test_fp32_mode_forces():
     c32["wall"] = cfg["wall"].astype(np.float32).astype(np.float64)
     c32["box_len"] = [float(np.float32(x)) for x in cfg["box_len"]]
     ref = O.forces(c32)
-    for algo in ("cells", "allpairs"):
+    for algo in ("cells", "allpairs", "verlet"):
         check_step0(c32, algo, ref=ref, precision=32, ftol=1e-4)
 
 
-def test_energy_drift_and_long_run_statistics_dilute_gas():
-    # long runs are chaotic: compare the drift statistic (reading A8: wall-free dilute 3D gas, shifted energy)
-    # and the temperature with the oracle's, not trajectories
-    cfg = I.cylinder_config(4096, 4242, "drift", box=(4096 / 0.05) ** (1 / 3), length=0)
-    sim = md.Simulation(cfg, algo="cells")
+@pytest.mark.parametrize("algo", ["cells", "verlet"])
+def test_energy_drift_and_long_run_statistics_dilute_gas(algo):
+    # long runs are chaotic: compare the drift statistic (reading A8: wall-free dilute 3D gas, shifted energy,
+    # |<E>_{9000..10000} - <E>_{1000..2000}| / K(0)) and the temperature with the oracle's, not trajectories
+    # N = 16384: the statistic is a random walk of r_c-crossing kinks whose relative size falls as 1/sqrt(N)
+    cfg = I.cylinder_config(16384, 4242, "drift", box=(16384 / 0.05) ** (1 / 3), length=0)
+    sim = md.Simulation(cfg, algo=algo)
     e0 = sim.energy()
-    es = []
-    for _ in range(50):
-        sim.step(200)
-        e = sim.energy()
-        es.append((e["K"], e["U"]))
-    es = np.array(es)
-    tot = es.sum(axis=1)
-    drift = abs(tot[-5:].mean() - tot[5:10].mean()) / e0["K"]
+
+    def window():
+        out = []
+        for _ in range(100):
+            sim.step(10)
+            e = sim.energy()
+            out.append((e["K"], e["U"]))
+        return np.array(out)
+
+    sim.step(1000)
+    wa = window()
+    sim.step(7000)
+    wb = window()
+    assert sim.energy()["step"] == 10000
+    drift = abs(wb.sum(axis=1).mean() - wa.sum(axis=1).mean()) / e0["K"]
     assert drift <= 1e-4, drift
-    ref = O.run(cfg, 2000, cells=True, history=True)["hist"]
-    t_ref = ref[1800:2000, 0].mean()
-    t_gpu = es[8:10, 0].mean()
-    assert abs(t_gpu - t_ref) / t_ref < 0.03
+    ref = O.run(cfg, 1500, cells=True, history=True)["hist"]
+    t_ref = ref[1000:1500, 0].mean()
+    assert abs(wa[:50, 0].mean() - t_ref) / t_ref < 0.02
     sim.close()
