@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -120,6 +121,7 @@ struct Layout {
     unsigned long long* tests;
     double *stage0, *stage1, *wstage;
     int *nbr, *ncnt, *vflags;   // VERLET: neighbour list, counts, flags
+    unsigned long long* vtimes;
     int red_blocks;
     size_t bytes;
 };
@@ -160,6 +162,7 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.nbr = c.take<int>(verlet ? (size_t)nv * md::VL_MAXN : 1);
     l.ncnt = c.take<int>(verlet ? n : 1);
     l.vflags = c.take<int>(md::VF_COUNT);
+    l.vtimes = c.take<unsigned long long>(8);
     l.stage0 = c.take<double>(n * dim);
     l.stage1 = c.take<double>(n * dim);
     l.wstage = c.take<double>(m * dim);
@@ -207,6 +210,7 @@ struct Sim : md_sim {
     md::Verlet<T> vl;
     int curv = 0, coop_grid = 0;
     long long rebuilds_seen = 0;
+    unsigned long long phase_seen[4] = {0, 0, 0, 0}, phase_ns[4] = {0, 0, 0, 0};
 
     bool verlet() const { return algo == MD_FORCE_VERLET; }
 
@@ -373,6 +377,14 @@ struct Sim : md_sim {
             if ((rc = refresh())) return rc;
             float ms = 0.f;
             CK(cudaEventElapsedTime(&ms, ev[0], ev[1]));
+            unsigned long long t[8];
+            CK(cudaMemcpy(t, l.vtimes, sizeof(t), cudaMemcpyDeviceToHost));
+            if (getenv("MD_DEBUG_TIMES"))
+                fprintf(stderr, "[md] cumulative ns: step %llu barrier %llu rebuild %llu final %llu | bin %llu scan %llu "
+                        "scatter %llu build %llu\n", t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7]);
+            for (int q = 0; q < 4; ++q) { phase_ns[q] = t[q] - phase_seen[q]; phase_seen[q] = t[q]; }
+            // VERLET: ms[0] step phases, ms[1] grid barriers, ms[2] rebuilds (as seen by thread 0), ms[3] whole launch
+            out->ms[0] = phase_ns[0] * 1e-6; out->ms[1] = phase_ns[1] * 1e-6; out->ms[2] = phase_ns[2] * 1e-6;
             out->ms[3] = out->total_ms = ms;
             out->launches[3] = n > 0 ? 1 : 0;
             out->steps = n; out->rebuilds = rebuilds_seen - r0;
@@ -489,7 +501,7 @@ struct Sim : md_sim {
             CK(cudaMemcpyAsync(h.data(), l.ncnt, sizeof(int) * h.size(), cudaMemcpyDeviceToHost, stream));
             CK(cudaStreamSynchronize(stream));
             long long t = 0;
-            for (int c : h) t += c;
+            for (int c : h) t += c & (md::VL_FOLD - 1);
             *tests = t;
             return MD_OK;
         }
@@ -560,6 +572,8 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
     if (verlet()) {
         // walls (cell order) appended to both position buffers; then bin + list + f(0) in one persistent launch
         CK(cudaMemsetAsync(l.vflags, 0, sizeof(int) * md::VF_COUNT, stream));
+        CK(cudaMemsetAsync(l.vtimes, 0, 8 * sizeof(unsigned long long), stream));
+        CK(cudaMemsetAsync(l.tile_sum, 0, sizeof(int) * (size_t)(cdiv(p.ncell, md::SCAN_TILE) + 1), stream));
         if (nw > 0)
             for (int b = 0; b < 2; ++b)
                 CK(cudaMemcpyAsync(l.st[b].r + nv, l.wr, sizeof(md::Vec4<T>) * (size_t)nw, cudaMemcpyDeviceToDevice,
@@ -624,7 +638,7 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
         v.st[0] = s->l.st[0]; v.st[1] = s->l.st[1]; v.f = s->l.f;
         v.nbr = s->l.nbr; v.ncnt = s->l.ncnt;
         v.cell = s->l.cell; v.slot = s->l.slot; v.count = s->l.count; v.start = s->l.start; v.tile_sum = s->l.tile_sum;
-        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags;
+        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.times = s->l.vtimes;
         v.rl2 = (T)(rl * rl); v.half_skin = (T)(0.5 * skin);
     }
     int rc = s->init(box, lj, o, nv, pos, vel, nw, wall);

@@ -39,6 +39,8 @@ struct Verlet {
     const int* wstart;         // walls: [ncell + 1] ranges into the wall tail
     const uint8_t* wnear;
     int* flags;                // VF_*
+    unsigned long long* times; // [8] ns seen by thread 0: step phases, step barriers, rebuilds, final phase,
+                               // rebuild split: bin, scan, scatter, list build (each with its barrier)
     T rl2, half_skin;          // (r_c + skin)^2, skin / 2
 };
 
@@ -59,6 +61,13 @@ __device__ __forceinline__ float fold(float a, float b, float L, float halfL)
     return d;
 }
 
+__device__ __forceinline__ unsigned long long now_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+
 template <typename V>
 __device__ __forceinline__ V group_sum(V v)
 {
@@ -68,22 +77,34 @@ __device__ __forceinline__ V group_sum(V v)
 }
 
 // ---- one particle's force from its neighbour list, VL_G lanes ---------------------------------
+// ncnt[i] = list length | VL_FOLD if the particle sat in a cell on a periodic face when the list was
+// built: only such particles can have a neighbour across the face, all others skip the image folding.
+constexpr int VL_FOLD = 1 << 30;
+
+template <typename T, bool ENERGY, bool FOLD>
+__device__ __forceinline__ void list_loop(const Params<T>& p, const int* __restrict__ lst, int n, const Vec4<T>* __restrict__ r,
+                                          int g, const Vec4<T>& ri, Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
+{
+    const bool px = FOLD && p.bc[0] == BC_PERIODIC, py = FOLD && p.bc[1] == BC_PERIODIC, pz = FOLD && p.bc[2] == BC_PERIODIC;
+    for (int k = g; k < n; k += VL_G) {
+        const int j = lst[k];
+        const Vec4<T> rj = r[j];
+        const T dx = px ? fold(ri.x, rj.x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj.x;
+        const T dy = py ? fold(ri.y, rj.y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj.y;
+        const T dz = pz ? fold(ri.z, rj.z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj.z;
+        if (j < p.nv) pair_term<T, ENERGY>(dx, dy, dz, p.rc2, p.sig2_vv, p.e24_vv, p.e4_vv, p.uc_vv, av);
+        else pair_term<T, ENERGY>(dx, dy, dz, p.rc2, p.sig2_vw, p.e24_vw, p.e4_vw, p.uc_vw, aw);
+    }
+}
+
 template <typename T, bool ENERGY>
 __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& v, const Vec4<T>* __restrict__ r, int i,
                                            int g, const Vec4<T>& ri, Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
-    const int n = v.ncnt[i];
+    const int raw = v.ncnt[i];
     const int* __restrict__ lst = v.nbr + (size_t)i * VL_MAXN;
-    const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
-    for (int k = g; k < n; k += VL_G) {
-        const int j = lst[k];
-        const Vec4<T> rj = r[j];
-        T dx = px ? fold(ri.x, rj.x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj.x;
-        T dy = py ? fold(ri.y, rj.y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj.y;
-        T dz = pz ? fold(ri.z, rj.z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj.z;
-        if (j < p.nv) pair_term<T, ENERGY>(dx, dy, dz, p.rc2, p.sig2_vv, p.e24_vv, p.e4_vv, p.uc_vv, av);
-        else pair_term<T, ENERGY>(dx, dy, dz, p.rc2, p.sig2_vw, p.e24_vw, p.e4_vw, p.uc_vw, aw);
-    }
+    if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, raw & (VL_FOLD - 1), r, g, ri, av, aw);
+    else list_loop<T, ENERGY, false>(p, lst, raw, r, g, ri, av, aw);
 }
 
 // ---- phase: [forces] -> [kick completing the step] -> [kick + drift of the next step] -----------
@@ -94,13 +115,20 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
                                            bool kick, bool drift, int req, int gtid, int gthreads)
 {
     const Vec4<T>* __restrict__ rcur = v.st[c].r;
-    Vec4<T>* __restrict__ rnew = v.st[c ^ 1].r;
+    T* __restrict__ rnew = reinterpret_cast<T*>(v.st[c ^ 1].r);
     const State<T>& s = v.st[cv];
     const int g = gtid & (VL_G - 1);
     const int ngroups = gthreads / VL_G;
+    // after the group reduction every lane holds f_i: lane g < 3 integrates component g (x, y, z)
+    T* __restrict__ vcomp = g == 0 ? s.vx : (g == 1 ? s.vy : s.vz);
+    T* __restrict__ fcomp = g == 0 ? v.f.fx : (g == 1 ? v.f.fy : v.f.fz);
+    const T Lg = p.L[g < 3 ? g : 0];
+    const int bcg = g < 3 ? p.bc[g] : BC_NONE;
     for (int i0 = gtid / VL_G; i0 < ((p.nv + 3) & ~3); i0 += ngroups) {     // whole warps stay in the loop together
         const int i = min(i0, p.nv - 1);
         const Vec4<T> ri = rcur[i];
+        T vg = T(0);
+        if (g < 3) vg = vcomp[i];                     // issued early, consumed after the force loop
         T fx, fy, fz;
         if (force) {
             Acc<T, false> av, aw;
@@ -111,27 +139,31 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         } else {
             fx = v.f.fx[i]; fy = v.f.fy[i]; fz = v.f.fz[i];
         }
-        if (g != 0 || i0 >= p.nv) continue;
-        T vx = s.vx[i], vy = s.vy[i], vz = s.vz[i];
-        if (force) { v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz; }
-        if (kick) {                                    // F3: v(t) = v(t - dt/2) + (dt/2m) f(t)
-            vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
-        }
+        const bool mine = g < 3 && i0 < p.nv;
+        const T fg = g == 0 ? fx : (g == 1 ? fy : fz);
+        const T rg = g == 0 ? ri.x : (g == 1 ? ri.y : ri.z);
+        if (mine && force) fcomp[i] = fg;
+        if (kick) vg = vg + p.hk * fg;                 // F3: v(t) = v(t - dt/2) + (dt/2m) f(t)
+        T step2 = T(0);
         if (drift) {                                   // F2: v(t + dt/2), r(t + dt)
-            vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
-            const T sx = p.dt * vx, sy = p.dt * vy, sz = p.dt * vz;
-            Vec4<T> rn;
-            rn.x = ri.x + sx; rn.y = ri.y + sy; rn.z = ri.z + sz;
+            vg = vg + p.hk * fg;
+            const T sg = p.dt * vg;
+            T rn = rg + sg;
             // periodic dimensions are left unwrapped until the next rebuild; reflection is immediate
-            int* err = v.flags + VF_ESCAPE;
-            if (p.bc[0] == BC_REFLECT) boundary(rn.x, vx, p.L[0], BC_REFLECT, err);
-            if (p.bc[1] == BC_REFLECT) boundary(rn.y, vy, p.L[1], BC_REFLECT, err);
-            if (p.bc[2] == BC_REFLECT) boundary(rn.z, vz, p.L[2], BC_REFLECT, err);
-            rn.w = ri.w + sqrt(sx * sx + sy * sy + sz * sz);      // path length >= displacement
-            if (rn.w > v.half_skin) v.flags[VF_REQ0 + req] = 1;
-            rnew[i] = rn;
+            if (mine && bcg == BC_REFLECT) boundary(rn, vg, Lg, BC_REFLECT, v.flags + VF_ESCAPE);
+            if (mine) rnew[4 * (size_t)i + g] = rn;
+            step2 = g < 3 ? sg * sg : T(0);
         }
-        if (kick || drift) { s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz; }
+        if (mine && (kick || drift)) vcomp[i] = vg;
+        if (drift) {                                   // path length since the last rebuild (>= displacement)
+            step2 += __shfl_xor_sync(0xffffffffu, step2, 1);
+            step2 += __shfl_xor_sync(0xffffffffu, step2, 2);
+            if (g == 3 && i0 < p.nv) {
+                const T w = ri.w + sqrt(step2);
+                rnew[4 * (size_t)i + 3] = w;
+                if (w > v.half_skin) v.flags[VF_REQ0 + req] = 1;
+            }
+        }
     }
 }
 
@@ -189,7 +221,11 @@ __device__ __forceinline__ void phase_scan_apply(int* __restrict__ count, int n,
     const int tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
     for (int t = blockIdx.x; t < tiles; t += gridDim.x) {
         int off = 0;
-        for (int k = threadIdx.x; k < t; k += SCAN_THREADS) off += tile_sum[k];
+        if (tile_sum) {
+            for (int k = threadIdx.x; k < t; k += SCAN_THREADS) off += tile_sum[k];
+        } else {            // few tiles: sum the earlier counts directly and save a phase + barrier
+            for (int k = threadIdx.x; k < t * SCAN_TILE; k += SCAN_THREADS) off += count[k];
+        }
         off = warp_sum(off);
         __syncthreads();
         if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = off;
@@ -218,7 +254,7 @@ __device__ __forceinline__ void phase_scan_apply(int* __restrict__ count, int n,
         int run = off + wofs + incl - s;
 #pragma unroll
         for (int k = 0; k < SCAN_ITEMS; ++k) {
-            if (base + k < n) { start[base + k] = run; count[base + k] = 0; }
+            if (base + k < n) start[base + k] = run;     // counts are cleared in the list-build phase
             run += val[k];
         }
         if (base <= n - 1 && n - 1 < base + SCAN_ITEMS) start[n] = run;
@@ -243,11 +279,12 @@ __device__ __forceinline__ void phase_scatter(const Params<T>& p, const Verlet<T
 }
 
 // R4: neighbour list from the cell list (a3's cell traversal, cached): every j within r_c + skin of i,
-// vapor (j < nv) or wall (j = nv + k).  One thread per particle walks its 3^(d-1) cell rows; each row is
-// one contiguous range of the cell-ordered arrays.  Positions are wrapped here, so distances fold.
+// vapor (j < nv) or wall (j = nv + k).  ROWS = 3^(d-1) lanes cooperate on one particle: lane `row` walks the
+// cell row (cy+ky, cz+kz) -- its three cells are one contiguous range of the cell-ordered arrays -- and
+// appends its hits through a shared-memory counter.  Positions are wrapped here, so distances fold.
 template <typename T>
-__device__ __forceinline__ int list_range(const Params<T>& p, const Vec4<T>* __restrict__ r, int jb, int je, int skip,
-                                          const Vec4<T>& ri, T rl2, int* __restrict__ lst, int n)
+__device__ __forceinline__ void list_range(const Params<T>& p, const Vec4<T>* __restrict__ r, int jb, int je, int skip,
+                                           const Vec4<T>& ri, T rl2, int* __restrict__ lst, int* cnt)
 {
     const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
     for (int j = jb; j < je; ++j) {
@@ -258,46 +295,71 @@ __device__ __forceinline__ int list_range(const Params<T>& p, const Vec4<T>* __r
         const T dz = pz ? fold(ri.z, rj.z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj.z;
         const T r2 = fma_(dz, dz, fma_(dy, dy, dx * dx));
         if (r2 < rl2) {
-            if (n < VL_MAXN) lst[n] = j;
-            ++n;
+            const int k = atomicAdd(cnt, 1);
+            if (k < VL_MAXN) lst[k] = j;
         }
     }
-    return n;
 }
 
 template <typename T, int ROWS>
 __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>& v, int c, int gtid, int gthreads)
 {
+    constexpr int PPW = 32 / ROWS;                       // particles per warp
+    __shared__ int s_cnt[(VL_THREADS / 32) * PPW];
     const Vec4<T>* __restrict__ r = v.st[c].r;
     const int nx = p.nc[0], ny = p.nc[1], nz = p.nc[2];
-    for (int i = gtid; i < p.nv; i += gthreads) {
-        const Vec4<T> ri = r[i];
-        int cx, cy, cz;
-        const int ci = cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
-        int* __restrict__ lst = v.nbr + (size_t)i * VL_MAXN;
-        const bool do_wall = p.nw > 0 && v.wnear[ci];
-        const int x0 = max(cx - 1, 0), x1 = min(cx + 1, nx - 1);
-        int xw = -1;
-        if (p.bc[0] == BC_PERIODIC) { if (cx == 0) xw = nx - 1; else if (cx == nx - 1) xw = 0; }
-        int n = 0;
-        for (int row = 0; row < ROWS; ++row) {
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int pl = lane / ROWS, row = lane - pl * ROWS;
+    const int warp = gtid >> 5, nwarps = gthreads >> 5;
+    int* cnt = s_cnt + wib * PPW + min(pl, PPW - 1);
+    for (int base = warp * PPW; base < p.nv; base += nwarps * PPW) {
+        const int i = base + pl;
+        const bool active = pl < PPW && i < p.nv;
+        if (active && row == 0) *cnt = 0;
+        __syncwarp();
+        if (active) {
+            const Vec4<T> ri = r[i];
+            int cx, cy, cz;
+            const int ci = cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
+            int* __restrict__ lst = v.nbr + (size_t)i * VL_MAXN;
             int qy = cy + row % 3 - 1, qz = cz + (ROWS == 9 ? row / 3 - 1 : 0);
-            if (qz < 0) { if (p.bc[2] != BC_PERIODIC) continue; qz += nz; }
-            else if (qz >= nz) { if (p.bc[2] != BC_PERIODIC) continue; qz -= nz; }
-            if (qy < 0) { if (p.bc[1] != BC_PERIODIC) continue; qy += ny; }
-            else if (qy >= ny) { if (p.bc[1] != BC_PERIODIC) continue; qy -= ny; }
-            const int rowc = (qz * ny + qy) * nx;
-            n = list_range<T>(p, r, v.start[rowc + x0], v.start[rowc + x1 + 1], i, ri, v.rl2, lst, n);
-            if (xw >= 0) n = list_range<T>(p, r, v.start[rowc + xw], v.start[rowc + xw + 1], i, ri, v.rl2, lst, n);
-            if (do_wall) {
-                n = list_range<T>(p, r, p.nv + v.wstart[rowc + x0], p.nv + v.wstart[rowc + x1 + 1], -1, ri, v.rl2, lst, n);
-                if (xw >= 0)
-                    n = list_range<T>(p, r, p.nv + v.wstart[rowc + xw], p.nv + v.wstart[rowc + xw + 1], -1, ri, v.rl2,
-                                      lst, n);
+            bool ok = true;
+            if (qz < 0) { ok = p.bc[2] == BC_PERIODIC; qz += nz; }
+            else if (qz >= nz) { ok = p.bc[2] == BC_PERIODIC; qz -= nz; }
+            if (qy < 0) { ok = ok && p.bc[1] == BC_PERIODIC; qy += ny; }
+            else if (qy >= ny) { ok = ok && p.bc[1] == BC_PERIODIC; qy -= ny; }
+            if (ok) {
+                const int x0 = max(cx - 1, 0), x1 = min(cx + 1, nx - 1);
+                int xw = -1;
+                if (p.bc[0] == BC_PERIODIC) { if (cx == 0) xw = nx - 1; else if (cx == nx - 1) xw = 0; }
+                const int rowc = (qz * ny + qy) * nx;
+                const bool do_wall = p.nw > 0 && v.wnear[ci];
+                const int jb = v.start[rowc + x0], je = v.start[rowc + x1 + 1];
+                int jb2 = 0, je2 = 0, wb = 0, we = 0, wb2 = 0, we2 = 0;
+                if (xw >= 0) { jb2 = v.start[rowc + xw]; je2 = v.start[rowc + xw + 1]; }
+                if (do_wall) {
+                    wb = v.wstart[rowc + x0]; we = v.wstart[rowc + x1 + 1];
+                    if (xw >= 0) { wb2 = v.wstart[rowc + xw]; we2 = v.wstart[rowc + xw + 1]; }
+                }
+                list_range<T>(p, r, jb, je, i, ri, v.rl2, lst, cnt);
+                list_range<T>(p, r, jb2, je2, i, ri, v.rl2, lst, cnt);
+                list_range<T>(p, r, p.nv + wb, p.nv + we, -1, ri, v.rl2, lst, cnt);
+                list_range<T>(p, r, p.nv + wb2, p.nv + we2, -1, ri, v.rl2, lst, cnt);
             }
         }
-        v.ncnt[i] = min(n, VL_MAXN);
-        if (n > VL_MAXN) v.flags[VF_OVERFLOW] = 1;
+        __syncwarp();
+        if (active && row == 0) {
+            const int n = *cnt;
+            const Vec4<T> ri = r[i];
+            int cx, cy, cz;
+            cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
+            const bool face = (p.bc[0] == BC_PERIODIC && (cx == 0 || cx == nx - 1)) ||
+                              (p.bc[1] == BC_PERIODIC && (cy == 0 || cy == ny - 1)) ||
+                              (p.bc[2] == BC_PERIODIC && (cz == 0 || cz == nz - 1));
+            v.ncnt[i] = min(n, VL_MAXN) | (face ? VL_FOLD : 0);
+            if (n > VL_MAXN) v.flags[VF_OVERFLOW] = 1;
+        }
+        __syncwarp();
     }
 }
 
@@ -306,38 +368,50 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
 // phase(force; kick): n + 1 phases and n grid barriers for n steps, plus 5 barriers per rebuild.
 // force_rebuild (md_create): bin + build the list first, then evaluate f(0).
 template <typename T, int ROWS>
-__global__ void __launch_bounds__(VL_THREADS, 2) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
+__global__ void __launch_bounds__(VL_THREADS, 4) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
 {
     cg::grid_group grid = cg::this_grid();
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
     const int gthreads = gridDim.x * blockDim.x;
     int c = v.flags[VF_CUR], cv = v.flags[VF_CURV];
     bool rebuild = force_rebuild != 0;
+    unsigned long long t0 = gtid == 0 ? now_ns() : 0ull, t1;
     for (long long s = 0;; ++s) {
         if (rebuild) {
+            unsigned long long u0 = gtid == 0 ? now_ns() : 0ull, u1;
             phase_bin<T>(p, v, c, gtid, gthreads);
             grid.sync();
-            phase_scan_reduce(v.count, p.ncell, v.tile_sum);
+            if (gtid == 0) { u1 = now_ns(); v.times[4] += u1 - u0; u0 = u1; }
+            const bool two_level = p.ncell > 64 * SCAN_TILE;
+            if (two_level) {
+                phase_scan_reduce(v.count, p.ncell, v.tile_sum);
+                grid.sync();
+            }
+            phase_scan_apply(v.count, p.ncell, two_level ? v.tile_sum : nullptr, v.start);
             grid.sync();
-            phase_scan_apply(v.count, p.ncell, v.tile_sum, v.start);
-            grid.sync();
+            if (gtid == 0) { u1 = now_ns(); v.times[5] += u1 - u0; u0 = u1; }
             phase_scatter<T>(p, v, c, cv, gtid, gthreads);
             grid.sync();
+            if (gtid == 0) { u1 = now_ns(); v.times[6] += u1 - u0; u0 = u1; }
             c ^= 1; cv ^= 1;
             phase_build<T, ROWS>(p, v, c, gtid, gthreads);
+            for (int q = gtid; q < p.ncell; q += gthreads) v.count[q] = 0;                  // for the next rebuild
             if (gtid == 0) v.flags[VF_NREBUILD] += 1;
             grid.sync();
+            if (gtid == 0) { t1 = now_ns(); v.times[2] += t1 - t0; t0 = t1; v.times[7] += t1 - u0; }
         }
         if (s == n_steps) break;
         const int req = (int)(s % 3);
         if (gtid == 0) v.flags[VF_REQ0 + (req + 1) % 3] = 0;      // slot of step s + 1
         phase_step<T>(p, v, c, cv, s > 0, s > 0, true, req, gtid, gthreads);
+        if (gtid == 0) { t1 = now_ns(); v.times[0] += t1 - t0; t0 = t1; }
         grid.sync();
+        if (gtid == 0) { t1 = now_ns(); v.times[1] += t1 - t0; t0 = t1; }
         c ^= 1;
         rebuild = *(volatile int*)(v.flags + VF_REQ0 + req) != 0;
     }
     if (n_steps > 0 || force_rebuild) phase_step<T>(p, v, c, cv, true, n_steps > 0, false, 0, gtid, gthreads);
-    if (gtid == 0) { v.flags[VF_CUR] = c; v.flags[VF_CURV] = cv; }
+    if (gtid == 0) { v.flags[VF_CUR] = c; v.flags[VF_CURV] = cv; v.times[3] += now_ns() - t0; }
 }
 
 // a5 energy pass over the neighbour list (ordinary launch; the host passes the buffer parities).
