@@ -68,7 +68,7 @@ typedef struct { double eps, sigma, eps_w, sigma_w, r_cut; int shift_energy; } m
  *             skin/2, cached as a neighbour list of all pairs within r_cut + skin (exact: no pair
  *             within r_cut is ever missed); the whole md_step batch is one persistent launch;
  *   AUTO      VERLET when the grid allows it and n_vapor >= 2048, else CELLS, else ALLPAIRS.
- * skin >= 0 is the VERLET list margin in length units; 0 selects the default 0.16 r_cut. */
+ * skin >= 0 is the VERLET list margin in length units; 0 selects the default 0.24 r_cut. */
 typedef struct { double dt, mass; int precision, force_algo; double skin; } md_opts;
 
 /* potential = potential_vv + potential_vw = sum_i pe_i; virial = sum over unordered vv pairs and

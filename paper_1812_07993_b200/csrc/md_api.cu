@@ -81,7 +81,7 @@ const char* validate(const md_box* box, const md_lj* lj, const md_opts* o, long 
     return nullptr;
 }
 
-double list_skin(const md_lj& lj, const md_opts& o) { return o.skin > 0 ? o.skin : 0.16 * lj.r_cut; }
+double list_skin(const md_lj& lj, const md_opts& o) { return o.skin > 0 ? o.skin : 0.24 * lj.r_cut; }
 
 // Grid the handle uses: cells of side >= r_cut (CELLS) or >= r_cut + skin (VERLET).
 GridSpec grid_for(const md_box& box, const md_lj& lj, const md_opts& o, int algo)
@@ -159,10 +159,10 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.eout = c.take<double>(8);
     l.err = c.take<int>(4);
     l.tests = c.take<unsigned long long>(2);
-    l.nbr = c.take<int>(verlet ? (size_t)nv * md::VL_MAXN : 1);
+    l.nbr = c.take<int>(verlet ? n * md::VL_MAXN : 1);
     l.ncnt = c.take<int>(verlet ? n : 1);
     l.vflags = c.take<int>(md::VF_COUNT);
-    l.vtimes = c.take<unsigned long long>(8);
+    l.vtimes = c.take<unsigned long long>(8 + 8192);
     l.stage0 = c.take<double>(n * dim);
     l.stage1 = c.take<double>(n * dim);
     l.wstage = c.take<double>(m * dim);
@@ -233,8 +233,9 @@ struct Sim : md_sim {
             CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
             CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, md::VL_THREADS, 0));
             if (nb < 1) { err = "persistent kernel does not fit on an SM"; return MD_ERR_CUDA; }
-            const int want = cdiv((long long)p.nv * md::VL_G, md::VL_THREADS);
-            coop_grid = std::max(1, std::min(nb * sms, want));
+            // one thread per particle; whole multiples of the SM count keep the SMs evenly loaded
+            const int want = cdiv(cdiv(p.nv, md::VL_THREADS), sms) * sms;
+            coop_grid = std::max(1, std::min(nb * sms, p.nv <= md::VL_THREADS * sms ? cdiv(p.nv, md::VL_THREADS) : want));
         }
         CK(cudaMemsetAsync(l.vflags + md::VF_REQ0, 0, 3 * sizeof(int), stream));   // rebuild-request slots
         void* args[] = {(void*)&p, (void*)&vl, (void*)&n, (void*)&force_rebuild};
@@ -280,7 +281,7 @@ struct Sim : md_sim {
     {
         if (verlet()) {
             if (ENERGY)
-                md::k_verlet_energy<T><<<cdiv((long long)p.nv * md::VL_G, md::VL_THREADS), md::VL_THREADS, 0, stream>>>(
+                md::k_verlet_energy<T><<<cdiv(p.nv, md::VL_THREADS), md::VL_THREADS, 0, stream>>>(
                     p, vl, cur, l.eo);
         } else if (algo == MD_FORCE_CELLS) {
             // ROWS lanes per particle: 9 in 3D (3 particles per warp), 3 in 2D (10 per warp)
@@ -379,6 +380,16 @@ struct Sim : md_sim {
             CK(cudaEventElapsedTime(&ms, ev[0], ev[1]));
             unsigned long long t[8];
             CK(cudaMemcpy(t, l.vtimes, sizeof(t), cudaMemcpyDeviceToHost));
+            if (getenv("MD_DEBUG_TIMES")) {
+                std::vector<unsigned long long> w(8192);
+                CK(cudaMemcpy(w.data(), l.vtimes + 8, 8192 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+                const int nwarp = coop_grid * md::VL_THREADS / 32;
+                fprintf(stderr, "[md] per-warp cumulative step-phase us (every 37th of %d warps):", nwarp);
+                for (int k = 0; k < nwarp && k < 8192; k += 37) fprintf(stderr, " %.0f", w[k] * 1e-3);
+                unsigned long long mx = 0, sm = 0;
+                for (int k = 0; k < nwarp && k < 8192; ++k) { mx = std::max(mx, w[k]); sm += w[k]; }
+                fprintf(stderr, "\n[md] max %.0f us mean %.0f us\n", mx * 1e-3, sm * 1e-3 / nwarp);
+            }
             if (getenv("MD_DEBUG_TIMES"))
                 fprintf(stderr, "[md] cumulative ns: step %llu barrier %llu rebuild %llu final %llu | bin %llu scan %llu "
                         "scatter %llu build %llu\n", t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7]);
@@ -572,7 +583,7 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
     if (verlet()) {
         // walls (cell order) appended to both position buffers; then bin + list + f(0) in one persistent launch
         CK(cudaMemsetAsync(l.vflags, 0, sizeof(int) * md::VF_COUNT, stream));
-        CK(cudaMemsetAsync(l.vtimes, 0, 8 * sizeof(unsigned long long), stream));
+        CK(cudaMemsetAsync(l.vtimes, 0, (8 + 8192) * sizeof(unsigned long long), stream));
         CK(cudaMemsetAsync(l.tile_sum, 0, sizeof(int) * (size_t)(cdiv(p.ncell, md::SCAN_TILE) + 1), stream));
         if (nw > 0)
             for (int b = 0; b < 2; ++b)
@@ -636,9 +647,9 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
         const double skin = list_skin(lj, o), rl = lj.r_cut + skin;
         md::Verlet<T>& v = s->vl;
         v.st[0] = s->l.st[0]; v.st[1] = s->l.st[1]; v.f = s->l.f;
-        v.nbr = s->l.nbr; v.ncnt = s->l.ncnt;
+        v.nbr = s->l.nbr; v.ncnt = s->l.ncnt; v.stride = align_up((size_t)nv, 64);
         v.cell = s->l.cell; v.slot = s->l.slot; v.count = s->l.count; v.start = s->l.start; v.tile_sum = s->l.tile_sum;
-        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.times = s->l.vtimes;
+        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.times = s->l.vtimes; v.dbg = getenv("MD_DEBUG_TIMES") ? s->l.vtimes + 8 : nullptr;
         v.rl2 = (T)(rl * rl); v.half_skin = (T)(0.5 * skin);
     }
     int rc = s->init(box, lj, o, nv, pos, vel, nw, wall);

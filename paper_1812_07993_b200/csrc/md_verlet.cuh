@@ -19,7 +19,6 @@ namespace md {
 namespace cg = cooperative_groups;
 
 constexpr int VL_THREADS = 256;
-constexpr int VL_G = 8;        // lanes cooperating on one particle in the force phase
 constexpr int VL_MAXN = 128;   // neighbour-list stride (entries per particle)
 
 // flags: rebuild request, list overflow, position-buffer parity, velocity/id-buffer parity, rebuild count, escape
@@ -34,11 +33,13 @@ struct Verlet {
     // static); st[cv].{vx,vy,vz,id}: owner-only data, swapped only by the rebuild's scatter
     State<T> st[2];
     Force<T> f;
-    int *nbr, *ncnt;           // [nv * VL_MAXN], [nv]; j >= nv means wall particle j - nv
+    int *nbr, *ncnt;           // nbr[k * stride + i], k < VL_MAXN; ncnt[nv]; j >= nv means wall particle j - nv
+    size_t stride;             // >= nv
     int *cell, *slot, *count, *start, *tile_sum;
     const int* wstart;         // walls: [ncell + 1] ranges into the wall tail
     const uint8_t* wnear;
     int* flags;                // VF_*
+    unsigned long long* dbg;   // optional per-warp step-phase ns (diagnostics), or nullptr
     unsigned long long* times; // [8] ns seen by thread 0: step phases, step barriers, rebuilds, final phase,
                                // rebuild split: bin, scan, scatter, list build (each with its barrier)
     T rl2, half_skin;          // (r_c + skin)^2, skin / 2
@@ -68,43 +69,82 @@ __device__ __forceinline__ unsigned long long now_ns()
     return t;
 }
 
-template <typename V>
-__device__ __forceinline__ V group_sum(V v)
-{
-#pragma unroll
-    for (int o = VL_G / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// ---- one particle's force from its neighbour list, VL_G lanes ---------------------------------
+// ---- one particle's force from its neighbour list, one thread per particle ----------------------
+// The list is stored transposed, nbr[k * stride + i], so a warp's loads of entry k are coalesced.
 // ncnt[i] = list length | VL_FOLD if the particle sat in a cell on a periodic face when the list was
 // built: only such particles can have a neighbour across the face, all others skip the image folding.
+// Entries are consumed four at a time: four index loads, then four position loads, are in flight together.
 constexpr int VL_FOLD = 1 << 30;
 
+// 1 / x without the division's special-case branch: hardware seed (>= 20 bits) + two Newton steps.
+__device__ __forceinline__ double rcp_fast(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+__device__ __forceinline__ float rcp_fast(float x) { return 1.0f / x; }
+
+// Branch-free pair term: the four pairs of a batch form four independent dependency chains.
+template <typename T, bool ENERGY>
+__device__ __forceinline__ void pair_term_nb(const Params<T>& p, bool valid, bool wall, T dx, T dy, T dz,
+                                             Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
+{
+    const T r2 = fma_(dz, dz, fma_(dy, dy, dx * dx));
+    const bool hit = valid && r2 < p.rc2;                   // strict, same r^2 arithmetic as every other path
+    const T inv = rcp_fast(hit ? r2 : T(1));
+    const T s = (wall ? p.sig2_vw : p.sig2_vv) * inv;
+    const T s3 = s * s * s;
+    const T s6 = s3 * s3;
+    const T g = hit ? (wall ? p.e24_vw : p.e24_vv) * inv * (T(2) * s6 - s3) : T(0);
+    const T gw = wall ? g : T(0), gv = wall ? T(0) : g;
+    av.fx = fma_(gv, dx, av.fx); av.fy = fma_(gv, dy, av.fy); av.fz = fma_(gv, dz, av.fz);
+    aw.fx = fma_(gw, dx, aw.fx); aw.fy = fma_(gw, dy, aw.fy); aw.fz = fma_(gw, dz, aw.fz);
+    if (ENERGY) {
+        const double u = hit ? (double)((wall ? p.e4_vw : p.e4_vv) * (s6 - s3) - (wall ? p.uc_vw : p.uc_vv)) : 0.0;
+        const double w = (double)(g * r2);
+        if (wall) { aw.u += u; aw.w += w; aw.c += hit; }
+        else { av.u += u; av.w += w; av.c += hit; }
+    }
+}
+
 template <typename T, bool ENERGY, bool FOLD>
-__device__ __forceinline__ void list_loop(const Params<T>& p, const int* __restrict__ lst, int n, const Vec4<T>* __restrict__ r,
-                                          int g, const Vec4<T>& ri, Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
+__device__ __forceinline__ void list_loop(const Params<T>& p, const int* __restrict__ lst, size_t stride, int n,
+                                          const Vec4<T>* __restrict__ r, const Vec4<T>& ri, Acc<T, ENERGY>& av,
+                                          Acc<T, ENERGY>& aw)
 {
     const bool px = FOLD && p.bc[0] == BC_PERIODIC, py = FOLD && p.bc[1] == BC_PERIODIC, pz = FOLD && p.bc[2] == BC_PERIODIC;
-    for (int k = g; k < n; k += VL_G) {
-        const int j = lst[k];
-        const Vec4<T> rj = r[j];
-        const T dx = px ? fold(ri.x, rj.x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj.x;
-        const T dy = py ? fold(ri.y, rj.y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj.y;
-        const T dz = pz ? fold(ri.z, rj.z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj.z;
-        if (j < p.nv) pair_term<T, ENERGY>(dx, dy, dz, p.rc2, p.sig2_vv, p.e24_vv, p.e4_vv, p.uc_vv, av);
-        else pair_term<T, ENERGY>(dx, dy, dz, p.rc2, p.sig2_vw, p.e24_vw, p.e4_vw, p.uc_vw, aw);
+    int jn[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) jn[u] = u < n ? lst[(size_t)u * stride] : -1;
+    for (int k = 0; k < n; k += 4) {
+        int j[4];
+        Vec4<T> rj[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { j[u] = jn[u]; rj[u] = r[max(j[u], 0)]; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) jn[u] = k + 4 + u < n ? lst[(size_t)(k + 4 + u) * stride] : -1;   // next batch
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
+            const T dy = py ? fold(ri.y, rj[u].y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj[u].y;
+            const T dz = pz ? fold(ri.z, rj[u].z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj[u].z;
+            pair_term_nb<T, ENERGY>(p, j[u] >= 0, j[u] >= p.nv, dx, dy, dz, av, aw);
+        }
     }
 }
 
 template <typename T, bool ENERGY>
 __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& v, const Vec4<T>* __restrict__ r, int i,
-                                           int g, const Vec4<T>& ri, Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
+                                           const Vec4<T>& ri, Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
     const int raw = v.ncnt[i];
-    const int* __restrict__ lst = v.nbr + (size_t)i * VL_MAXN;
-    if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, raw & (VL_FOLD - 1), r, g, ri, av, aw);
-    else list_loop<T, ENERGY, false>(p, lst, raw, r, g, ri, av, aw);
+    const int* __restrict__ lst = v.nbr + i;
+    if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & (VL_FOLD - 1), r, ri, av, aw);
+    else list_loop<T, ENERGY, false>(p, lst, v.stride, raw, r, ri, av, aw);
 }
 
 // ---- phase: [forces] -> [kick completing the step] -> [kick + drift of the next step] -----------
@@ -115,55 +155,38 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
                                            bool kick, bool drift, int req, int gtid, int gthreads)
 {
     const Vec4<T>* __restrict__ rcur = v.st[c].r;
-    T* __restrict__ rnew = reinterpret_cast<T*>(v.st[c ^ 1].r);
+    Vec4<T>* __restrict__ rnew = v.st[c ^ 1].r;
     const State<T>& s = v.st[cv];
-    const int g = gtid & (VL_G - 1);
-    const int ngroups = gthreads / VL_G;
-    // after the group reduction every lane holds f_i: lane g < 3 integrates component g (x, y, z)
-    T* __restrict__ vcomp = g == 0 ? s.vx : (g == 1 ? s.vy : s.vz);
-    T* __restrict__ fcomp = g == 0 ? v.f.fx : (g == 1 ? v.f.fy : v.f.fz);
-    const T Lg = p.L[g < 3 ? g : 0];
-    const int bcg = g < 3 ? p.bc[g] : BC_NONE;
-    for (int i0 = gtid / VL_G; i0 < ((p.nv + 3) & ~3); i0 += ngroups) {     // whole warps stay in the loop together
-        const int i = min(i0, p.nv - 1);
+    for (int i = gtid; i < p.nv; i += gthreads) {
         const Vec4<T> ri = rcur[i];
-        T vg = T(0);
-        if (g < 3) vg = vcomp[i];                     // issued early, consumed after the force loop
+        T vx = s.vx[i], vy = s.vy[i], vz = s.vz[i];      // issued early, consumed after the force loop
         T fx, fy, fz;
         if (force) {
             Acc<T, false> av, aw;
-            list_force<T, false>(p, v, rcur, i, g, ri, av, aw);
-            fx = group_sum(av.fx + aw.fx);
-            fy = group_sum(av.fy + aw.fy);
-            fz = group_sum(av.fz + aw.fz);
+            list_force<T, false>(p, v, rcur, i, ri, av, aw);
+            fx = av.fx + aw.fx; fy = av.fy + aw.fy; fz = av.fz + aw.fz;
+            v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz;
         } else {
             fx = v.f.fx[i]; fy = v.f.fy[i]; fz = v.f.fz[i];
         }
-        const bool mine = g < 3 && i0 < p.nv;
-        const T fg = g == 0 ? fx : (g == 1 ? fy : fz);
-        const T rg = g == 0 ? ri.x : (g == 1 ? ri.y : ri.z);
-        if (mine && force) fcomp[i] = fg;
-        if (kick) vg = vg + p.hk * fg;                 // F3: v(t) = v(t - dt/2) + (dt/2m) f(t)
-        T step2 = T(0);
+        if (kick) {                                    // F3: v(t) = v(t - dt/2) + (dt/2m) f(t)
+            vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
+        }
         if (drift) {                                   // F2: v(t + dt/2), r(t + dt)
-            vg = vg + p.hk * fg;
-            const T sg = p.dt * vg;
-            T rn = rg + sg;
+            vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
+            const T sx = p.dt * vx, sy = p.dt * vy, sz = p.dt * vz;
+            Vec4<T> rn;
+            rn.x = ri.x + sx; rn.y = ri.y + sy; rn.z = ri.z + sz;
             // periodic dimensions are left unwrapped until the next rebuild; reflection is immediate
-            if (mine && bcg == BC_REFLECT) boundary(rn, vg, Lg, BC_REFLECT, v.flags + VF_ESCAPE);
-            if (mine) rnew[4 * (size_t)i + g] = rn;
-            step2 = g < 3 ? sg * sg : T(0);
+            int* err = v.flags + VF_ESCAPE;
+            if (p.bc[0] == BC_REFLECT) boundary(rn.x, vx, p.L[0], BC_REFLECT, err);
+            if (p.bc[1] == BC_REFLECT) boundary(rn.y, vy, p.L[1], BC_REFLECT, err);
+            if (p.bc[2] == BC_REFLECT) boundary(rn.z, vz, p.L[2], BC_REFLECT, err);
+            rn.w = ri.w + sqrt(sx * sx + sy * sy + sz * sz);      // path length >= displacement
+            if (rn.w > v.half_skin) v.flags[VF_REQ0 + req] = 1;
+            rnew[i] = rn;
         }
-        if (mine && (kick || drift)) vcomp[i] = vg;
-        if (drift) {                                   // path length since the last rebuild (>= displacement)
-            step2 += __shfl_xor_sync(0xffffffffu, step2, 1);
-            step2 += __shfl_xor_sync(0xffffffffu, step2, 2);
-            if (g == 3 && i0 < p.nv) {
-                const T w = ri.w + sqrt(step2);
-                rnew[4 * (size_t)i + 3] = w;
-                if (w > v.half_skin) v.flags[VF_REQ0 + req] = 1;
-            }
-        }
+        if (kick || drift) { s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz; }
     }
 }
 
@@ -224,7 +247,12 @@ __device__ __forceinline__ void phase_scan_apply(int* __restrict__ count, int n,
         if (tile_sum) {
             for (int k = threadIdx.x; k < t; k += SCAN_THREADS) off += tile_sum[k];
         } else {            // few tiles: sum the earlier counts directly and save a phase + barrier
-            for (int k = threadIdx.x; k < t * SCAN_TILE; k += SCAN_THREADS) off += count[k];
+            const int4* __restrict__ c4 = reinterpret_cast<const int4*>(count);     // t * SCAN_TILE is a multiple of 4
+#pragma unroll 8
+            for (int k = threadIdx.x; k < t * (SCAN_TILE / 4); k += SCAN_THREADS) {
+                const int4 q = c4[k];
+                off += q.x + q.y + q.z + q.w;
+            }
         }
         off = warp_sum(off);
         __syncthreads();
@@ -284,19 +312,24 @@ __device__ __forceinline__ void phase_scatter(const Params<T>& p, const Verlet<T
 // appends its hits through a shared-memory counter.  Positions are wrapped here, so distances fold.
 template <typename T>
 __device__ __forceinline__ void list_range(const Params<T>& p, const Vec4<T>* __restrict__ r, int jb, int je, int skip,
-                                           const Vec4<T>& ri, T rl2, int* __restrict__ lst, int* cnt)
+                                           const Vec4<T>& ri, T rl2, int* __restrict__ lst, size_t stride, int* cnt)
 {
     const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
-    for (int j = jb; j < je; ++j) {
-        if (j == skip) continue;
-        const Vec4<T> rj = r[j];
-        const T dx = px ? fold(ri.x, rj.x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj.x;
-        const T dy = py ? fold(ri.y, rj.y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj.y;
-        const T dz = pz ? fold(ri.z, rj.z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj.z;
-        const T r2 = fma_(dz, dz, fma_(dy, dy, dx * dx));
-        if (r2 < rl2) {
-            const int k = atomicAdd(cnt, 1);
-            if (k < VL_MAXN) lst[k] = j;
+    for (int j0 = jb; j0 < je; j0 += 4) {
+        Vec4<T> rj[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) rj[u] = r[min(j0 + u, je - 1)];      // four loads in flight
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int j = j0 + u;
+            const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
+            const T dy = py ? fold(ri.y, rj[u].y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj[u].y;
+            const T dz = pz ? fold(ri.z, rj[u].z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj[u].z;
+            const T r2 = fma_(dz, dz, fma_(dy, dy, dx * dx));
+            if (j < je && j != skip && r2 < rl2) {
+                const int k = atomicAdd(cnt, 1);
+                if (k < VL_MAXN) lst[(size_t)k * stride] = j;
+            }
         }
     }
 }
@@ -321,7 +354,7 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
             const Vec4<T> ri = r[i];
             int cx, cy, cz;
             const int ci = cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
-            int* __restrict__ lst = v.nbr + (size_t)i * VL_MAXN;
+            int* __restrict__ lst = v.nbr + i;
             int qy = cy + row % 3 - 1, qz = cz + (ROWS == 9 ? row / 3 - 1 : 0);
             bool ok = true;
             if (qz < 0) { ok = p.bc[2] == BC_PERIODIC; qz += nz; }
@@ -341,10 +374,10 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
                     wb = v.wstart[rowc + x0]; we = v.wstart[rowc + x1 + 1];
                     if (xw >= 0) { wb2 = v.wstart[rowc + xw]; we2 = v.wstart[rowc + xw + 1]; }
                 }
-                list_range<T>(p, r, jb, je, i, ri, v.rl2, lst, cnt);
-                list_range<T>(p, r, jb2, je2, i, ri, v.rl2, lst, cnt);
-                list_range<T>(p, r, p.nv + wb, p.nv + we, -1, ri, v.rl2, lst, cnt);
-                list_range<T>(p, r, p.nv + wb2, p.nv + we2, -1, ri, v.rl2, lst, cnt);
+                list_range<T>(p, r, jb, je, i, ri, v.rl2, lst, v.stride, cnt);
+                list_range<T>(p, r, jb2, je2, i, ri, v.rl2, lst, v.stride, cnt);
+                list_range<T>(p, r, p.nv + wb, p.nv + we, -1, ri, v.rl2, lst, v.stride, cnt);
+                list_range<T>(p, r, p.nv + wb2, p.nv + we2, -1, ri, v.rl2, lst, v.stride, cnt);
             }
         }
         __syncwarp();
@@ -368,7 +401,7 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
 // phase(force; kick): n + 1 phases and n grid barriers for n steps, plus 5 barriers per rebuild.
 // force_rebuild (md_create): bin + build the list first, then evaluate f(0).
 template <typename T, int ROWS>
-__global__ void __launch_bounds__(VL_THREADS, 4) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
+__global__ void __launch_bounds__(VL_THREADS, 2) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
 {
     cg::grid_group grid = cg::this_grid();
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -403,7 +436,10 @@ __global__ void __launch_bounds__(VL_THREADS, 4) k_md_run(Params<T> p, Verlet<T>
         if (s == n_steps) break;
         const int req = (int)(s % 3);
         if (gtid == 0) v.flags[VF_REQ0 + (req + 1) % 3] = 0;      // slot of step s + 1
+        unsigned long long dbg0 = 0;
+        if (v.dbg) dbg0 = now_ns();
         phase_step<T>(p, v, c, cv, s > 0, s > 0, true, req, gtid, gthreads);
+        if (v.dbg && (threadIdx.x & 31) == 0) atomicAdd(v.dbg + (gtid >> 5), now_ns() - dbg0);
         if (gtid == 0) { t1 = now_ns(); v.times[0] += t1 - t0; t0 = t1; }
         grid.sync();
         if (gtid == 0) { t1 = now_ns(); v.times[1] += t1 - t0; t0 = t1; }
@@ -418,22 +454,17 @@ __global__ void __launch_bounds__(VL_THREADS, 4) k_md_run(Params<T> p, Verlet<T>
 template <typename T>
 __global__ void __launch_bounds__(VL_THREADS) k_verlet_energy(Params<T> p, Verlet<T> v, int c, EnergyOut eo)
 {
-    const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
-    const int g = gtid & (VL_G - 1);
-    const int i0 = gtid / VL_G;
-    const int i = min(i0, p.nv - 1);
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.nv) return;
     const Vec4<T>* __restrict__ r = v.st[c].r;
     const Vec4<T> ri = r[i];
     Acc<T, true> av, aw;
-    list_force<T, true>(p, v, r, i, g, ri, av, aw);
-    const double uv = group_sum(av.u), uw = group_sum(aw.u), wv = group_sum(av.w), ww = group_sum(aw.w);
-    const int cvv = group_sum(av.c), cvw = group_sum(aw.c);
-    if (g != 0 || i0 >= p.nv) return;
-    eo.pe[i] = 0.5 * uv + uw;
-    eo.pew[i] = uw;
-    eo.vir[i] = 0.5 * wv + ww;
-    eo.cvv[i] = cvv;
-    eo.cvw[i] = cvw;
+    list_force<T, true>(p, v, r, i, ri, av, aw);
+    eo.pe[i] = 0.5 * av.u + aw.u;
+    eo.pew[i] = aw.u;
+    eo.vir[i] = 0.5 * av.w + aw.w;
+    eo.cvv[i] = av.c;
+    eo.cvw[i] = aw.c;
 }
 
 } // namespace md

@@ -84,8 +84,8 @@ def test_config0_forces_and_trajectory(algo):
 @pytest.mark.parametrize("dim,box,bc,nw,seed", [
     (3, (8.0, 9.3, 7.6), (0, 0, 0), 40, 1), (3, (8.1, 7.5, 5.2), (0, 0, 1), 40, 2), (3, (4.0, 8.0, 8.0), (1, 0, 0), 0, 3),
     (2, (13.7, 9.9), (0, 1), 12, 4), (2, (7.5, 7.5), (0, 0), 12, 5), (2, (2.6, 30.0), (1, 0), 5, 6),
-    (3, (3.0, 3.0, 3.0), (1, 1, 1), 2, 7), (3, (9.0, 10.5, 9.3), (0, 0, 0), 30, 8), (3, (9.5, 9.0, 5.2), (0, 0, 1), 30, 9),
-    (2, (12.0, 9.0), (0, 0), 10, 10)])
+    (3, (3.0, 3.0, 3.0), (1, 1, 1), 2, 7), (3, (9.6, 10.5, 9.9), (0, 0, 0), 30, 8), (3, (9.5, 9.6, 5.2), (0, 0, 1), 30, 9),
+    (2, (12.0, 9.6), (0, 0), 10, 10)])
 @pytest.mark.parametrize("algo", ALGOS)
 def test_small_ragged_cases(dim, box, bc, nw, seed, algo):
     vol = float(np.prod(box))
@@ -100,7 +100,7 @@ def test_small_ragged_cases(dim, box, bc, nw, seed, algo):
 
 
 def test_single_particle_and_no_walls():
-    cfg = I.small_case(3, 1, (9.0, 9.0, 9.0), (0, 1, 0), seed=3)
+    cfg = I.small_case(3, 1, (10.0, 10.0, 10.0), (0, 1, 0), seed=3)
     for algo in ALGOS:
         sim = md.Simulation(cfg, algo=algo)
         sim.step(10)
