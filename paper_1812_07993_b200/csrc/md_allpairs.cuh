@@ -1,0 +1,210 @@
+// md_allpairs.cuh -- variant A of a3 for fp64: all-pairs force kernel bound by the FP64 pipe.
+//
+// The paper's F1 tests every pair (Fig. 1 at :69-73).  With r_c = 2.5 sigma only ~5e-5 of
+// the tests at N = 65,536 are hits, so the kernel is the distance TEST, and the test is written to cost
+// four FP64 instructions:
+//     r^2 = (|r_i|^2 + |r_j|^2) - 2 x_i x_j - 2 y_i y_j - 2 z_i z_j      1 DADD + 3 DFMA  (7 flops)
+// with (x_j, y_j, z_j, |r_j|^2) staged through shared memory as one 32-byte entry, four particles i per
+// thread in registers, and the comparison done on the high word of r^2 by the integer pipe.  That form
+// loses ~1e-12 absolute in r^2, so it is only a conservative FILTER (threshold r_c^2 + margin): a group
+// of tests with any candidate re-evaluates its pairs exactly -- d = r_i - r_j, r^2 = fma(dz,dz,fma(dy,dy,
+// dx*dx)), strict r^2 < r_c^2 -- and only that exact path produces forces and energies.
+// Periodic images are materialised once per step as ghost entries (particles within r_c of a periodic
+// face), so the inner loop has no minimum-image arithmetic.  Coordinates are centred on the box middle
+// to halve |r|^2.  fp32 mode keeps the per-pair minimum-image kernel of md_kernels.cuh.
+#pragma once
+#include "md_kernels.cuh"
+
+namespace md {
+
+constexpr int AD_THREADS = 128;   // threads per block = entries per shared-memory tile
+constexpr int AD_IB = 4;          // particles i per thread
+constexpr int AD_UNROLL = 8;      // tests per i between two candidate checks
+
+struct AllPairsDot {
+    Vec4<double>* jv;      // [nv + cap_ghost]: real vapor entries in particle order, then this step's ghosts
+    Vec4<double>* jw;      // [nwg]: wall particles and their ghosts (static)
+    int* ghost_count;      // number of vapor ghosts appended this step
+    int nwg;
+    int thr_hi;            // candidate iff hi32(r^2 filter value) < thr_hi
+    double half[3];        // box centre
+    double edge;           // r_c + margin: distance from a periodic face that spawns a ghost
+};
+
+// Appends (x, y, z) -- already centred -- and its periodic images to a j list.
+__device__ __forceinline__ void push_images(const Params<double>& p, const AllPairsDot& a, double x, double y, double z,
+                                            Vec4<double>* __restrict__ out, int base, int* __restrict__ counter)
+{
+    // shift options per dimension: 0, and +-L when within `edge` of the opposite face
+    double sx[2] = {0.0, 0.0}, sy[2] = {0.0, 0.0}, sz[2] = {0.0, 0.0};
+    int nx = 1, ny = 1, nz = 1;
+    if (p.bc[0] == BC_PERIODIC) { if (x < a.edge - a.half[0]) sx[nx++] = p.L[0]; else if (x > a.half[0] - a.edge) sx[nx++] = -p.L[0]; }
+    if (p.bc[1] == BC_PERIODIC) { if (y < a.edge - a.half[1]) sy[ny++] = p.L[1]; else if (y > a.half[1] - a.edge) sy[ny++] = -p.L[1]; }
+    if (p.bc[2] == BC_PERIODIC) { if (z < a.edge - a.half[2]) sz[nz++] = p.L[2]; else if (z > a.half[2] - a.edge) sz[nz++] = -p.L[2]; }
+    for (int c = 0; c < nz; ++c)
+        for (int b = 0; b < ny; ++b)
+            for (int q = 0; q < nx; ++q) {
+                if (q + b + c == 0) continue;
+                Vec4<double> e;
+                e.x = x + sx[q]; e.y = y + sy[b]; e.z = z + sz[c];
+                e.w = fma(e.z, e.z, fma(e.y, e.y, e.x * e.x));
+                out[base + atomicAdd(counter, 1)] = e;
+            }
+}
+
+// a1 for the all-pairs path: half-kick + drift + boundary, then the step's j list (entry + ghosts); f is
+// cleared for the force kernel's accumulation.  MOVE = false only builds the list (md_create).
+template <bool MOVE>
+__global__ void __launch_bounds__(256) k_ap_kick_drift_list(Params<double> p, State<double> s, Force<double> f,
+                                                            AllPairsDot a, int* __restrict__ err)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.nv) return;
+    Vec4<double> ri = s.r[i];
+    if (MOVE) {
+        double vx = s.vx[i] + p.hk * f.fx[i];
+        double vy = s.vy[i] + p.hk * f.fy[i];
+        double vz = s.vz[i] + p.hk * f.fz[i];
+        ri.x += p.dt * vx; ri.y += p.dt * vy; ri.z += p.dt * vz;
+        boundary(ri.x, vx, p.L[0], p.bc[0], err);
+        boundary(ri.y, vy, p.L[1], p.bc[1], err);
+        boundary(ri.z, vz, p.L[2], p.bc[2], err);
+        s.r[i] = ri;
+        s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz;
+    }
+    f.fx[i] = 0.0; f.fy[i] = 0.0; f.fz[i] = 0.0;
+    Vec4<double> e;
+    e.x = ri.x - a.half[0]; e.y = ri.y - a.half[1]; e.z = ri.z - a.half[2];
+    e.w = fma(e.z, e.z, fma(e.y, e.y, e.x * e.x));
+    a.jv[i] = e;
+    push_images(p, a, e.x, e.y, e.z, a.jv, p.nv, a.ghost_count);
+}
+
+// Static wall list (md_create): entry + ghosts of every wall particle.
+__global__ void k_ap_wall_list(Params<double> p, const Vec4<double>* __restrict__ wr, AllPairsDot a, int* __restrict__ counter)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.nw) return;
+    Vec4<double> e;
+    e.x = wr[i].x - a.half[0]; e.y = wr[i].y - a.half[1]; e.z = wr[i].z - a.half[2];
+    e.w = fma(e.z, e.z, fma(e.y, e.y, e.x * e.x));
+    a.jw[i] = e;
+    push_images(p, a, e.x, e.y, e.z, a.jw, p.nw, counter);
+}
+
+// a4 for the all-pairs path: second half-kick once every block's force contributions have landed; also
+// re-arms the ghost counter for the next step.
+__global__ void __launch_bounds__(256) k_ap_kick(Params<double> p, State<double> s, Force<double> f, int* __restrict__ ghost_count)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) *ghost_count = 0;
+    if (i >= p.nv) return;
+    s.vx[i] = s.vx[i] + p.hk * f.fx[i];
+    s.vy[i] = s.vy[i] + p.hk * f.fy[i];
+    s.vz[i] = s.vz[i] + p.hk * f.fz[i];
+}
+
+// Exact re-evaluation of one (i, j) pair found by the filter (reading A2: strict r^2 < r_c^2).
+template <bool ENERGY>
+__device__ __forceinline__ void ap_exact(const Params<double>& p, bool wall, double xi, double yi, double zi,
+                                         const Vec4<double>& q, double& fx, double& fy, double& fz, double& u, double& w,
+                                         int& c)
+{
+    const double dx = xi - q.x, dy = yi - q.y, dz = zi - q.z;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    if (r2 < p.rc2) {
+        const double inv = 1.0 / r2;
+        const double s = (wall ? p.sig2_vw : p.sig2_vv) * inv;
+        const double s3 = s * s * s, s6 = s3 * s3;
+        const double g = (wall ? p.e24_vw : p.e24_vv) * inv * (2.0 * s6 - s3);
+        fx = fma(g, dx, fx); fy = fma(g, dy, fy); fz = fma(g, dz, fz);
+        if (ENERGY) {
+            u += (wall ? p.e4_vw : p.e4_vv) * (s6 - s3) - (wall ? p.uc_vw : p.uc_vv);
+            w += g * r2;
+            c += 1;
+        }
+    }
+}
+
+// grid = (i blocks, j slices).  Block (bi, sj) owns particles [bi * 512, bi * 512 + 512) (thread t: i = base +
+// t + 128 b, b < 4) and the tiles t with t % gridDim.y == sj of the j lists (vapor + ghosts, then walls).
+// Forces are accumulated with fp64 atomics (f was cleared by k_ap_kick_drift_list); ENERGY instead
+// accumulates pe, pe_w, virial and hit counts (cleared by the host) and leaves f alone.
+template <bool ENERGY>
+__global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double> p, AllPairsDot a, Force<double> f,
+                                                                   EnergyOut eo)
+{
+    __shared__ Vec4<double> sj[AD_THREADS];
+    const int base = blockIdx.x * (AD_THREADS * AD_IB) + threadIdx.x;
+    double ax[AD_IB], ay[AD_IB], az[AD_IB], si[AD_IB];      // -2 x_i, -2 y_i, -2 z_i, |r_i|^2
+    int idx[AD_IB];
+#pragma unroll
+    for (int b = 0; b < AD_IB; ++b) {
+        idx[b] = base + b * AD_THREADS;
+        // particles beyond nv: parked far away so that they never pass the filter
+        Vec4<double> e = {1.0e9, 1.0e9, 1.0e9, 3.0e18};
+        if (idx[b] < p.nv) e = a.jv[idx[b]];
+        ax[b] = -2.0 * e.x; ay[b] = -2.0 * e.y; az[b] = -2.0 * e.z; si[b] = e.w;
+    }
+    double fx[AD_IB] = {}, fy[AD_IB] = {}, fz[AD_IB] = {}, uv[AD_IB] = {}, uw[AD_IB] = {}, wv[AD_IB] = {}, ww[AD_IB] = {};
+    int cv[AD_IB] = {}, cw[AD_IB] = {};
+    bool any = false;
+    const int nvj = p.nv + *a.ghost_count;
+    const int tiles_v = (nvj + AD_THREADS - 1) / AD_THREADS, tiles_w = (a.nwg + AD_THREADS - 1) / AD_THREADS;
+    const int thr = a.thr_hi;
+    for (int t = blockIdx.y; t < tiles_v + tiles_w; t += gridDim.y) {
+        const bool wall = t >= tiles_v;
+        const int j0 = (wall ? t - tiles_v : t) * AD_THREADS;
+        const int nj = wall ? a.nwg : nvj;
+        __syncthreads();
+        {
+            Vec4<double> e = {-1.0e9, -1.0e9, -1.0e9, 3.0e18};          // padding: far from everything
+            if (j0 + threadIdx.x < nj) e = (wall ? a.jw : a.jv)[j0 + threadIdx.x];
+            sj[threadIdx.x] = e;
+        }
+        __syncthreads();
+        for (int k0 = 0; k0 < AD_THREADS; k0 += AD_UNROLL) {
+            int cand = 0;
+#pragma unroll
+            for (int u = 0; u < AD_UNROLL; ++u) {
+                const Vec4<double> q = sj[k0 + u];
+#pragma unroll
+                for (int b = 0; b < AD_IB; ++b) {
+                    const double r2 = fma(ax[b], q.x, fma(ay[b], q.y, fma(az[b], q.z, si[b] + q.w)));
+                    cand |= (__double2hiint(r2) < thr);
+                }
+            }
+            if (cand) {      // rare: redo this group's pairs exactly
+                for (int u = 0; u < AD_UNROLL; ++u) {
+                    const Vec4<double> q = sj[k0 + u];
+#pragma unroll
+                    for (int b = 0; b < AD_IB; ++b) {
+                        if (!wall && j0 + k0 + u == idx[b]) continue;          // j == i skipped by index
+                        if (wall) ap_exact<ENERGY>(p, true, -0.5 * ax[b], -0.5 * ay[b], -0.5 * az[b], q, fx[b], fy[b], fz[b], uw[b], ww[b], cw[b]);
+                        else ap_exact<ENERGY>(p, false, -0.5 * ax[b], -0.5 * ay[b], -0.5 * az[b], q, fx[b], fy[b], fz[b], uv[b], wv[b], cv[b]);
+                    }
+                }
+                any = true;
+            }
+        }
+    }
+    if (!any) return;
+#pragma unroll
+    for (int b = 0; b < AD_IB; ++b) {
+        const int i = idx[b];
+        if (i >= p.nv) continue;
+        if (!ENERGY) {
+            if (fx[b] != 0.0 || fy[b] != 0.0 || fz[b] != 0.0) {
+                atomicAdd(&f.fx[i], fx[b]); atomicAdd(&f.fy[i], fy[b]); atomicAdd(&f.fz[i], fz[b]);
+            }
+        } else if (cv[b] | cw[b]) {
+            atomicAdd(&eo.pe[i], 0.5 * uv[b] + uw[b]);
+            atomicAdd(&eo.pew[i], uw[b]);
+            atomicAdd(&eo.vir[i], 0.5 * wv[b] + ww[b]);
+            atomicAdd(&eo.cvv[i], cv[b]);
+            atomicAdd(&eo.cvw[i], cw[b]);
+        }
+    }
+}
+
+} // namespace md

@@ -3,12 +3,14 @@
 #include "../../include/md.h"
 #include "md_kernels.cuh"
 #include "md_verlet.cuh"
+#include "md_allpairs.cuh"
 
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 namespace {
@@ -122,6 +124,8 @@ struct Layout {
     double *stage0, *stage1, *wstage;
     int *nbr, *ncnt, *vflags;   // VERLET: neighbour list, counts, flags
     unsigned long long* vtimes;
+    md::Vec4<double> *jv, *jw;  // ALLPAIRS fp64: j lists (entries + ghosts) of the dot-product kernel
+    int* ghost_count;
     int red_blocks;
     size_t bytes;
 };
@@ -162,6 +166,10 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.nbr = c.take<int>(verlet ? n * md::VL_MAXN : 1);
     l.ncnt = c.take<int>(verlet ? n : 1);
     l.vflags = c.take<int>(md::VF_COUNT);
+    const bool dot = algo == MD_FORCE_ALLPAIRS && sizeof(T) == 8;
+    l.jv = c.take<md::Vec4<double>>(dot ? 8 * n : 1);     // <= 7 periodic images per particle
+    l.jw = c.take<md::Vec4<double>>(dot ? 8 * m : 1);
+    l.ghost_count = c.take<int>(4);
     l.vtimes = c.take<unsigned long long>(8 + 8192);
     l.stage0 = c.take<double>(n * dim);
     l.stage1 = c.take<double>(n * dim);
@@ -211,6 +219,11 @@ struct Sim : md_sim {
     int curv = 0, coop_grid = 0;
     long long rebuilds_seen = 0;
     unsigned long long phase_seen[4] = {0, 0, 0, 0}, phase_ns[4] = {0, 0, 0, 0};
+
+    md::AllPairsDot ad;
+    bool dot = false;           // fp64 all-pairs through the dot-product kernel (md_allpairs.cuh)
+    int ad_slices = 1;
+    int gpar = 0;               // which of the two ghost counters describes the current j list
 
     bool verlet() const { return algo == MD_FORCE_VERLET; }
 
@@ -291,6 +304,22 @@ struct Sim : md_sim {
             else
                 md::k_force_cells<T, 3, ENERGY, KICK, COUNT><<<cdiv(cdiv(p.nv, 10), 4), 128, 0, stream>>>(
                     p, l.st[cur], l.start, walls, l.f, l.eo, l.tests);
+        } else if (dot) {
+            if constexpr (std::is_same<T, double>::value) {
+                ad.ghost_count = l.ghost_count + gpar;
+                if (ENERGY) {
+                    const size_t n = (size_t)p.nv;
+                    cudaMemsetAsync(l.eo.pe, 0, n * sizeof(double), stream);
+                    cudaMemsetAsync(l.eo.pew, 0, n * sizeof(double), stream);
+                    cudaMemsetAsync(l.eo.vir, 0, n * sizeof(double), stream);
+                    cudaMemsetAsync(l.eo.cvv, 0, n * sizeof(int), stream);
+                    cudaMemsetAsync(l.eo.cvw, 0, n * sizeof(int), stream);
+                }
+                const dim3 grid(cdiv(p.nv, md::AD_THREADS * md::AD_IB), ad_slices);
+                md::k_force_allpairs_dot<ENERGY><<<grid, md::AD_THREADS, 0, stream>>>(p, ad, l.f, l.eo);
+                // the second half-kick also clears the OTHER ghost counter, which the next step's list will fill
+                if (KICK) md::k_ap_kick<<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, l.ghost_count + (gpar ^ 1));
+            }
         } else
             md::k_force_allpairs<T, ENERGY, KICK><<<blocks(md::AP_THREADS), md::AP_THREADS, 0, stream>>>(
                 p, l.st[cur], l.wtr, l.f, l.eo);
@@ -311,8 +340,14 @@ struct Sim : md_sim {
             cur ^= 1;
             if (t) cudaEventRecord(t[3], stream);
         } else {
-            md::k_kick_drift_bin<T, true, false><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, nullptr, nullptr,
-                                                                                 nullptr, l.err);
+            if (dot) {
+                gpar ^= 1;
+                ad.ghost_count = l.ghost_count + gpar;
+                if constexpr (std::is_same<T, double>::value)
+                    md::k_ap_kick_drift_list<true><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, ad, l.err);
+            } else
+                md::k_kick_drift_bin<T, true, false><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, nullptr, nullptr,
+                                                                                     nullptr, l.err);
             if (t) { cudaEventRecord(t[1], stream); cudaEventRecord(t[2], stream); cudaEventRecord(t[3], stream); }
         }
         launch_force<false, true, false>();
@@ -348,15 +383,16 @@ struct Sim : md_sim {
             return MD_OK;
         }
         while (n > 0) {
-            const int par = algo == MD_FORCE_CELLS ? cur : 0;
+            const int par = algo == MD_FORCE_CELLS ? cur : (dot ? gpar : 0);
             if (n >= CHUNK) {
-                if (!gN[par]) { int c0 = cur; int rc = capture(CHUNK, &gN[par]); cur = c0; if (rc) return rc; }
+                if (!gN[par]) { int c0 = cur, g0 = gpar; int rc = capture(CHUNK, &gN[par]); cur = c0; gpar = g0; if (rc) return rc; }
                 CK(cudaGraphLaunch(gN[par], stream));
                 n -= CHUNK; step_no += CHUNK;       // CHUNK is even: buffer parity unchanged
             } else {
-                if (!g1[par]) { int c0 = cur; int rc = capture(1, &g1[par]); cur = c0; if (rc) return rc; }
+                if (!g1[par]) { int c0 = cur, g0 = gpar; int rc = capture(1, &g1[par]); cur = c0; gpar = g0; if (rc) return rc; }
                 CK(cudaGraphLaunch(g1[par], stream));
                 if (algo == MD_FORCE_CELLS) cur ^= 1;
+                if (dot) { gpar ^= 1; ad.ghost_count = l.ghost_count + gpar; }
                 n -= 1; step_no += 1;
             }
         }
@@ -503,6 +539,12 @@ struct Sim : md_sim {
         if (!tests) { err = "tests is NULL"; return MD_ERR_INVALID_ARG; }
         if (algo == MD_FORCE_ALLPAIRS) {
             *tests = (long long)p.nv * ((long long)p.nv - 1 + p.nw);
+            if (dot) {   // the kernel also tests this step's periodic ghost entries
+                int g = 0;
+                CK(cudaMemcpyAsync(&g, l.ghost_count + gpar, sizeof(int), cudaMemcpyDeviceToHost, stream));
+                CK(cudaStreamSynchronize(stream));
+                *tests = (long long)p.nv * ((long long)p.nv - 1 + g + ad.nwg);
+            }
             return MD_OK;
         }
         if (verlet()) {   // one test per neighbour-list entry
@@ -529,7 +571,7 @@ struct Sim : md_sim {
     {
         if (a) *a = algo;
         if (nc) for (int k = 0; k < 3; ++k) nc[k] = p.nc[k];
-        if (kps) *kps = algo == MD_FORCE_CELLS ? 5 : (verlet() ? 1 : 2);
+        if (kps) *kps = algo == MD_FORCE_CELLS ? 5 : (verlet() ? 1 : (dot ? 3 : 2));
     }
 
     int init(const md_box& box, const md_lj& lj, const md_opts& o, long long nv, const double* pos, const double* vel,
@@ -600,6 +642,19 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
         md::k_scatter<T><<<blocks(256), 256, 0, stream>>>(p.nv, l.st[0], l.st[1], l.f, l.f, l.cell, l.slot, l.start, 0);
         cur = 1;
     }
+    if (dot) {
+        if constexpr (std::is_same<T, double>::value) {
+            CK(cudaMemsetAsync(l.ghost_count, 0, 4 * sizeof(int), stream));
+            if (nw > 0) md::k_ap_wall_list<<<cdiv(nw, 256), 256, 0, stream>>>(p, l.wtr, ad, l.ghost_count + 2);
+            int wg = 0;
+            CK(cudaMemcpyAsync(&wg, l.ghost_count + 2, sizeof(int), cudaMemcpyDeviceToHost, stream));
+            CK(cudaStreamSynchronize(stream));
+            ad.nwg = (int)nw + wg;
+            const int tiles = cdiv(nv, md::AD_THREADS) + cdiv(ad.nwg, md::AD_THREADS) + 1;
+            ad_slices = std::max(1, std::min(tiles, cdiv(148 * 8, cdiv(nv, md::AD_THREADS * md::AD_IB))));
+            md::k_ap_kick_drift_list<false><<<blocks(256), 256, 0, stream>>>(p, l.st[0], l.f, ad, l.err);
+        }
+    }
     launch_force<false, false, false>();   // f(0)
     CK(cudaStreamSynchronize(stream));
     CK(cudaGetLastError());
@@ -643,6 +698,28 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
     p.sig2_vw = (T)(lj.sigma_w * lj.sigma_w); p.e24_vw = (T)(24.0 * lj.eps_w); p.e4_vw = (T)(4.0 * lj.eps_w);
     p.uc_vw = (T)ucut(lj.eps_w, lj.sigma_w);
     p.dt = (T)o.dt; p.hk = (T)(o.dt / (2.0 * o.mass)); p.mass = o.mass;
+    if (algo == MD_FORCE_ALLPAIRS && sizeof(T) == 8) {
+        // dot-product kernel: needs at most one periodic image per dimension inside r_c + margin of a face
+        bool ok = true;
+        double smax = 0.0;
+        for (int a = 0; a < box.dim; ++a) {
+            if (box.bc[a] == MD_BC_PERIODIC && box.len[a] < 2.2 * lj.r_cut) ok = false;
+            const double h = 0.5 * box.len[a] + 1.1 * lj.r_cut;
+            smax += 2.0 * h * h;
+        }
+        if (ok) {
+            md::AllPairsDot& a = s->ad;
+            s->dot = true;
+            a.jv = s->l.jv; a.jw = s->l.jw; a.ghost_count = s->l.ghost_count; a.nwg = 0;
+            for (int k = 0; k < 3; ++k) a.half[k] = k < box.dim ? 0.5 * box.len[k] : 0.0;
+            a.edge = lj.r_cut * (1.0 + 1e-9) + 1e-9;
+            // filter threshold: r_c^2 plus a bound on the rounding of the 4-term dot-product form
+            const double thr = lj.r_cut * lj.r_cut + 64.0 * 2.3e-16 * smax + 1e-12;
+            long long bits;
+            memcpy(&bits, &thr, sizeof(bits));
+            a.thr_hi = (int)(bits >> 32) + 1;
+        }
+    }
     if (algo == MD_FORCE_VERLET) {
         const double skin = list_skin(lj, o), rl = lj.r_cut + skin;
         md::Verlet<T>& v = s->vl;
