@@ -651,7 +651,18 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
             CK(cudaStreamSynchronize(stream));
             ad.nwg = (int)nw + wg;
             const int tiles = cdiv(nv, md::AD_THREADS) + cdiv(ad.nwg, md::AD_THREADS) + 1;
-            ad_slices = std::max(1, std::min(tiles, cdiv(148 * 8, cdiv(nv, md::AD_THREADS * md::AD_IB))));
+            // j slices: enough blocks to fill the GPU, and a block count that wastes little of the last wave
+            int dev = 0, sms = 148, nb = 4;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, md::k_force_allpairs_dot<false>, md::AD_THREADS, 0);
+            const int slots = std::max(1, nb * sms), ib = cdiv(nv, md::AD_THREADS * md::AD_IB);
+            double best = -1.0;
+            for (int sl = 1; sl <= std::min(tiles, 96); ++sl) {
+                const double waves = (double)ib * sl / slots;
+                const double eff = waves / std::ceil(waves) - (sl * 1e-4) + (waves >= 1.0 ? 0.0 : waves - 1.0);
+                if (eff > best) { best = eff; ad_slices = sl; }
+            }
             md::k_ap_kick_drift_list<false><<<blocks(256), 256, 0, stream>>>(p, l.st[0], l.f, ad, l.err);
         }
     }
