@@ -73,7 +73,9 @@ class ClockSampler:
 
 
 def dist_env():
-    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    from paper_1812_07993_b200 import replicas
+
+    return replicas.dist_env()
 
 
 def oracle_sample(cfg, n_steps):
@@ -134,7 +136,9 @@ def run_ours(args):
 
         dist.init_process_group("nccl", device_id=dev)
     md.load_library()
-    cfg = I.config2(seed=I.BASE_SEED + 2 + 7919 * rank)         # one independent replica per rank
+    from paper_1812_07993_b200 import replicas
+
+    cfg = replicas.replica_config(rank)                         # one independent replica per rank
     nv, nw, dim = cfg["n_vapor"], cfg["n_wall"], cfg["dim"]
     inner = args.inner
 
@@ -145,18 +149,10 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(x, dev)
 
     def sum_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+        return replicas.sum_over_ranks(x, dev)
 
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
@@ -230,6 +226,9 @@ def run_ours(args):
         per_step = nv * (136 + 4) + 4 * tests
         top_name, t_top, alg = "k_md_run (persistent: %d time steps per launch)" % prof_steps, kt["ms"][3] * 1e-3, per_step * prof_steps
         shares = {"k_md_run": 1.0}
+        # DRAM traffic of k_md_run from the committed ncu --set full capture (profiles/r01_v3_cfg2.md):
+        # dram__bytes_read.sum + dram__bytes_write.sum = 10.69 MB for a 200-step launch = 53.5 KB per time step
+        traffic = 53.5e3 * prof_steps
         extra = {"time_steps_per_launch": prof_steps, "rebuilds_in_launch": kt["rebuilds"],
                  "us_per_time_step": kt["ms"][3] * 1e3 / prof_steps}
     else:
@@ -241,10 +240,10 @@ def run_ours(args):
         top = max(range(4), key=lambda k: kt["ms"][k])
         alg_bytes = {0: 144 * nv, 1: 12 * ncell, 2: 128 * nv + 4 * ncell, 3: 104 * nv + 4 * (ncell + 1)}
         top_name, t_top, alg = names[top], kt["ms"][top] * 1e-3 / kt["launches"][top], alg_bytes[top]
-        extra = {}
+        extra, traffic = {}, None
     achieved = alg / t_top * 1e-9
     roofline = {"kernel": top_name, "bound": "hbm", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / pk["hbm_gbs"], "traffic": None, "peak_source": pk_src + " (MEASURED_PEAKS.json hbm_gbs)",
+                "frac": achieved / pk["hbm_gbs"], "traffic": traffic, "peak_source": pk_src + " (MEASURED_PEAKS.json hbm_gbs)",
                 "algorithmic_bytes_per_launch": alg, "us_per_launch": t_top * 1e6, "kernel_share_of_step": shares,
                 "note": "the 4.7 MB state is L2-resident across time steps, so the step is bound by L2 latency and the "
                         "grid barrier, not by HBM: a low fraction here is expected (DESIGN.md)"}
