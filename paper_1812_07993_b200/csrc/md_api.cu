@@ -123,7 +123,7 @@ struct Layout {
     unsigned long long* tests;
     double *stage0, *stage1, *wstage;
     int *nbr, *ncnt, *vflags;   // VERLET: neighbour list, counts, flags
-    unsigned long long* vtimes;
+    unsigned long long *vtimes, *vbar;
     md::Vec4<double> *jv, *jw;  // ALLPAIRS fp64: j lists (entries + ghosts) of the dot-product kernel
     int* ghost_count;
     int red_blocks;
@@ -171,6 +171,7 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.jw = c.take<md::Vec4<double>>(dot ? 8 * m : 1);
     l.ghost_count = c.take<int>(4);
     l.vtimes = c.take<unsigned long long>(8 + 8192);
+    l.vbar = c.take<unsigned long long>(2);
     l.stage0 = c.take<double>(n * dim);
     l.stage1 = c.take<double>(n * dim);
     l.wstage = c.take<double>(m * dim);
@@ -251,6 +252,7 @@ struct Sim : md_sim {
             coop_grid = std::max(1, std::min(nb * sms, p.nv <= md::VL_THREADS * sms ? cdiv(p.nv, md::VL_THREADS) : want));
         }
         CK(cudaMemsetAsync(l.vflags + md::VF_REQ0, 0, 3 * sizeof(int), stream));   // rebuild-request slots
+        CK(cudaMemsetAsync(l.vbar, 0, 2 * sizeof(unsigned long long), stream));        // grid barrier counter
         void* args[] = {(void*)&p, (void*)&vl, (void*)&n, (void*)&force_rebuild};
         CK(cudaLaunchCooperativeKernel(kernel, dim3(coop_grid), dim3(md::VL_THREADS), args, 0, stream));
         return MD_OK;
@@ -737,7 +739,7 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
         v.st[0] = s->l.st[0]; v.st[1] = s->l.st[1]; v.f = s->l.f;
         v.nbr = s->l.nbr; v.ncnt = s->l.ncnt; v.stride = align_up((size_t)nv, 64);
         v.cell = s->l.cell; v.slot = s->l.slot; v.count = s->l.count; v.start = s->l.start; v.tile_sum = s->l.tile_sum;
-        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.times = s->l.vtimes; v.dbg = getenv("MD_DEBUG_TIMES") ? s->l.vtimes + 8 : nullptr;
+        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.bar = s->l.vbar; v.times = s->l.vtimes; v.dbg = getenv("MD_DEBUG_TIMES") ? s->l.vtimes + 8 : nullptr;
         v.rl2 = (T)(rl * rl); v.half_skin = (T)(0.5 * skin);
     }
     int rc = s->init(box, lj, o, nv, pos, vel, nw, wall);

@@ -39,6 +39,7 @@ struct Verlet {
     const int* wstart;         // walls: [ncell + 1] ranges into the wall tail
     const uint8_t* wnear;
     int* flags;                // VF_*
+    unsigned long long* bar;   // grid barrier arrival counter
     unsigned long long* dbg;   // optional per-warp step-phase ns (diagnostics), or nullptr
     unsigned long long* times; // [8] ns seen by thread 0: step phases, step barriers, rebuilds, final phase,
                                // rebuild split: bin, scan, scatter, list build (each with its barrier)
@@ -60,6 +61,26 @@ __device__ __forceinline__ float fold(float a, float b, float L, float halfL)
     if (d > halfL) d = (a - L) - b;
     else if (d < -halfL) d = a - (b - L);
     return d;
+}
+
+// Grid barrier of the cooperative launch (all blocks are co-resident).  One arrival atomic per block; the wait
+// polls with relaxed loads and fences ONCE when released -- cooperative_groups' grid.sync() re-acquires (and so
+// invalidates the SM's L1, CCTL.IVALL) on every poll, which also evicts the lines of the other block still
+// computing on that SM (profiles/r01_v3_cfg2.md).  `bar` is zeroed by the host before every launch.
+__device__ __forceinline__ void grid_barrier(unsigned long long* bar, unsigned long long& target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += gridDim.x;
+        __threadfence();                                   // release this block's writes
+        atomicAdd(bar, 1ull);
+        unsigned long long seen;
+        do {
+            asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(bar) : "memory");
+        } while (seen < target);
+        __threadfence();                                   // acquire: later loads see every block's writes
+    }
+    __syncthreads();
 }
 
 __device__ __forceinline__ unsigned long long now_ns()
@@ -111,15 +132,18 @@ __device__ __forceinline__ void pair_term_nb(const Params<T>& p, bool valid, boo
     }
 }
 
+// Batches of four list entries; while batch b is evaluated the indices of batch b + 1 are in flight.  The first
+// index loads do not wait for the list length (rows beyond it are allocated; their values are masked), so the
+// first positions are requested one round trip after the thread starts.
 template <typename T, bool ENERGY, bool FOLD>
 __device__ __forceinline__ void list_loop(const Params<T>& p, const int* __restrict__ lst, size_t stride, int n,
-                                          const Vec4<T>* __restrict__ r, const Vec4<T>& ri, Acc<T, ENERGY>& av,
-                                          Acc<T, ENERGY>& aw)
+                                          const Vec4<T>* __restrict__ r, const Vec4<T>& ri, const int (&j0)[4],
+                                          Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
     const bool px = FOLD && p.bc[0] == BC_PERIODIC, py = FOLD && p.bc[1] == BC_PERIODIC, pz = FOLD && p.bc[2] == BC_PERIODIC;
     int jn[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) jn[u] = u < n ? lst[(size_t)u * stride] : -1;
+    for (int u = 0; u < 4; ++u) jn[u] = u < n ? j0[u] : -1;
     for (int k = 0; k < n; k += 4) {
         int j[4];
         Vec4<T> rj[4];
@@ -141,10 +165,13 @@ template <typename T, bool ENERGY>
 __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& v, const Vec4<T>* __restrict__ r, int i,
                                            const Vec4<T>& ri, Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
-    const int raw = v.ncnt[i];
     const int* __restrict__ lst = v.nbr + i;
-    if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & (VL_FOLD - 1), r, ri, av, aw);
-    else list_loop<T, ENERGY, false>(p, lst, v.stride, raw, r, ri, av, aw);
+    int j0[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) j0[u] = lst[(size_t)u * v.stride];       // in flight together with ncnt (and r_i, v_i)
+    const int raw = v.ncnt[i];
+    if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & (VL_FOLD - 1), r, ri, j0, av, aw);
+    else list_loop<T, ENERGY, false>(p, lst, v.stride, raw, r, ri, j0, av, aw);
 }
 
 // ---- phase: [forces] -> [kick completing the step] -> [kick + drift of the next step] -----------
@@ -403,7 +430,7 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
 template <typename T, int ROWS>
 __global__ void __launch_bounds__(VL_THREADS, 2) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
 {
-    cg::grid_group grid = cg::this_grid();
+    unsigned long long bar_target = 0;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
     const int gthreads = gridDim.x * blockDim.x;
     int c = v.flags[VF_CUR], cv = v.flags[VF_CURV];
@@ -413,24 +440,24 @@ __global__ void __launch_bounds__(VL_THREADS, 2) k_md_run(Params<T> p, Verlet<T>
         if (rebuild) {
             unsigned long long u0 = gtid == 0 ? now_ns() : 0ull, u1;
             phase_bin<T>(p, v, c, gtid, gthreads);
-            grid.sync();
+            grid_barrier(v.bar, bar_target);
             if (gtid == 0) { u1 = now_ns(); v.times[4] += u1 - u0; u0 = u1; }
             const bool two_level = p.ncell > 64 * SCAN_TILE;
             if (two_level) {
                 phase_scan_reduce(v.count, p.ncell, v.tile_sum);
-                grid.sync();
+                grid_barrier(v.bar, bar_target);
             }
             phase_scan_apply(v.count, p.ncell, two_level ? v.tile_sum : nullptr, v.start);
-            grid.sync();
+            grid_barrier(v.bar, bar_target);
             if (gtid == 0) { u1 = now_ns(); v.times[5] += u1 - u0; u0 = u1; }
             phase_scatter<T>(p, v, c, cv, gtid, gthreads);
-            grid.sync();
+            grid_barrier(v.bar, bar_target);
             if (gtid == 0) { u1 = now_ns(); v.times[6] += u1 - u0; u0 = u1; }
             c ^= 1; cv ^= 1;
             phase_build<T, ROWS>(p, v, c, gtid, gthreads);
             for (int q = gtid; q < p.ncell; q += gthreads) v.count[q] = 0;                  // for the next rebuild
             if (gtid == 0) v.flags[VF_NREBUILD] += 1;
-            grid.sync();
+            grid_barrier(v.bar, bar_target);
             if (gtid == 0) { t1 = now_ns(); v.times[2] += t1 - t0; t0 = t1; v.times[7] += t1 - u0; }
         }
         if (s == n_steps) break;
@@ -441,7 +468,7 @@ __global__ void __launch_bounds__(VL_THREADS, 2) k_md_run(Params<T> p, Verlet<T>
         phase_step<T>(p, v, c, cv, s > 0, s > 0, true, req, gtid, gthreads);
         if (v.dbg && (threadIdx.x & 31) == 0) atomicAdd(v.dbg + (gtid >> 5), now_ns() - dbg0);
         if (gtid == 0) { t1 = now_ns(); v.times[0] += t1 - t0; t0 = t1; }
-        grid.sync();
+        grid_barrier(v.bar, bar_target);
         if (gtid == 0) { t1 = now_ns(); v.times[1] += t1 - t0; t0 = t1; }
         c ^= 1;
         rebuild = *(volatile int*)(v.flags + VF_REQ0 + req) != 0;
