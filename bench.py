@@ -305,6 +305,23 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_cpu_sweep():
+    """CPU baseline of BASELINE.json configs[4]: the brute-force oracle on the host cores for N_v <= 2^14."""
+    from oracle import md_oracle as O
+    from paper_1812_07993_b200 import inputs as I
+
+    print("| N_v | N_w | cores | s per step | ordered pair tests/s |\n|---|---|---|---|---|")
+    for log2n in (10, 12, 14):
+        cfg = I.config4(log2n)
+        O.forces(cfg)
+        n = 3
+        t0 = time.perf_counter()
+        O.run(cfg, n)
+        sec = (time.perf_counter() - t0) / (n + 1)              # n steps + the initial force evaluation
+        nv, nw = cfg["n_vapor"], cfg["n_wall"]
+        print("| %d | %d | %d | %.4g | %.4g |" % (nv, nw, O.n_threads(), sec, nv * (nv - 1 + nw) / sec))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -315,8 +332,11 @@ def main():
     ap.add_argument("--ref-inner", type=int, default=20, help="oracle timesteps per bench step (--impl reference)")
     ap.add_argument("--cpu-steps", type=int, default=300, help="oracle timesteps of the cpu_baseline sample")
     ap.add_argument("--allpairs-steps", type=int, default=10)
+    ap.add_argument("--cpu-sweep", action="store_true", help="time the brute-force oracle for N_v = 2^10, 2^12, 2^14")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.cpu_sweep:
+        run_cpu_sweep()
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -67,7 +67,8 @@ typedef struct { double eps, sigma, eps_w, sigma_w, r_cut; int shift_energy; } m
  *   VERLET    the same cell list, rebuilt only when a particle's path since the last rebuild exceeds
  *             skin/2, cached as a neighbour list of all pairs within r_cut + skin (exact: no pair
  *             within r_cut is ever missed); the whole md_step batch is one persistent launch;
- *   AUTO      VERLET when the grid allows it and n_vapor >= 2048, else CELLS, else ALLPAIRS.
+ *   AUTO      VERLET when the box holds >= 3 cells of side r_cut + skin per periodic dimension, else CELLS
+ *             under the same rule with r_cut, else ALLPAIRS.
  * skin >= 0 is the VERLET list margin in length units; 0 selects the default 0.24 r_cut. */
 typedef struct { double dt, mass; int precision, force_algo; double skin; } md_opts;
 

@@ -174,11 +174,13 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double
                     cand |= (__double2hiint(r2) < thr);
                 }
             }
-            if (cand) {      // rare: redo this group's pairs exactly
+            if (cand) {      // some lane of the warp has a candidate: each lane redoes ITS flagged pairs exactly
                 for (int u = 0; u < AD_UNROLL; ++u) {
                     const Vec4<double> q = sj[k0 + u];
 #pragma unroll
                     for (int b = 0; b < AD_IB; ++b) {
+                        const double r2 = fma(ax[b], q.x, fma(ay[b], q.y, fma(az[b], q.z, si[b] + q.w)));
+                        if (__double2hiint(r2) >= thr) continue;               // same filter value as above
                         if (!wall && j0 + k0 + u == idx[b]) continue;          // j == i skipped by index
                         if (wall) ap_exact<ENERGY>(p, true, -0.5 * ax[b], -0.5 * ay[b], -0.5 * az[b], q, fx[b], fy[b], fz[b], uw[b], ww[b], cw[b]);
                         else ap_exact<ENERGY>(p, false, -0.5 * ax[b], -0.5 * ay[b], -0.5 * az[b], q, fx[b], fy[b], fz[b], uv[b], wv[b], cv[b]);

@@ -105,8 +105,9 @@ int pick_algo(const md_box& box, const md_lj& lj, const md_opts& o, long long nv
     if (o.force_algo == MD_FORCE_ALLPAIRS) return MD_FORCE_ALLPAIRS;
     if (o.force_algo == MD_FORCE_CELLS) return cells_ok ? MD_FORCE_CELLS : -1;
     if (o.force_algo == MD_FORCE_VERLET) return verlet_ok(box, lj, o, nv, nw) ? MD_FORCE_VERLET : -1;
-    if (nv >= 2048 && verlet_ok(box, lj, o, nv, nw)) return MD_FORCE_VERLET;
-    return (cells_ok && nv >= 2048) ? MD_FORCE_CELLS : MD_FORCE_ALLPAIRS;
+    // AUTO: the fastest valid path (measured on every configuration, profiles/r01_report_all_configs.md)
+    if (verlet_ok(box, lj, o, nv, nw)) return MD_FORCE_VERLET;
+    return cells_ok ? MD_FORCE_CELLS : MD_FORCE_ALLPAIRS;
 }
 
 template <typename T>

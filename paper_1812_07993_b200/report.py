@@ -1,0 +1,114 @@
+"""Per-configuration throughput report (BASELINE.json configs[0..4]) -- `python -m paper_1812_07993_b200.report`.
+
+For every configuration and force path: MD steps/s, pair-interactions/s (ordered within-cut-off evaluations,
+algorithm-independent), executed pair tests/s, and for the all-pairs kernel the executed FP64/FP32 rate against the
+FMA-chain peak measured in the same run.  Prints one markdown table; all inputs are the seeded synthetic
+configurations of inputs.py.  (The CPU baseline for N <= 2^14 that configs[4] asks for is `bench.py --cpu-sweep`.)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import sys
+
+
+def time_steps(sim, n_steps, torch):
+    sim.step(min(n_steps, 64))                       # warm-up (graph capture, first rebuilds)
+    sim.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(sim.stream)
+    sim.step(n_steps)
+    b.record(sim.stream)
+    sim.synchronize()
+    return a.elapsed_time(b) * 1e-3 / n_steps
+
+
+def measure(cfg, algo, precision, n_steps, torch, md, peaks):
+    try:
+        sim = md.Simulation(cfg, algo=algo, precision=precision)
+    except md.MDError as e:
+        if e.code == md.MD_ERR_UNSUPPORTED:
+            return None
+        raise
+    sec = time_steps(sim, n_steps, torch)
+    e = sim.energy()
+    tests = sim.pair_tests()
+    inter = 2 * e["pairs_vv"] + e["pairs_vw"]
+    row = dict(config=cfg["name"], n_vapor=cfg["n_vapor"], n_wall=cfg["n_wall"], algo=sim.info()["algo"], precision=precision,
+               steps_timed=n_steps, md_steps_per_s=1.0 / sec, pair_interactions_per_s=inter / sec,
+               pair_tests_per_s=tests / sec, us_per_step=sec * 1e6)
+    if algo == "allpairs":
+        flops = 7.0 if precision == 64 else 14.0     # executed per test: DESIGN.md section 5
+        peak = peaks["fp64_tflops"] if precision == 64 else peaks["fp32_tflops"]
+        row["alu_tflops"] = tests * flops / sec * 1e-12
+        row["alu_frac_of_measured_peak"] = row["alu_tflops"] / peak
+    sim.close()
+    return row
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", default="0,1,2,3,4")
+    ap.add_argument("--max-log2n", type=int, default=20)
+    ap.add_argument("--json", default="")
+    args = ap.parse_args()
+    import torch
+
+    from . import inputs as I
+    from . import md
+
+    if not torch.cuda.is_available():
+        raise SystemExit("report: no CUDA device; the CUDA path has no fallback")
+    peaks = md.measure_peaks()
+    want = {int(x) for x in args.configs.split(",")}
+    rows = []
+
+    def add(cfg, algo, precision, n_steps):
+        r = measure(cfg, algo, precision, n_steps, torch, md, peaks)
+        if r:
+            rows.append(r)
+            print("  %-22s %-8s fp%d  %10.0f steps/s" % (r["config"], r["algo"], precision, r["md_steps_per_s"]), file=sys.stderr)
+
+    if 0 in want:
+        cfg = I.config0()
+        for algo in ("allpairs", "cells", "verlet"):
+            add(cfg, algo, 64, 2000)
+    if 1 in want:
+        cfg = I.config1()
+        for algo in ("cells", "verlet"):
+            add(cfg, algo, 64, 4000)
+    if 2 in want:
+        cfg = I.config2()
+        for algo in ("cells", "verlet"):
+            add(cfg, algo, 64, 4000)
+        add(cfg, "allpairs", 64, 20)
+    if 3 in want:
+        for shape in ("cone", "inkbottle", "slit"):
+            cfg = I.config3(shape)
+            for algo in ("cells", "verlet"):
+                add(cfg, algo, 64, 2000)
+    if 4 in want:
+        for log2n in range(10, args.max_log2n + 1, 2):
+            cfg = I.config4(log2n)
+            for precision in (64, 32):
+                for algo in ("cells", "verlet"):
+                    add(cfg, algo, precision, 1000)
+                # all-pairs cost grows as N^2: 1000 steps up to 2^14, fewer beyond (stated in the table)
+                ap_steps = {10: 1000, 12: 1000, 14: 1000, 16: 100, 18: 10, 20: 2}[log2n]
+                add(cfg, "allpairs", precision, ap_steps)
+    print("peaks measured in this run: FP64 %.1f TFLOP/s, FP32 %.1f TFLOP/s, copy %.0f GB/s\n" %
+          (peaks["fp64_tflops"], peaks["fp32_tflops"], peaks["copy_gbs"]))
+    print("| config | N_v | N_w | path | fp | steps timed | MD steps/s | pair-interactions/s | pair tests/s | ALU TFLOP/s (frac of measured peak) |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    for r in rows:
+        alu = "%.2f (%.3f)" % (r["alu_tflops"], r["alu_frac_of_measured_peak"]) if "alu_tflops" in r else ""
+        print("| %s | %d | %d | %s | %d | %d | %.4g | %.4g | %.4g | %s |" %
+              (r["config"], r["n_vapor"], r["n_wall"], r["algo"], r["precision"], r["steps_timed"], r["md_steps_per_s"],
+               r["pair_interactions_per_s"], r["pair_tests_per_s"], alu))
+    if args.json:
+        with open(args.json, "w") as fh:
+            json.dump(dict(peaks=peaks, rows=rows), fh)
+
+
+if __name__ == "__main__":
+    main()
