@@ -219,6 +219,7 @@ struct Sim : md_sim {
     // VERLET (persistent kernel): device-side buffer parities are mirrored here by refresh()
     md::Verlet<T> vl;
     int curv = 0, coop_grid = 0;
+    int minb3_threshold = getenv("MD_MINB3_THRESHOLD") ? atoi(getenv("MD_MINB3_THRESHOLD")) : 500000;
     long long rebuilds_seen = 0;
     unsigned long long phase_seen[4] = {0, 0, 0, 0}, phase_ns[4] = {0, 0, 0, 0};
 
@@ -239,7 +240,9 @@ struct Sim : md_sim {
 
     int launch_run(long long n, int force_rebuild)
     {
-        void* kernel = dim == 3 ? (void*)md::k_md_run<T, 9> : (void*)md::k_md_run<T, 3>;
+        const bool big = p.nv > minb3_threshold;
+        void* kernel = dim == 3 ? (big ? (void*)md::k_md_run<T, 9, 3> : (void*)md::k_md_run<T, 9, 2>)
+                                : (big ? (void*)md::k_md_run<T, 3, 3> : (void*)md::k_md_run<T, 3, 2>);
         if (!coop_grid) {
             int dev = 0, sms = 0, coop = 0, nb = 0;
             CK(cudaGetDevice(&dev));

@@ -427,8 +427,10 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
 // md_step(n): phase(stored f; kick + drift), then n - 1 fused phases (force; kick; kick + drift), then
 // phase(force; kick): n + 1 phases and n grid barriers for n steps, plus 5 barriers per rebuild.
 // force_rebuild (md_create): bin + build the list first, then evaluate f(0).
-template <typename T, int ROWS>
-__global__ void __launch_bounds__(VL_THREADS, 2) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
+// MINB = resident blocks per SM the register budget is sized for: 2 (up to 128 registers, the latency-bound
+// sizes that fit one wave) or 3 (more warps to hide HBM latency once the state no longer fits in L2).
+template <typename T, int ROWS, int MINB>
+__global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
 {
     unsigned long long bar_target = 0;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;

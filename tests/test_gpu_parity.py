@@ -227,3 +227,50 @@ def test_energy_drift_and_long_run_statistics_dilute_gas(algo):
     t_ref = ref[1000:1500, 0].mean()
     assert abs(wa[:50, 0].mean() - t_ref) / t_ref < 0.02
     sim.close()
+
+
+def _profiles(pos, cfg, r_max=10.0, n_r=10, n_z=11):
+    """Radial (about the pore axis, inside the pore's z range) and axial vapor density profiles (host side)."""
+    L = np.array(cfg["box_len"])
+    c = 0.5 * L
+    half = 0.5 * cfg["pore_length"]
+    d = pos - c
+    rho = np.hypot(d[:, 0], d[:, 1])
+    inside = np.abs(d[:, 2]) <= half
+    hr, edges = np.histogram(rho[inside], bins=n_r, range=(0.0, r_max))
+    shell = np.pi * (edges[1:] ** 2 - edges[:-1] ** 2) * 2 * half
+    hz, _ = np.histogram(pos[:, 2], bins=n_z, range=(0.0, L[2]))
+    return hr / shell, hz / (L[0] * L[1] * L[2] / n_z)
+
+
+@pytest.mark.parametrize("algo", ["cells", "verlet"])
+def test_long_run_density_profiles_match_oracle_statistically(algo):
+    # beyond 100 steps trajectories are chaotic: north_star compares the radial / axial density profile instead.
+    # Same input, 3000 steps, profiles averaged over the last 1000 steps (every 50th); the two runs are different
+    # realisations of the same ensemble, so bins must agree within counting noise (5 sigma + 5 %).
+    cfg = I.config4(12)
+    sim = md.Simulation(cfg, algo=algo)
+    pos, vel = cfg["pos"], cfg["vel"]
+    acc_g, acc_o, n_samples = None, None, 0
+    sim.step(2000)
+    o = O.run(cfg, 2000, cells=True)
+    pos, vel = o["pos"], o["vel"]
+    for _ in range(20):
+        sim.step(50)
+        o = O.run(cfg, 50, pos=pos, vel=vel, cells=True)
+        pos, vel = o["pos"], o["vel"]
+        pg = _profiles(sim.get_state(vel=False, force=False, pe=False)["pos"], cfg)
+        po = _profiles(pos, cfg)
+        acc_g = pg if acc_g is None else tuple(a + b for a, b in zip(acc_g, pg))
+        acc_o = po if acc_o is None else tuple(a + b for a, b in zip(acc_o, po))
+        n_samples += 1
+    L = np.array(cfg["box_len"])
+    half = 0.5 * cfg["pore_length"]
+    vol_r = np.pi * (np.linspace(0, 10, 11)[1:] ** 2 - np.linspace(0, 10, 11)[:-1] ** 2) * 2 * half
+    vol_z = np.full(11, L.prod() / 11)
+    for g, o_, vol in ((acc_g[0], acc_o[0], vol_r), (acc_g[1], acc_o[1], vol_z)):
+        g, o_ = g / n_samples, o_ / n_samples
+        counts = np.maximum(o_ * vol, 1.0)                         # mean particles per bin per sample
+        sigma = np.sqrt(counts) / vol                              # >= counting noise of one sample (correlated samples)
+        assert (np.abs(g - o_) <= 5 * sigma + 0.05 * np.maximum(o_, g)).all(), (g, o_)
+    sim.close()
