@@ -342,12 +342,13 @@ __device__ __forceinline__ void list_range(const Params<T>& p, const Vec4<T>* __
                                            const Vec4<T>& ri, T rl2, int* __restrict__ lst, size_t stride, int* cnt)
 {
     const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
-    for (int j0 = jb; j0 < je; j0 += 4) {
-        Vec4<T> rj[4];
+    constexpr int NB = 8;                                                // a cell row rarely holds more
+    for (int j0 = jb; j0 < je; j0 += NB) {
+        Vec4<T> rj[NB];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) rj[u] = r[min(j0 + u, je - 1)];      // four loads in flight
+        for (int u = 0; u < NB; ++u) rj[u] = r[min(j0 + u, je - 1)];     // NB loads in flight
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < NB; ++u) {
             const int j = j0 + u;
             const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
             const T dy = py ? fold(ri.y, rj[u].y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj[u].y;

@@ -274,3 +274,75 @@ def test_long_run_density_profiles_match_oracle_statistically(algo):
         sigma = np.sqrt(counts) / vol                              # >= counting noise of one sample (correlated samples)
         assert (np.abs(g - o_) <= 5 * sigma + 0.05 * np.maximum(o_, g)).all(), (g, o_)
     sim.close()
+
+
+def test_boundary_helpers_and_error_paths():
+    cfg = I.config4(10)
+    ref = O.forces(cfg)
+    # pair-test counters: all-pairs is analytic (+ ghosts), cell walk >= list entries >= ordered hits
+    hits = 2 * ref["pairs_vv"] + ref["pairs_vw"]
+    counts = {}
+    for algo in ALGOS:
+        sim = md.Simulation(cfg, algo=algo)
+        counts[algo] = sim.pair_tests()
+        sim.step(0)                                            # no-op
+        assert sim.get_state()["step"] == 0
+        k = sim.profile_step(7)
+        assert k["steps"] == 7 and k["total_ms"] > 0 and sim.energy()["step"] == 7
+        sim.close()
+    nv, nw = cfg["n_vapor"], cfg["n_wall"]
+    assert counts["allpairs"] >= nv * (nv - 1 + nw) and counts["cells"] >= counts["verlet"] >= hits
+    # profile_step and step advance the same dynamics
+    a, b = md.Simulation(cfg, algo="verlet"), md.Simulation(cfg, algo="verlet")
+    a.step(23)
+    b.profile_step(23)
+    assert np.abs(a.get_state()["pos"] - b.get_state()["pos"]).max() < 1e-12
+    a.close(), b.close()
+    # workspace too small
+    import ctypes as C
+    box, lj, opts = md._structs(cfg, 64, "verlet")
+    ws = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    h = C.c_void_p()
+    pos, vel, wall = (np.ascontiguousarray(cfg[k]) for k in ("pos", "vel", "wall"))
+    rc = md.load_library().md_create(C.byref(h), C.byref(box), None, C.byref(lj), C.byref(opts), nv, md._dptr(pos),
+                                     md._dptr(vel), nw, md._dptr(wall), ws.data_ptr(), ws.numel(), None)
+    assert rc == md.MD_ERR_WORKSPACE and not h.value
+    peaks = md.measure_peaks(scratch_mib=128)
+    assert 10 < peaks["fp64_tflops"] < 60 and peaks["fp32_tflops"] > peaks["fp64_tflops"] and peaks["copy_gbs"] > 1000
+
+
+def test_verlet_list_overflow_is_reported_not_dropped():
+    # 160 particles inside a sphere of radius 1.2: every particle has > 128 neighbours within r_c + skin
+    rng = I.SplitMix64(5)
+    pts = []
+    while len(pts) < 160:
+        p = (rng.uniform(3) * 2 - 1) * 1.2
+        if p @ p < 1.44:
+            pts.append(p + 10.0)
+    cfg = I.small_case(3, 160, (20.0, 20.0, 20.0), (0, 0, 0), seed=3, min_sep=0.5)
+    cfg["pos"] = np.array(pts)
+    cfg["eps"] = 0.0                                           # overlapping sites: keep the forces finite
+    with pytest.raises(md.MDError) as e:
+        md.Simulation(cfg, algo="verlet")
+    assert e.value.code == md.MD_ERR_WORKSPACE
+    sim = md.Simulation(cfg, algo="cells")                     # the per-step cell walk has no such limit
+    assert sim.energy()["pairs_vv"] == 160 * 159 // 2
+    sim.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_fp32_trajectory_stays_close(algo):
+    # fp32 mode over 100 steps against the fp64 oracle on the float-rounded input: rounding of the state
+    # (ulp(L) ~ 4e-6 per step in position) bounds the agreement, not the force law
+    cfg = I.config4(12)
+    c32 = dict(cfg)
+    for k in ("pos", "wall", "vel"):
+        c32[k] = cfg[k].astype(np.float32).astype(np.float64)
+    c32["box_len"] = [float(np.float32(x)) for x in cfg["box_len"]]
+    ref = O.run(c32, 100, cells=True)
+    sim = make_sim(c32, algo, precision=32)
+    sim.step(100)
+    st, en = sim.get_state(), sim.energy()
+    assert traj_error(st["pos"], ref["pos"], c32["box_len"], c32["bc"]) < 2e-3
+    assert abs(en["K"] - ref["K"]) < 1e-4 * ref["K"] and abs(en["U"] - ref["U"]) < 2e-3 * max(abs(ref["U"]), 1.0)
+    sim.close()
