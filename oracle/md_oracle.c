@@ -38,6 +38,7 @@ typedef struct {
     double r_cut;
     int shift_energy;   /* 1: u(r) - u(r_c) inside the cut-off (reading A2) */
     double dt, mass;
+    double tau_b, t_target; /* Berendsen thermostat F4: rise time (<= 0: off), T_0 */
 } orc_params;
 
 /* ---- c.1 definitions ------------------------------------------------- */
@@ -313,6 +314,15 @@ int orc_run(const orc_params *p, int use_cells, long nv, double *pos, double *ve
         for (long i = 0; i < nv; ++i)
             for (int a = 0; a < dim; ++a)
                 vel[i * dim + a] = vel[i * dim + a] + hk * f[i * dim + a];                       /* F3 */
+        if (p->tau_b > 0.0) {                                                                    /* F4 */
+            /* Berendsen: v <- lambda v, lambda = sqrt(1 + (dt / tau_B)(T_0 / T - 1)), T = 2K / (d N) with k_B = 1
+             * (the paper names lambda(t) and tau_B but prints no formula: reading A9 / NEXT-1 of DESIGN.md) */
+            const double T = 2.0 * orc_kinetic(p, nv, vel) / ((double)dim * (double)nv);
+            if (T > 0.0) {
+                const double lambda = sqrt(1.0 + (p->dt / p->tau_b) * (p->t_target / T - 1.0));
+                for (long i = 0; i < nv * dim; ++i) vel[i] = lambda * vel[i];
+            }
+        }
     }
     return 0;
 }

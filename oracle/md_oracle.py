@@ -16,7 +16,8 @@ from . import build as _build
 class OrcParams(C.Structure):
     _fields_ = [("dim", C.c_int), ("L", C.c_double * 3), ("bc", C.c_int * 3), ("eps", C.c_double),
                 ("sigma", C.c_double), ("eps_w", C.c_double), ("sigma_w", C.c_double), ("r_cut", C.c_double),
-                ("shift_energy", C.c_int), ("dt", C.c_double), ("mass", C.c_double)]
+                ("shift_energy", C.c_int), ("dt", C.c_double), ("mass", C.c_double), ("tau_b", C.c_double),
+                ("t_target", C.c_double)]
 
 
 _lib = None
@@ -53,6 +54,7 @@ def params(cfg) -> OrcParams:
     p.r_cut = float(cfg["r_cut"])
     p.shift_energy = int(cfg.get("shift_energy", 1))
     p.dt, p.mass = float(cfg["dt"]), float(cfg["mass"])
+    p.tau_b, p.t_target = float(cfg.get("tau_b", 0.0)), float(cfg.get("t_target", 1.0))
     return p
 
 

@@ -305,3 +305,32 @@ def test_energy_conservation_dilute_gas_10k_steps():
     drift = abs(e[-1000:].mean() - e[1000:2000].mean()) / h[0, 0]
     assert drift <= 1e-4, drift
     assert np.abs(e - e[0]).max() / h[0, 0] < 1e-3
+
+
+def test_berendsen_thermostat_closed_forms():
+    # F4.  Without forces K only changes through lambda, so T_{n+1} = T_n lambda^2 =
+    # T_n + (dt/tau)(T_0 - T_n) exactly:  T_n = T_0 + (T_init - T_0)(1 - dt/tau)^n.
+    cfg = I.small_case(3, 200, (12.0, 12.0, 12.0), (0, 0, 1), n_wall=6, seed=17, t_star=2.5)
+    cfg["eps"] = cfg["eps_w"] = 0.0
+    n, dim = cfg["n_vapor"], 3
+    t_init = 2.0 * O.kinetic(cfg, cfg["vel"]) / (dim * n)
+    cfg.update(tau_b=0.1, t_target=1.2, dt=0.005)
+    h = O.run(cfg, 60, history=True)["hist"]
+    t = 2.0 * h[:, 0] / (dim * n)
+    expect = 1.2 + (t_init - 1.2) * (1.0 - 0.005 / 0.1) ** np.arange(61)
+    assert np.abs(t - expect).max() < 1e-12 * t_init
+    # tau_B = dt reaches T_0 in one step; T = T_0 leaves the dynamics untouched (lambda = 1)
+    cfg.update(tau_b=0.005)
+    h = O.run(cfg, 2, history=True)["hist"]
+    assert abs(2.0 * h[1, 0] / (dim * n) - 1.2) < 1e-13
+    lj = I.small_case(3, 150, (8.0, 8.0, 8.0), (0, 0, 1), n_wall=10, seed=9)
+    nve = O.run(lj, 1)
+    t1 = 2.0 * nve["K"] / (3 * 150)
+    thermo = dict(lj, tau_b=0.3, t_target=t1)
+    out = O.run(thermo, 1)
+    assert np.abs(out["vel"] - nve["vel"]).max() < 1e-14
+    # with forces on, a cold target pulls the system to T_0 within a few tau_B and holds it there
+    cold = dict(lj, tau_b=0.05, t_target=0.3)
+    hh = O.run(cold, 300, history=True)["hist"]
+    tt = 2.0 * hh[:, 0] / (3 * 150)
+    assert tt[0] > 0.9 and np.abs(tt[50:] - 0.3).max() < 0.06
