@@ -69,8 +69,10 @@ typedef struct { double eps, sigma, eps_w, sigma_w, r_cut; int shift_energy; } m
  *             within r_cut is ever missed); the whole md_step batch is one persistent launch;
  *   AUTO      VERLET when the box holds >= 3 cells of side r_cut + skin per periodic dimension, else CELLS
  *             under the same rule with r_cut, else ALLPAIRS.
- * skin >= 0 is the VERLET list margin in length units; 0 selects the default 0.24 r_cut. */
-typedef struct { double dt, mass; int precision, force_algo; double skin; } md_opts;
+ * skin >= 0 is the VERLET list margin in length units; 0 selects the default 0.24 r_cut.
+ * tau_b > 0 switches on the Berendsen thermostat (the paper's kernel F4) after every step:
+ * v <- lambda v, lambda = sqrt(1 + (dt / tau_b)(t_target / T - 1)), T = 2K / (dim n_vapor) (k_B = 1); tau_b <= 0: NVE. */
+typedef struct { double dt, mass; int precision, force_algo; double skin; double tau_b, t_target; } md_opts;
 
 /* potential = potential_vv + potential_vw = sum_i pe_i; virial = sum over unordered vv pairs and
  * vw pairs of g.d (g = force on the vapor particle, d = r_i - r_j); pairs_* = pairs with r < r_cut. */

@@ -71,6 +71,8 @@ const char* validate(const md_box* box, const md_lj* lj, const md_opts* o, long 
     if (o->precision != 64 && o->precision != 32) return "precision must be 64 or 32";
     if (o->force_algo < MD_FORCE_AUTO || o->force_algo > MD_FORCE_VERLET) return "unknown force_algo";
     if (!(o->skin >= 0) || !std::isfinite(o->skin)) return "skin must be >= 0";
+    if (!std::isfinite(o->tau_b) || !std::isfinite(o->t_target)) return "tau_b, t_target must be finite";
+    if (o->tau_b > 0 && (o->tau_b < o->dt || !(o->t_target > 0))) return "thermostat needs tau_b >= dt and t_target > 0";
     if (!(lj->r_cut > 0) || !std::isfinite(lj->r_cut)) return "r_cut must be > 0";
     if (!(lj->sigma > 0) || !(lj->sigma_w > 0)) return "sigma, sigma_w must be > 0";
     if (!std::isfinite(lj->eps) || !std::isfinite(lj->eps_w)) return "eps, eps_w must be finite";
@@ -125,6 +127,7 @@ struct Layout {
     double *stage0, *stage1, *wstage;
     int *nbr, *ncnt, *vflags;   // VERLET: neighbour list, counts, flags
     unsigned long long *vtimes, *vbar;
+    double* vksum;              // VERLET thermostat: rotating kinetic-energy accumulators
     md::Vec4<double> *jv, *jw;  // ALLPAIRS fp64: j lists (entries + ghosts) of the dot-product kernel
     int* ghost_count;
     int red_blocks;
@@ -173,6 +176,7 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.ghost_count = c.take<int>(4);
     l.vtimes = c.take<unsigned long long>(8 + 8192);
     l.vbar = c.take<unsigned long long>(2);
+    l.vksum = c.take<double>(4);
     l.stage0 = c.take<double>(n * dim);
     l.stage1 = c.take<double>(n * dim);
     l.wstage = c.take<double>(m * dim);
@@ -257,6 +261,7 @@ struct Sim : md_sim {
         }
         CK(cudaMemsetAsync(l.vflags + md::VF_REQ0, 0, 3 * sizeof(int), stream));   // rebuild-request slots
         CK(cudaMemsetAsync(l.vbar, 0, 2 * sizeof(unsigned long long), stream));        // grid barrier counter
+        CK(cudaMemsetAsync(l.vksum, 0, 4 * sizeof(double), stream));
         void* args[] = {(void*)&p, (void*)&vl, (void*)&n, (void*)&force_rebuild};
         CK(cudaLaunchCooperativeKernel(kernel, dim3(coop_grid), dim3(md::VL_THREADS), args, 0, stream));
         return MD_OK;
@@ -357,6 +362,10 @@ struct Sim : md_sim {
             if (t) { cudaEventRecord(t[1], stream); cudaEventRecord(t[2], stream); cudaEventRecord(t[3], stream); }
         }
         launch_force<false, true, false>();
+        if (p.thermo_rate > 0.0) {   // F4: K partial sums, then lambda + rescale
+            md::k_kinetic_partial<T><<<l.red_blocks, md::RED_THREADS, 0, stream>>>(p.nv, p.mass, l.st[cur], l.part);
+            md::k_thermo_scale<T><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.red_blocks, l.part);
+        }
         if (t) cudaEventRecord(t[4], stream);
     }
 
@@ -577,7 +586,7 @@ struct Sim : md_sim {
     {
         if (a) *a = algo;
         if (nc) for (int k = 0; k < 3; ++k) nc[k] = p.nc[k];
-        if (kps) *kps = algo == MD_FORCE_CELLS ? 5 : (verlet() ? 1 : (dot ? 3 : 2));
+        if (kps) *kps = verlet() ? 1 : (algo == MD_FORCE_CELLS ? 5 : (dot ? 3 : 2)) + (p.thermo_rate > 0.0 ? 2 : 0);
     }
 
     int init(const md_box& box, const md_lj& lj, const md_opts& o, long long nv, const double* pos, const double* vel,
@@ -715,6 +724,7 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
     p.sig2_vw = (T)(lj.sigma_w * lj.sigma_w); p.e24_vw = (T)(24.0 * lj.eps_w); p.e4_vw = (T)(4.0 * lj.eps_w);
     p.uc_vw = (T)ucut(lj.eps_w, lj.sigma_w);
     p.dt = (T)o.dt; p.hk = (T)(o.dt / (2.0 * o.mass)); p.mass = o.mass;
+    p.thermo_rate = o.tau_b > 0 ? o.dt / o.tau_b : 0.0; p.t_target = o.t_target; p.dof = (double)box.dim * (double)nv;
     if (algo == MD_FORCE_ALLPAIRS && sizeof(T) == 8) {
         // dot-product kernel: needs at most one periodic image per dimension inside r_c + margin of a face
         bool ok = true;
@@ -743,7 +753,7 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
         v.st[0] = s->l.st[0]; v.st[1] = s->l.st[1]; v.f = s->l.f;
         v.nbr = s->l.nbr; v.ncnt = s->l.ncnt; v.stride = align_up((size_t)nv, 64);
         v.cell = s->l.cell; v.slot = s->l.slot; v.count = s->l.count; v.start = s->l.start; v.tile_sum = s->l.tile_sum;
-        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.bar = s->l.vbar; v.times = s->l.vtimes; v.dbg = getenv("MD_DEBUG_TIMES") ? s->l.vtimes + 8 : nullptr;
+        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.bar = s->l.vbar; v.ksum = s->l.vksum; v.times = s->l.vtimes; v.dbg = getenv("MD_DEBUG_TIMES") ? s->l.vtimes + 8 : nullptr;
         v.rl2 = (T)(rl * rl); v.half_skin = (T)(0.5 * skin);
     }
     int rc = s->init(box, lj, o, nv, pos, vel, nw, wall);

@@ -23,6 +23,7 @@ struct Params {
     T sig2_vw, e24_vw, e4_vw, uc_vw;
     T dt, hk; // hk = dt / (2 m)
     double mass;
+    double thermo_rate, t_target, dof;   // Berendsen F4: dt / tau_B (0 = off), T_0, dim * n_vapor
 };
 
 // Packed position: one 4-wide vector load per neighbour (w is spare; the cell path keeps the
@@ -601,6 +602,51 @@ __global__ void __launch_bounds__(RED_THREADS) k_energy_final(int nblocks, const
 #pragma unroll
         for (int q = 0; q < 6; ++q) v[q] += part[q * nblocks + b];
     block_sum6(v, out, 1);
+}
+
+// ---------------------------------------------------------------------------
+// F4, Berendsen thermostat for the multi-kernel paths: block partial sums of K, then every
+// block re-sums the partials in the same fixed order, forms lambda and rescales its velocities.
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ double berendsen_lambda(double kinetic, double rate, double t_target, double dof)
+{
+    const double T = 2.0 * kinetic / dof;
+    return T > 0.0 ? sqrt(1.0 + rate * (t_target / T - 1.0)) : 1.0;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(RED_THREADS) k_kinetic_partial(int n, double mass, State<T> s, double* __restrict__ part)
+{
+    __shared__ double sh[RED_THREADS / 32];
+    double k = 0.0;
+    for (int i = blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += gridDim.x * RED_THREADS) {
+        const double vx = (double)s.vx[i], vy = (double)s.vy[i], vz = (double)s.vz[i];
+        k += 0.5 * mass * (vx * vx + vy * vy + vz * vz);
+    }
+    k = warp_sum_d(k);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = k;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int q = 0; q < RED_THREADS / 32; ++q) t += sh[q];
+        part[blockIdx.x] = t;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_thermo_scale(Params<T> p, State<T> s, int nblocks, const double* __restrict__ part)
+{
+    __shared__ double s_lambda;
+    if (threadIdx.x == 0) {
+        double k = 0.0;
+        for (int b = 0; b < nblocks; ++b) k += part[b];
+        s_lambda = berendsen_lambda(k, p.thermo_rate, p.t_target, p.dof);
+    }
+    __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.nv) return;
+    const T lam = (T)s_lambda;
+    s.vx[i] = lam * s.vx[i]; s.vy[i] = lam * s.vy[i]; s.vz[i] = lam * s.vz[i];
 }
 
 // ---------------------------------------------------------------------------

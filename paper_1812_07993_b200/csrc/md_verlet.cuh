@@ -40,6 +40,7 @@ struct Verlet {
     const uint8_t* wnear;
     int* flags;                // VF_*
     unsigned long long* bar;   // grid barrier arrival counter
+    double* ksum;              // [3] kinetic-energy accumulators of the thermostat, rotating like the requests
     unsigned long long* dbg;   // optional per-warp step-phase ns (diagnostics), or nullptr
     unsigned long long* times; // [8] ns seen by thread 0: step phases, step barriers, rebuilds, final phase,
                                // rebuild split: bin, scan, scatter, list build (each with its barrier)
@@ -179,14 +180,17 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
 // drift: start the next step (F2).
 template <typename T>
 __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& v, int c, int cv, bool force,
-                                           bool kick, bool drift, int req, int gtid, int gthreads)
+                                           bool kick, bool drift, int req, int gtid, int gthreads,
+                                           T lam = T(1), double* ksum = nullptr)
 {
     const Vec4<T>* __restrict__ rcur = v.st[c].r;
     Vec4<T>* __restrict__ rnew = v.st[c ^ 1].r;
     const State<T>& s = v.st[cv];
+    double kacc = 0.0;
     for (int i = gtid; i < p.nv; i += gthreads) {
         const Vec4<T> ri = rcur[i];
         T vx = s.vx[i], vy = s.vy[i], vz = s.vz[i];      // issued early, consumed after the force loop
+        vx = lam * vx; vy = lam * vy; vz = lam * vz;     // F4 of the step just completed (lam = 1 without thermostat)
         T fx, fy, fz;
         if (force) {
             Acc<T, false> av, aw;
@@ -199,6 +203,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         if (kick) {                                    // F3: v(t) = v(t - dt/2) + (dt/2m) f(t)
             vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
         }
+        if (ksum) kacc += 0.5 * p.mass * ((double)vx * vx + (double)vy * vy + (double)vz * vz);
         if (drift) {                                   // F2: v(t + dt/2), r(t + dt)
             vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
             const T sx = p.dt * vx, sy = p.dt * vy, sz = p.dt * vz;
@@ -213,7 +218,11 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             if (rn.w > v.half_skin) v.flags[VF_REQ0 + req] = 1;
             rnew[i] = rn;
         }
-        if (kick || drift) { s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz; }
+        if (kick || drift || lam != T(1)) { s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz; }
+    }
+    if (ksum) {                                        // thermostat: this thread's share of K(t), one atomic per warp
+        kacc = warp_sum_d(kacc);
+        if ((threadIdx.x & 31) == 0 && kacc != 0.0) atomicAdd(ksum, kacc);
     }
 }
 
@@ -434,6 +443,7 @@ template <typename T, int ROWS, int MINB>
 __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
 {
     unsigned long long bar_target = 0;
+    const bool thermo = p.thermo_rate > 0.0;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
     const int gthreads = gridDim.x * blockDim.x;
     int c = v.flags[VF_CUR], cv = v.flags[VF_CURV];
@@ -465,10 +475,19 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
         }
         if (s == n_steps) break;
         const int req = (int)(s % 3);
-        if (gtid == 0) v.flags[VF_REQ0 + (req + 1) % 3] = 0;      // slot of step s + 1
+        if (gtid == 0) { v.flags[VF_REQ0 + (req + 1) % 3] = 0; if (thermo) v.ksum[(s + 1) % 3] = 0.0; }   // slots of step s + 1
         unsigned long long dbg0 = 0;
         if (v.dbg) dbg0 = now_ns();
-        phase_step<T>(p, v, c, cv, s > 0, s > 0, true, req, gtid, gthreads);
+        if (!thermo || s == 0) {
+            phase_step<T>(p, v, c, cv, s > 0, s > 0, true, req, gtid, gthreads);
+        } else {
+            // with the thermostat lambda(t) needs K(t) of ALL particles before the next drift: the fused phase splits
+            // into [F1 + F3 + K partial sums] | barrier | [F4 rescale + F2], one extra barrier per step
+            phase_step<T>(p, v, c, cv, true, true, false, req, gtid, gthreads, T(1), v.ksum + s % 3);
+            grid_barrier(v.bar, bar_target);
+            const double lam = berendsen_lambda(*(volatile double*)(v.ksum + s % 3), p.thermo_rate, p.t_target, p.dof);
+            phase_step<T>(p, v, c, cv, false, false, true, req, gtid, gthreads, (T)lam);
+        }
         if (v.dbg && (threadIdx.x & 31) == 0) atomicAdd(v.dbg + (gtid >> 5), now_ns() - dbg0);
         if (gtid == 0) { t1 = now_ns(); v.times[0] += t1 - t0; t0 = t1; }
         grid_barrier(v.bar, bar_target);
@@ -476,7 +495,15 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
         c ^= 1;
         rebuild = *(volatile int*)(v.flags + VF_REQ0 + req) != 0;
     }
-    if (n_steps > 0 || force_rebuild) phase_step<T>(p, v, c, cv, true, n_steps > 0, false, 0, gtid, gthreads);
+    if (thermo && n_steps > 0) {
+        double* ks = v.ksum + n_steps % 3;
+        phase_step<T>(p, v, c, cv, true, true, false, 0, gtid, gthreads, T(1), ks);
+        grid_barrier(v.bar, bar_target);
+        const double lam = berendsen_lambda(*(volatile double*)ks, p.thermo_rate, p.t_target, p.dof);
+        phase_step<T>(p, v, c, cv, false, false, false, 0, gtid, gthreads, (T)lam);      // F4 of the last step
+    } else if (n_steps > 0 || force_rebuild) {
+        phase_step<T>(p, v, c, cv, true, n_steps > 0, false, 0, gtid, gthreads);
+    }
     if (gtid == 0) { v.flags[VF_CUR] = c; v.flags[VF_CURV] = cv; v.times[3] += now_ns() - t0; }
 }
 

@@ -40,7 +40,7 @@ class md_lj(C.Structure):
 
 class md_opts(C.Structure):
     _fields_ = [("dt", C.c_double), ("mass", C.c_double), ("precision", C.c_int), ("force_algo", C.c_int),
-                ("skin", C.c_double)]
+                ("skin", C.c_double), ("tau_b", C.c_double), ("t_target", C.c_double)]
 
 
 class md_energy_out(C.Structure):
@@ -116,6 +116,7 @@ def _structs(cfg, precision=64, algo=None):
     opts.dt, opts.mass, opts.precision = float(cfg["dt"]), float(cfg["mass"]), int(precision)
     opts.force_algo = _ALGO[algo if algo is not None else cfg.get("algo", "auto")]
     opts.skin = float(cfg.get("skin", 0.0))
+    opts.tau_b, opts.t_target = float(cfg.get("tau_b", 0.0)), float(cfg.get("t_target", 1.0))
     return box, lj, opts
 
 

@@ -346,3 +346,28 @@ def test_fp32_trajectory_stays_close(algo):
     assert traj_error(st["pos"], ref["pos"], c32["box_len"], c32["bc"]) < 2e-3
     assert abs(en["K"] - ref["K"]) < 1e-4 * ref["K"] and abs(en["U"] - ref["U"]) < 2e-3 * max(abs(ref["U"]), 1.0)
     sim.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_berendsen_thermostat_matches_oracle(algo):
+    # NEXT-1: the paper's kernel F4 after every step; same tolerances as the NVE trajectories
+    cfg = dict(I.config4(12), tau_b=0.1, t_target=0.6)
+    ref = O.run(cfg, 100, cells=True, history=True)
+    sim = make_sim(cfg, algo)
+    for chunk in (1, 36, 63):
+        sim.step(chunk)
+    st, en = sim.get_state(), sim.energy()
+    assert traj_error(st["pos"], ref["pos"], cfg["box_len"], cfg["bc"]) <= TRAJ_TOL
+    assert np.abs(st["vel"] - ref["vel"]).max() <= 1e-7
+    assert abs(en["K"] - ref["K"]) <= 1e-9 * ref["K"]
+    t0 = 2 * ref["hist"][0, 0] / (3 * cfg["n_vapor"])
+    t100 = 2 * en["K"] / (3 * cfg["n_vapor"])
+    assert t0 > 0.95 and abs(t100 - 0.6) < 0.05                 # 5 rise times later the gas sits at T_0
+    sim.close()
+    # small 2D case, other parities of the step count
+    c2 = dict(I.small_case(2, 40, (13.7, 9.9), (0, 1), n_wall=12, seed=4, min_sep=0.9), tau_b=0.02, t_target=1.5)
+    r2 = O.run(c2, 33)
+    s2 = make_sim(c2, algo)
+    s2.step(33)
+    assert traj_error(s2.get_state()["pos"], r2["pos"], c2["box_len"], c2["bc"]) <= TRAJ_TOL
+    s2.close()

@@ -31,7 +31,7 @@ def test_exports_every_declared_symbol(lib):
 
 
 def test_struct_sizes_match_header_layout():
-    assert C.sizeof(md.md_box) == 48 and C.sizeof(md.md_lj) == 48 and C.sizeof(md.md_opts) == 32
+    assert C.sizeof(md.md_box) == 48 and C.sizeof(md.md_lj) == 48 and C.sizeof(md.md_opts) == 48
     assert C.sizeof(md.md_energy_out) == 64 and C.sizeof(md.md_kernel_times) == 88 and C.sizeof(md.md_peaks) == 24
 
 
@@ -78,6 +78,9 @@ def test_host_validation_errors(lib):
     bad["pos"] = cfg["pos"] * np.array([0.5, 1, 1])
     rc, msg, _ = _create_raw(lib, bad)
     assert rc == md.MD_ERR_INVALID_ARG and "2 r_cut" in msg
+    bad = dict(cfg, tau_b=0.001, t_target=1.0)               # tau_B < dt: lambda^2 could go negative
+    rc, msg, _ = _create_raw(lib, bad)
+    assert rc == md.MD_ERR_INVALID_ARG and "thermostat" in msg
     thin = I.small_case(2, 10, (6.0, 20.0), (0, 0), seed=2)
     rc, msg, _ = _create_raw(lib, thin, algo="cells")
     assert rc == md.MD_ERR_UNSUPPORTED
