@@ -11,7 +11,8 @@
 // dx*dx)), strict r^2 < r_c^2 -- and only that exact path produces forces and energies.
 // Periodic images are materialised once per step as ghost entries (particles within r_c of a periodic
 // face), so the inner loop has no minimum-image arithmetic.  Coordinates are centred on the box middle
-// to halve |r|^2.  fp32 mode keeps the per-pair minimum-image kernel of md_kernels.cuh.
+// to halve |r|^2.  The fp32 variant is at the end of this file; boxes with a periodic length below 2.2 r_c
+// (more than one image per dimension) keep the per-pair minimum-image kernel of md_kernels.cuh.
 #pragma once
 #include "md_kernels.cuh"
 
@@ -94,7 +95,8 @@ __global__ void k_ap_wall_list(Params<double> p, const Vec4<double>* __restrict_
 
 // a4 for the all-pairs path: second half-kick once every block's force contributions have landed; also
 // re-arms the ghost counter for the next step.
-__global__ void __launch_bounds__(256) k_ap_kick(Params<double> p, State<double> s, Force<double> f, int* __restrict__ ghost_count)
+template <typename T>
+__global__ void __launch_bounds__(256) k_ap_kick(Params<T> p, State<T> s, Force<T> f, int* __restrict__ ghost_count)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) *ghost_count = 0;
@@ -205,6 +207,170 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double
             atomicAdd(&eo.vir[i], 0.5 * wv[b] + ww[b]);
             atomicAdd(&eo.cvv[i], cv[b]);
             atomicAdd(&eo.cvw[i], cw[b]);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// fp32 mode of the same kernel.  The filter is the same 4-instruction form in FP32 (1 FADD + 3 FFMA); its
+// rounding (~1e-6 |r|^2) is covered by a wider margin.  Candidates are NOT re-evaluated from the centred
+// ghost entries -- a ghost coordinate x +- L rounded to fp32 would cost 4e-6 sigma -- but from the original
+// positions with the two-sided minimum image of md_kernels.cuh (exact differences for near pairs), found
+// through the original index every entry carries.
+// ---------------------------------------------------------------------------------------------------------
+struct AllPairsDotF {
+    Vec4<float>* jv;  int* jv_id;      // vapor entries + ghosts; id = particle index
+    Vec4<float>* jw;  int* jw_id;      // wall entries + ghosts (static); id = wall index (caller order)
+    const Vec4<float>* wr;             // wall positions, caller order
+    int* ghost_count;
+    int nwg;
+    float thr;                         // candidate iff filter r^2 < thr
+    float half[3];
+    float edge;
+};
+
+__device__ __forceinline__ void push_images_f(const Params<float>& p, const AllPairsDotF& a, float x, float y, float z, int id,
+                                              Vec4<float>* __restrict__ out, int* __restrict__ out_id, int base,
+                                              int* __restrict__ counter)
+{
+    float sx[2] = {0.f, 0.f}, sy[2] = {0.f, 0.f}, sz[2] = {0.f, 0.f};
+    int nx = 1, ny = 1, nz = 1;
+    if (p.bc[0] == BC_PERIODIC) { if (x < a.edge - a.half[0]) sx[nx++] = p.L[0]; else if (x > a.half[0] - a.edge) sx[nx++] = -p.L[0]; }
+    if (p.bc[1] == BC_PERIODIC) { if (y < a.edge - a.half[1]) sy[ny++] = p.L[1]; else if (y > a.half[1] - a.edge) sy[ny++] = -p.L[1]; }
+    if (p.bc[2] == BC_PERIODIC) { if (z < a.edge - a.half[2]) sz[nz++] = p.L[2]; else if (z > a.half[2] - a.edge) sz[nz++] = -p.L[2]; }
+    for (int c = 0; c < nz; ++c)
+        for (int b = 0; b < ny; ++b)
+            for (int q = 0; q < nx; ++q) {
+                if (q + b + c == 0) continue;
+                Vec4<float> e;
+                e.x = x + sx[q]; e.y = y + sy[b]; e.z = z + sz[c];
+                e.w = fmaf(e.z, e.z, fmaf(e.y, e.y, e.x * e.x));
+                const int k = base + atomicAdd(counter, 1);
+                out[k] = e;
+                out_id[k] = id;
+            }
+}
+
+template <bool MOVE>
+__global__ void __launch_bounds__(256) k_apf_kick_drift_list(Params<float> p, State<float> s, Force<float> f,
+                                                             AllPairsDotF a, int* __restrict__ err)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.nv) return;
+    Vec4<float> ri = s.r[i];
+    if (MOVE) {
+        float vx = s.vx[i] + p.hk * f.fx[i];
+        float vy = s.vy[i] + p.hk * f.fy[i];
+        float vz = s.vz[i] + p.hk * f.fz[i];
+        ri.x += p.dt * vx; ri.y += p.dt * vy; ri.z += p.dt * vz;
+        boundary(ri.x, vx, p.L[0], p.bc[0], err);
+        boundary(ri.y, vy, p.L[1], p.bc[1], err);
+        boundary(ri.z, vz, p.L[2], p.bc[2], err);
+        s.r[i] = ri;
+        s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz;
+    }
+    f.fx[i] = 0.f; f.fy[i] = 0.f; f.fz[i] = 0.f;
+    Vec4<float> e;
+    e.x = ri.x - a.half[0]; e.y = ri.y - a.half[1]; e.z = ri.z - a.half[2];
+    e.w = fmaf(e.z, e.z, fmaf(e.y, e.y, e.x * e.x));
+    a.jv[i] = e;
+    a.jv_id[i] = i;
+    push_images_f(p, a, e.x, e.y, e.z, i, a.jv, a.jv_id, p.nv, a.ghost_count);
+}
+
+__global__ void k_apf_wall_list(Params<float> p, AllPairsDotF a, int* __restrict__ counter)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.nw) return;
+    Vec4<float> e;
+    e.x = a.wr[i].x - a.half[0]; e.y = a.wr[i].y - a.half[1]; e.z = a.wr[i].z - a.half[2];
+    e.w = fmaf(e.z, e.z, fmaf(e.y, e.y, e.x * e.x));
+    a.jw[i] = e;
+    a.jw_id[i] = i;
+    push_images_f(p, a, e.x, e.y, e.z, i, a.jw, a.jw_id, p.nw, counter);
+}
+
+template <bool ENERGY>
+__global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dotf(Params<float> p, State<float> s, AllPairsDotF a,
+                                                                    Force<float> f, EnergyOut eo)
+{
+    __shared__ Vec4<float> sj[AD_THREADS];
+    __shared__ int sid[AD_THREADS];
+    const int base = blockIdx.x * (AD_THREADS * AD_IB) + threadIdx.x;
+    float ax[AD_IB], ay[AD_IB], az[AD_IB], si[AD_IB];
+    Vec4<float> ro[AD_IB];                                    // original positions, for the exact path
+    int idx[AD_IB];
+#pragma unroll
+    for (int b = 0; b < AD_IB; ++b) {
+        idx[b] = base + b * AD_THREADS;
+        Vec4<float> e = {1.0e9f, 1.0e9f, 1.0e9f, 3.0e18f};
+        ro[b] = e;
+        if (idx[b] < p.nv) { e = a.jv[idx[b]]; ro[b] = s.r[idx[b]]; }
+        ax[b] = -2.f * e.x; ay[b] = -2.f * e.y; az[b] = -2.f * e.z; si[b] = e.w;
+    }
+    Acc<float, ENERGY> av[AD_IB], aw[AD_IB];
+    bool any = false;
+    const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
+    const int nvj = p.nv + *a.ghost_count;
+    const int tiles_v = (nvj + AD_THREADS - 1) / AD_THREADS, tiles_w = (a.nwg + AD_THREADS - 1) / AD_THREADS;
+    const float thr = a.thr;
+    for (int t = blockIdx.y; t < tiles_v + tiles_w; t += gridDim.y) {
+        const bool wall = t >= tiles_v;
+        const int j0 = (wall ? t - tiles_v : t) * AD_THREADS;
+        const int nj = wall ? a.nwg : nvj;
+        __syncthreads();
+        {
+            Vec4<float> e = {-1.0e9f, -1.0e9f, -1.0e9f, 3.0e18f};
+            int id = -1;
+            if (j0 + threadIdx.x < nj) { e = (wall ? a.jw : a.jv)[j0 + threadIdx.x]; id = (wall ? a.jw_id : a.jv_id)[j0 + threadIdx.x]; }
+            sj[threadIdx.x] = e;
+            sid[threadIdx.x] = id;
+        }
+        __syncthreads();
+        for (int k0 = 0; k0 < AD_THREADS; k0 += AD_UNROLL) {
+            bool cand = false;
+#pragma unroll
+            for (int u = 0; u < AD_UNROLL; ++u) {
+                const Vec4<float> q = sj[k0 + u];
+#pragma unroll
+                for (int b = 0; b < AD_IB; ++b)
+                    cand |= fmaf(ax[b], q.x, fmaf(ay[b], q.y, fmaf(az[b], q.z, si[b] + q.w))) < thr;
+            }
+            if (cand) {
+                for (int u = 0; u < AD_UNROLL; ++u) {
+                    const Vec4<float> q = sj[k0 + u];
+                    const int jo = sid[k0 + u];
+#pragma unroll
+                    for (int b = 0; b < AD_IB; ++b) {
+                        if (!(fmaf(ax[b], q.x, fmaf(ay[b], q.y, fmaf(az[b], q.z, si[b] + q.w))) < thr)) continue;
+                        if (jo < 0 || idx[b] >= p.nv || (!wall && jo == idx[b])) continue;
+                        const Vec4<float> rj = wall ? a.wr[jo] : s.r[jo];
+                        float dx = ro[b].x - rj.x, dy = ro[b].y - rj.y, dz = ro[b].z - rj.z;
+                        if (px) dx = min_image(ro[b].x, rj.x, dx, p.L[0], p.invL[0]);
+                        if (py) dy = min_image(ro[b].y, rj.y, dy, p.L[1], p.invL[1]);
+                        if (pz) dz = min_image(ro[b].z, rj.z, dz, p.L[2], p.invL[2]);
+                        if (wall) pair_term<float, ENERGY>(dx, dy, dz, p.rc2, p.sig2_vw, p.e24_vw, p.e4_vw, p.uc_vw, aw[b]);
+                        else pair_term<float, ENERGY>(dx, dy, dz, p.rc2, p.sig2_vv, p.e24_vv, p.e4_vv, p.uc_vv, av[b]);
+                    }
+                }
+                any = true;
+            }
+        }
+    }
+    if (!any) return;
+#pragma unroll
+    for (int b = 0; b < AD_IB; ++b) {
+        const int i = idx[b];
+        if (i >= p.nv) continue;
+        const float fx = av[b].fx + aw[b].fx, fy = av[b].fy + aw[b].fy, fz = av[b].fz + aw[b].fz;
+        if (!ENERGY) {
+            if (fx != 0.f || fy != 0.f || fz != 0.f) { atomicAdd(&f.fx[i], fx); atomicAdd(&f.fy[i], fy); atomicAdd(&f.fz[i], fz); }
+        } else if (av[b].c | aw[b].c) {
+            atomicAdd(&eo.pe[i], 0.5 * av[b].u + aw[b].u);
+            atomicAdd(&eo.pew[i], aw[b].u);
+            atomicAdd(&eo.vir[i], 0.5 * av[b].w + aw[b].w);
+            atomicAdd(&eo.cvv[i], av[b].c);
+            atomicAdd(&eo.cvw[i], aw[b].c);
         }
     }
 }

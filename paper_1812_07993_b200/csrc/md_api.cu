@@ -128,7 +128,8 @@ struct Layout {
     int *nbr, *ncnt, *vflags;   // VERLET: neighbour list, counts, flags
     unsigned long long *vtimes, *vbar;
     double* vksum;              // VERLET thermostat: rotating kinetic-energy accumulators
-    md::Vec4<double> *jv, *jw;  // ALLPAIRS fp64: j lists (entries + ghosts) of the dot-product kernel
+    md::Vec4<T> *jv, *jw;       // ALLPAIRS: j lists (entries + ghosts) of the dot-product kernels
+    int *jv_id, *jw_id;         // fp32: original index of every entry
     int* ghost_count;
     int red_blocks;
     size_t bytes;
@@ -170,9 +171,11 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.nbr = c.take<int>(verlet ? n * md::VL_MAXN : 1);
     l.ncnt = c.take<int>(verlet ? n : 1);
     l.vflags = c.take<int>(md::VF_COUNT);
-    const bool dot = algo == MD_FORCE_ALLPAIRS && sizeof(T) == 8;
-    l.jv = c.take<md::Vec4<double>>(dot ? 8 * n : 1);     // <= 7 periodic images per particle
-    l.jw = c.take<md::Vec4<double>>(dot ? 8 * m : 1);
+    const bool dot = algo == MD_FORCE_ALLPAIRS;
+    l.jv = c.take<md::Vec4<T>>(dot ? 8 * n : 1);          // <= 7 periodic images per particle
+    l.jw = c.take<md::Vec4<T>>(dot ? 8 * m : 1);
+    l.jv_id = c.take<int>(dot && sizeof(T) == 4 ? 8 * n : 1);
+    l.jw_id = c.take<int>(dot && sizeof(T) == 4 ? 8 * m : 1);
     l.ghost_count = c.take<int>(4);
     l.vtimes = c.take<unsigned long long>(8 + 8192);
     l.vbar = c.take<unsigned long long>(2);
@@ -228,7 +231,8 @@ struct Sim : md_sim {
     unsigned long long phase_seen[4] = {0, 0, 0, 0}, phase_ns[4] = {0, 0, 0, 0};
 
     md::AllPairsDot ad;
-    bool dot = false;           // fp64 all-pairs through the dot-product kernel (md_allpairs.cuh)
+    md::AllPairsDotF adf;
+    bool dot = false;           // all-pairs through the dot-product kernels (md_allpairs.cuh)
     int ad_slices = 1;
     int gpar = 0;               // which of the two ghost counters describes the current j list
 
@@ -316,8 +320,8 @@ struct Sim : md_sim {
                 md::k_force_cells<T, 3, ENERGY, KICK, COUNT><<<cdiv(cdiv(p.nv, 10), 4), 128, 0, stream>>>(
                     p, l.st[cur], l.start, walls, l.f, l.eo, l.tests);
         } else if (dot) {
-            if constexpr (std::is_same<T, double>::value) {
-                ad.ghost_count = l.ghost_count + gpar;
+            {
+                ad.ghost_count = adf.ghost_count = l.ghost_count + gpar;
                 if (ENERGY) {
                     const size_t n = (size_t)p.nv;
                     cudaMemsetAsync(l.eo.pe, 0, n * sizeof(double), stream);
@@ -327,9 +331,12 @@ struct Sim : md_sim {
                     cudaMemsetAsync(l.eo.cvw, 0, n * sizeof(int), stream);
                 }
                 const dim3 grid(cdiv(p.nv, md::AD_THREADS * md::AD_IB), ad_slices);
-                md::k_force_allpairs_dot<ENERGY><<<grid, md::AD_THREADS, 0, stream>>>(p, ad, l.f, l.eo);
+                if constexpr (std::is_same<T, double>::value)
+                    md::k_force_allpairs_dot<ENERGY><<<grid, md::AD_THREADS, 0, stream>>>(p, ad, l.f, l.eo);
+                else
+                    md::k_force_allpairs_dotf<ENERGY><<<grid, md::AD_THREADS, 0, stream>>>(p, l.st[cur], adf, l.f, l.eo);
                 // the second half-kick also clears the OTHER ghost counter, which the next step's list will fill
-                if (KICK) md::k_ap_kick<<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, l.ghost_count + (gpar ^ 1));
+                if (KICK) md::k_ap_kick<T><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, l.ghost_count + (gpar ^ 1));
             }
         } else
             md::k_force_allpairs<T, ENERGY, KICK><<<blocks(md::AP_THREADS), md::AP_THREADS, 0, stream>>>(
@@ -353,9 +360,11 @@ struct Sim : md_sim {
         } else {
             if (dot) {
                 gpar ^= 1;
-                ad.ghost_count = l.ghost_count + gpar;
+                ad.ghost_count = adf.ghost_count = l.ghost_count + gpar;
                 if constexpr (std::is_same<T, double>::value)
                     md::k_ap_kick_drift_list<true><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, ad, l.err);
+                else
+                    md::k_apf_kick_drift_list<true><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, adf, l.err);
             } else
                 md::k_kick_drift_bin<T, true, false><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, nullptr, nullptr,
                                                                                      nullptr, l.err);
@@ -407,7 +416,7 @@ struct Sim : md_sim {
                 if (!g1[par]) { int c0 = cur, g0 = gpar; int rc = capture(1, &g1[par]); cur = c0; gpar = g0; if (rc) return rc; }
                 CK(cudaGraphLaunch(g1[par], stream));
                 if (algo == MD_FORCE_CELLS) cur ^= 1;
-                if (dot) { gpar ^= 1; ad.ghost_count = l.ghost_count + gpar; }
+                if (dot) { gpar ^= 1; ad.ghost_count = adf.ghost_count = l.ghost_count + gpar; }
                 n -= 1; step_no += 1;
             }
         }
@@ -558,7 +567,7 @@ struct Sim : md_sim {
                 int g = 0;
                 CK(cudaMemcpyAsync(&g, l.ghost_count + gpar, sizeof(int), cudaMemcpyDeviceToHost, stream));
                 CK(cudaStreamSynchronize(stream));
-                *tests = (long long)p.nv * ((long long)p.nv - 1 + g + ad.nwg);
+                *tests = (long long)p.nv * ((long long)p.nv - 1 + g + (sizeof(T) == 8 ? ad.nwg : adf.nwg));
             }
             return MD_OK;
         }
@@ -658,19 +667,27 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
         cur = 1;
     }
     if (dot) {
-        if constexpr (std::is_same<T, double>::value) {
+        {
             CK(cudaMemsetAsync(l.ghost_count, 0, 4 * sizeof(int), stream));
-            if (nw > 0) md::k_ap_wall_list<<<cdiv(nw, 256), 256, 0, stream>>>(p, l.wtr, ad, l.ghost_count + 2);
+            if (nw > 0) {
+                if constexpr (std::is_same<T, double>::value)
+                    md::k_ap_wall_list<<<cdiv(nw, 256), 256, 0, stream>>>(p, l.wtr, ad, l.ghost_count + 2);
+                else
+                    md::k_apf_wall_list<<<cdiv(nw, 256), 256, 0, stream>>>(p, adf, l.ghost_count + 2);
+            }
             int wg = 0;
             CK(cudaMemcpyAsync(&wg, l.ghost_count + 2, sizeof(int), cudaMemcpyDeviceToHost, stream));
             CK(cudaStreamSynchronize(stream));
-            ad.nwg = (int)nw + wg;
+            ad.nwg = adf.nwg = (int)nw + wg;
             const int tiles = cdiv(nv, md::AD_THREADS) + cdiv(ad.nwg, md::AD_THREADS) + 1;
             // j slices: enough blocks to fill the GPU, and a block count that wastes little of the last wave
             int dev = 0, sms = 148, nb = 4;
             cudaGetDevice(&dev);
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, md::k_force_allpairs_dot<false>, md::AD_THREADS, 0);
+            if constexpr (std::is_same<T, double>::value)
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, md::k_force_allpairs_dot<false>, md::AD_THREADS, 0);
+            else
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, md::k_force_allpairs_dotf<false>, md::AD_THREADS, 0);
             const int slots = std::max(1, nb * sms), ib = cdiv(nv, md::AD_THREADS * md::AD_IB);
             double best = -1.0;
             for (int sl = 1; sl <= std::min(tiles, 96); ++sl) {
@@ -678,7 +695,10 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
                 const double eff = waves / std::ceil(waves) - (sl * 1e-4) + (waves >= 1.0 ? 0.0 : waves - 1.0);
                 if (eff > best) { best = eff; ad_slices = sl; }
             }
-            md::k_ap_kick_drift_list<false><<<blocks(256), 256, 0, stream>>>(p, l.st[0], l.f, ad, l.err);
+            if constexpr (std::is_same<T, double>::value)
+                md::k_ap_kick_drift_list<false><<<blocks(256), 256, 0, stream>>>(p, l.st[0], l.f, ad, l.err);
+            else
+                md::k_apf_kick_drift_list<false><<<blocks(256), 256, 0, stream>>>(p, l.st[0], l.f, adf, l.err);
         }
     }
     launch_force<false, false, false>();   // f(0)
@@ -725,7 +745,7 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
     p.uc_vw = (T)ucut(lj.eps_w, lj.sigma_w);
     p.dt = (T)o.dt; p.hk = (T)(o.dt / (2.0 * o.mass)); p.mass = o.mass;
     p.thermo_rate = o.tau_b > 0 ? o.dt / o.tau_b : 0.0; p.t_target = o.t_target; p.dof = (double)box.dim * (double)nv;
-    if (algo == MD_FORCE_ALLPAIRS && sizeof(T) == 8) {
+    if (algo == MD_FORCE_ALLPAIRS) {
         // dot-product kernel: needs at most one periodic image per dimension inside r_c + margin of a face
         bool ok = true;
         double smax = 0.0;
@@ -737,7 +757,8 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
         if (ok) {
             md::AllPairsDot& a = s->ad;
             s->dot = true;
-            a.jv = s->l.jv; a.jw = s->l.jw; a.ghost_count = s->l.ghost_count; a.nwg = 0;
+            if constexpr (std::is_same<T, double>::value) { a.jv = s->l.jv; a.jw = s->l.jw; }
+            a.ghost_count = s->l.ghost_count; a.nwg = 0;
             for (int k = 0; k < 3; ++k) a.half[k] = k < box.dim ? 0.5 * box.len[k] : 0.0;
             a.edge = lj.r_cut * (1.0 + 1e-9) + 1e-9;
             // filter threshold: r_c^2 plus a bound on the rounding of the 4-term dot-product form
@@ -745,6 +766,15 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
             long long bits;
             memcpy(&bits, &thr, sizeof(bits));
             a.thr_hi = (int)(bits >> 32) + 1;
+            if constexpr (std::is_same<T, float>::value) {
+                md::AllPairsDotF& g = s->adf;
+                g.jv = s->l.jv; g.jw = s->l.jw; g.jv_id = s->l.jv_id; g.jw_id = s->l.jw_id; g.wr = s->l.wtr;
+                g.ghost_count = s->l.ghost_count; g.nwg = 0;
+                for (int k = 0; k < 3; ++k) g.half[k] = (float)a.half[k];
+                g.edge = (float)(lj.r_cut * (1.0 + 1e-5) + 1e-4);
+                // fp32 filter: rounding of the 4-term form (~6 eps32 |r|^2 terms) plus the centring error
+                g.thr = (float)(lj.r_cut * lj.r_cut + 1e-6 * smax + 1e-3);
+            }
         }
     }
     if (algo == MD_FORCE_VERLET) {

@@ -38,7 +38,7 @@ def measure(cfg, algo, precision, n_steps, torch, md, peaks):
                steps_timed=n_steps, md_steps_per_s=1.0 / sec, pair_interactions_per_s=inter / sec,
                pair_tests_per_s=tests / sec, us_per_step=sec * 1e6)
     if algo == "allpairs":
-        flops = 7.0 if precision == 64 else 14.0     # executed per test: DESIGN.md section 5
+        flops = 7.0                                   # executed per test (1 add + 3 fma): DESIGN.md section 5
         peak = peaks["fp64_tflops"] if precision == 64 else peaks["fp32_tflops"]
         row["alu_tflops"] = tests * flops / sec * 1e-12
         row["alu_frac_of_measured_peak"] = row["alu_tflops"] / peak
