@@ -52,7 +52,10 @@ enum { MD_PORE_NONE = 0, MD_PORE_SLIT, MD_PORE_CYLINDER, MD_PORE_CONE, MD_PORE_I
  * MD_BC_REFLECT (specular reflection after the drift). */
 typedef struct { int dim; double len[3]; int bc[3]; } md_box;
 
-/* Descriptive only (the hot path sees wall PARTICLES, not shapes); stored and returned untouched. */
+/* Pore region.  The hot path sees wall PARTICLES, not shapes; the descriptor only selects the volume md_pressure
+ * monitors: MD_PORE_CYLINDER (3D): distance from the axis line through `center` along dimension `axis` < r0 and
+ * |along - center[axis]| < length/2; MD_PORE_SLIT (2D): |r[axis] - center[axis]| < width/2 (axis = wall normal) and
+ * |r[1-axis] - center[1-axis]| < length/2.  Other kinds are stored but not monitored. */
 typedef struct { int kind, axis; double center[3], length, r0, r1, neck_len, width; } md_pore;
 
 /* 12-6 Lennard-Jones: u(r) = 4 eps [(sigma/r)^12 - (sigma/r)^6] for r < r_cut, else 0 (strict <);
@@ -78,6 +81,12 @@ typedef struct { double dt, mass; int precision, force_algo; double skin; double
  * vw pairs of g.d (g = force on the vapor particle, d = r_i - r_j); pairs_* = pairs with r < r_cut. */
 typedef struct { double kinetic, potential, potential_vv, potential_vw, virial;
                  long long pairs_vv, pairs_vw; long long step; } md_energy_out;
+
+/* Virial pressure: P = (2K + W) / (dim V), K and W = sum_i (1/2 sum_j g.d + sum_w g.d) summed over
+ * the particles inside the volume (k_B = 1; W as in md_energy_out.virial: positive = repulsive.  The paper prints the
+ * virial term with a minus sign, i.e. with the opposite sign convention for f(r_ij): DESIGN.md reading A17). */
+typedef struct { double pressure_box, volume_box, pressure_pore, volume_pore, kinetic_pore, virial_pore;
+                 long long n_pore; long long step; } md_pressure_out;
 
 /* Per-kernel device times of md_profile_step, milliseconds summed over the profiled steps, and
  * launch counts.  Index: 0 kick+drift(+bin count), 1 scan, 2 scatter, 3 force(+half-kick).  VERLET: the
@@ -114,6 +123,10 @@ int md_get_state(md_sim*, double* pos, double* vel, double* force, double* pe, l
 /* Kinetic / potential energies, virial and pair counts at the current step (host struct).
  * MD_ERR_NONFINITE if K or U is not finite. */
 int md_energy(md_sim*, md_energy_out* out);
+
+/* Box pressure and pressure inside the pore region given to md_create at the current step (host struct).
+ * MD_ERR_UNSUPPORTED if no monitored pore kind was given (pressure_box is still filled). */
+int md_pressure(md_sim*, md_pressure_out* out);
 
 /* Like md_step but synchronous, one launch at a time with CUDA events around every kernel. */
 int md_profile_step(md_sim*, long long n_steps, md_kernel_times* out);

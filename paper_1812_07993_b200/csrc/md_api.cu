@@ -198,6 +198,9 @@ struct md_sim {
     virtual int profile(long long n, md_kernel_times* out) = 0;
     virtual int pair_tests(long long* tests) = 0;
     virtual void info(int* algo, int nc[3], int* kps) const = 0;
+    virtual int pressure(md_pressure_out* out) = 0;
+    md_pore pore = {};
+    md_box box = {};
 };
 
 #define CK(call)                                                                                   \
@@ -591,6 +594,41 @@ struct Sim : md_sim {
         return MD_OK;
     }
 
+    int pressure(md_pressure_out* out) override
+    {
+        if (!out) { err = "out is NULL"; return MD_ERR_INVALID_ARG; }
+        int rc = check_err_flag();
+        if (rc) return rc;
+        if ((rc = energy_pass())) return rc;               // per-particle virial of the current step
+        md::PoreRegion g = {};
+        double vol_pore = 0.0;
+        const double PI = 3.14159265358979323846;
+        if (pore.kind == MD_PORE_SLIT && dim == 2 && (pore.axis == 0 || pore.axis == 1)) {
+            g.kind = 1; vol_pore = pore.width * pore.length;
+        } else if (pore.kind == MD_PORE_CYLINDER && dim == 3 && pore.axis >= 0 && pore.axis < 3) {
+            g.kind = 2; vol_pore = PI * pore.r0 * pore.r0 * pore.length;
+        }
+        g.axis = pore.axis;
+        for (int k = 0; k < 3; ++k) g.c[k] = pore.center[k];
+        g.half_len = 0.5 * pore.length; g.r0sq = pore.r0 * pore.r0; g.half_width = 0.5 * pore.width;
+        md::k_pressure_partial<T><<<l.red_blocks, md::RED_THREADS, 0, stream>>>(p, view(), l.eo.vir, g, l.part);
+        md::k_energy_final<<<1, md::RED_THREADS, 0, stream>>>(l.red_blocks, l.part, l.eout);
+        double h[6];
+        CK(cudaMemcpyAsync(h, l.eout, sizeof(h), cudaMemcpyDeviceToHost, stream));
+        CK(cudaStreamSynchronize(stream));
+        CK(cudaGetLastError());
+        double vol_box = 1.0;
+        for (int k = 0; k < dim; ++k) vol_box *= box.len[k];
+        out->volume_box = vol_box;
+        out->pressure_box = (2.0 * h[0] + h[1]) / (dim * vol_box);
+        out->volume_pore = vol_pore;
+        out->kinetic_pore = h[2]; out->virial_pore = h[3]; out->n_pore = (long long)llround(h[4]);
+        out->pressure_pore = vol_pore > 0 ? (2.0 * h[2] + h[3]) / (dim * vol_pore) : 0.0;
+        out->step = step_no;
+        if (g.kind == 0) { err = "no monitored pore region (MD_PORE_SLIT in 2D or MD_PORE_CYLINDER in 3D)"; return MD_ERR_UNSUPPORTED; }
+        return MD_OK;
+    }
+
     void info(int* a, int nc[3], int* kps) const override
     {
         if (a) *a = algo;
@@ -715,6 +753,7 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
     Sim<T>* s = new Sim<T>();
     const bool cells = algo != MD_FORCE_ALLPAIRS;
     s->dim = box.dim;
+    s->box = box;
     s->algo = algo;
     s->stream = (cudaStream_t)stream;
     s->l = carve<T>(ws, box.dim, nv, nw, g.ncell, algo);
@@ -835,7 +874,6 @@ int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj*
               const double* pos, const double* vel, long long nw, const double* wall, void* ws, size_t ws_bytes,
               void* stream)
 {
-    (void)pore;
     if (!out) { g_create_error = "out is NULL"; return MD_ERR_INVALID_ARG; }
     *out = nullptr;
     const char* why = validate(box, lj, o, nv, nw);
@@ -864,9 +902,11 @@ int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj*
         g_create_error = "no CUDA device (there is no CPU fallback)";
         return MD_ERR_CUDA;
     }
-    return o->precision == 64
-               ? create_t<double>(out, *box, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo)
-               : create_t<float>(out, *box, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo);
+    int rc = o->precision == 64
+                 ? create_t<double>(out, *box, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo)
+                 : create_t<float>(out, *box, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo);
+    if (rc == MD_OK && pore) (*out)->pore = *pore;
+    return rc;
 }
 
 int md_step(md_sim* s, long long n) { return s ? s->step(n) : MD_ERR_INVALID_ARG; }
@@ -877,6 +917,7 @@ int md_get_state(md_sim* s, double* pos, double* vel, double* force, double* pe,
 int md_energy(md_sim* s, md_energy_out* out) { return s ? s->energy(out) : MD_ERR_INVALID_ARG; }
 int md_profile_step(md_sim* s, long long n, md_kernel_times* out) { return s ? s->profile(n, out) : MD_ERR_INVALID_ARG; }
 int md_pair_tests(md_sim* s, long long* t) { return s ? s->pair_tests(t) : MD_ERR_INVALID_ARG; }
+int md_pressure(md_sim* s, md_pressure_out* out) { return s ? s->pressure(out) : MD_ERR_INVALID_ARG; }
 int md_info(const md_sim* s, int* algo, int nc[3], int* kps)
 {
     if (!s) return MD_ERR_INVALID_ARG;

@@ -604,6 +604,41 @@ __global__ void __launch_bounds__(RED_THREADS) k_energy_final(int nblocks, const
     block_sum6(v, out, 1);
 }
 
+// NEXT-2, virial pressure: per-block sums of K and W over all particles and over the particles
+// inside the pore region; part layout [6][nblocks]: K_all, W_all, K_in, W_in, n_in, 0 (summed by k_energy_final).
+struct PoreRegion {
+    int kind;          // 0 none, 1 slit (2D), 2 cylinder (3D)
+    int axis;
+    double c[3], half_len, r0sq, half_width;
+};
+
+template <typename T>
+__global__ void __launch_bounds__(RED_THREADS) k_pressure_partial(Params<T> p, State<T> s, const double* __restrict__ vir,
+                                                                 PoreRegion g, double* __restrict__ part)
+{
+    double v[6] = {0, 0, 0, 0, 0, 0};
+    for (int i = blockIdx.x * RED_THREADS + threadIdx.x; i < p.nv; i += gridDim.x * RED_THREADS) {
+        const double vx = (double)s.vx[i], vy = (double)s.vy[i], vz = (double)s.vz[i];
+        const double k = 0.5 * p.mass * (vx * vx + vy * vy + vz * vz), w = vir[i];
+        Vec4<T> ri = s.r[i];
+        T dummy = T(0);
+        int err = 0;
+        boundary(ri.x, dummy, p.L[0], p.bc[0] == BC_PERIODIC ? BC_PERIODIC : BC_NONE, &err);   // VERLET keeps them unwrapped
+        boundary(ri.y, dummy, p.L[1], p.bc[1] == BC_PERIODIC ? BC_PERIODIC : BC_NONE, &err);
+        boundary(ri.z, dummy, p.L[2], p.bc[2] == BC_PERIODIC ? BC_PERIODIC : BC_NONE, &err);
+        const double d[3] = {(double)ri.x - g.c[0], (double)ri.y - g.c[1], (double)ri.z - g.c[2]};
+        bool in = false;
+        if (g.kind == 1) in = fabs(d[g.axis]) < g.half_width && fabs(d[1 - g.axis]) < g.half_len;
+        else if (g.kind == 2) {
+            const int a1 = (g.axis + 1) % 3, a2 = (g.axis + 2) % 3;
+            in = fabs(d[g.axis]) < g.half_len && d[a1] * d[a1] + d[a2] * d[a2] < g.r0sq;
+        }
+        v[0] += k; v[1] += w;
+        if (in) { v[2] += k; v[3] += w; v[4] += 1.0; }
+    }
+    block_sum6(v, part + blockIdx.x, gridDim.x);
+}
+
 // ---------------------------------------------------------------------------
 // F4, Berendsen thermostat for the multi-kernel paths: block partial sums of K, then every
 // block re-sums the partials in the same fixed order, forms lambda and rescales its velocities.

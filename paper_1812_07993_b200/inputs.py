@@ -210,7 +210,7 @@ def config1(seed=BASE_SEED + 1, n_vapor=16384):
     c = (300.0, 300.0)
     wall = wall_slit2d_rows(c, 200, 2048, 5.0)
     return _finish("cfg1_slit2d_16k", seed, 2, (600.0, 600.0), (BC_PERIODIC, BC_REFLECT), wall, n_vapor, 0.3,
-                   10000, "cells")
+                   10000, "cells", pore=dict(kind="slit", axis=1, center=c, length=200.0, width=10.0))
 
 
 def cylinder_config(n_vapor, seed, name, steps=1000, algo="cells", density=0.05, box=None, length=None):
@@ -220,7 +220,8 @@ def cylinder_config(n_vapor, seed, name, steps=1000, algo="cells", density=0.05,
     c = (0.5 * L, 0.5 * L, 0.5 * L)
     wall = wall_cylinder(c, 5.0, length)
     return _finish(name, seed, 3, (L, L, L), (BC_PERIODIC, BC_PERIODIC, BC_REFLECT), wall, n_vapor, 0.3,
-                   steps, algo, pore_length=length)
+                   steps, algo, pore_length=length,
+                   pore=dict(kind="cylinder", axis=2, center=c, length=float(length), r0=5.0) if length > 0 else None)
 
 
 def config2(seed=BASE_SEED + 2):

@@ -20,7 +20,7 @@ MD_BC_PERIODIC, MD_BC_REFLECT = 0, 1
 MD_FORCE_AUTO, MD_FORCE_ALLPAIRS, MD_FORCE_CELLS, MD_FORCE_VERLET = 0, 1, 2, 3
 _ALGO = {"auto": MD_FORCE_AUTO, "allpairs": MD_FORCE_ALLPAIRS, "cells": MD_FORCE_CELLS, "verlet": MD_FORCE_VERLET}
 
-EXPORTS = ["md_workspace_bytes", "md_create", "md_step", "md_get_state", "md_energy", "md_profile_step",
+EXPORTS = ["md_workspace_bytes", "md_create", "md_step", "md_get_state", "md_energy", "md_pressure", "md_profile_step",
            "md_pair_tests", "md_info", "md_measure_peaks", "md_destroy", "md_last_error"]
 
 
@@ -47,6 +47,12 @@ class md_energy_out(C.Structure):
     _fields_ = [("kinetic", C.c_double), ("potential", C.c_double), ("potential_vv", C.c_double),
                 ("potential_vw", C.c_double), ("virial", C.c_double), ("pairs_vv", C.c_longlong),
                 ("pairs_vw", C.c_longlong), ("step", C.c_longlong)]
+
+
+class md_pressure_out(C.Structure):
+    _fields_ = [("pressure_box", C.c_double), ("volume_box", C.c_double), ("pressure_pore", C.c_double),
+                ("volume_pore", C.c_double), ("kinetic_pore", C.c_double), ("virial_pore", C.c_double),
+                ("n_pore", C.c_longlong), ("step", C.c_longlong)]
 
 
 class md_kernel_times(C.Structure):
@@ -89,6 +95,8 @@ def load_library():
         lib.md_get_state.argtypes = [C.c_void_p, _DP, _DP, _DP, _DP, C.POINTER(C.c_longlong)]
         lib.md_energy.restype = C.c_int
         lib.md_energy.argtypes = [C.c_void_p, C.POINTER(md_energy_out)]
+        lib.md_pressure.restype = C.c_int
+        lib.md_pressure.argtypes = [C.c_void_p, C.POINTER(md_pressure_out)]
         lib.md_profile_step.restype = C.c_int
         lib.md_profile_step.argtypes = [C.c_void_p, C.c_longlong, C.POINTER(md_kernel_times)]
         lib.md_pair_tests.restype = C.c_int
@@ -153,7 +161,16 @@ class Simulation:
         self.workspace = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=self.device)
         torch.cuda.synchronize(self.device)
         self._h = C.c_void_p()
-        rc = self._lib.md_create(C.byref(self._h), C.byref(box), None, C.byref(lj), C.byref(opts), self.n_vapor,
+        pore = None
+        if cfg.get("pore"):                       # dict(kind="cylinder"|"slit", axis, center, length, r0 | width)
+            pd = cfg["pore"]
+            pore = md_pore()
+            pore.kind = {"slit": 1, "cylinder": 2}[pd["kind"]]
+            pore.axis = int(pd["axis"])
+            for a, c in enumerate(pd["center"]):
+                pore.center[a] = float(c)
+            pore.length, pore.r0, pore.width = float(pd["length"]), float(pd.get("r0", 0.0)), float(pd.get("width", 0.0))
+        rc = self._lib.md_create(C.byref(self._h), C.byref(box), C.byref(pore) if pore else None, C.byref(lj), C.byref(opts), self.n_vapor,
                                  _dptr(pos), _dptr(vel), n_wall, _dptr(wall) if n_wall else None,
                                  self.workspace.data_ptr(), self.workspace.numel(), self.stream.cuda_stream)
         if rc != MD_OK:
@@ -184,6 +201,12 @@ class Simulation:
         self._check(self._lib.md_energy(self._h, C.byref(e)))
         return dict(K=e.kinetic, U=e.potential, U_vv=e.potential_vv, U_vw=e.potential_vw, virial=e.virial,
                     pairs_vv=e.pairs_vv, pairs_vw=e.pairs_vw, step=e.step)
+
+    def pressure(self):
+        o = md_pressure_out()
+        self._check(self._lib.md_pressure(self._h, C.byref(o)))
+        return dict(P_box=o.pressure_box, V_box=o.volume_box, P_pore=o.pressure_pore, V_pore=o.volume_pore,
+                    K_pore=o.kinetic_pore, W_pore=o.virial_pore, n_pore=o.n_pore, step=o.step)
 
     def profile_step(self, n_steps: int):
         t = md_kernel_times()

@@ -371,3 +371,51 @@ def test_berendsen_thermostat_matches_oracle(algo):
     s2.step(33)
     assert traj_error(s2.get_state()["pos"], r2["pos"], c2["box_len"], c2["bc"]) <= TRAJ_TOL
     s2.close()
+
+
+def _oracle_pressure(cfg, out):
+    """(P_box, P_pore, n_pore) from the oracle's positions, velocities and per-particle virial."""
+    dim = cfg["dim"]
+    L = np.array(cfg["box_len"][:dim])
+    k = 0.5 * cfg["mass"] * (out["vel"] ** 2).sum(axis=1)
+    w = out["vir"]
+    p_box = (2 * k.sum() + w.sum()) / (dim * L.prod())
+    pd = cfg["pore"]
+    d = out["pos"] - np.array(pd["center"][:dim])
+    if pd["kind"] == "cylinder":
+        ax = pd["axis"]
+        a1, a2 = (ax + 1) % 3, (ax + 2) % 3
+        inside = (np.abs(d[:, ax]) < 0.5 * pd["length"]) & (d[:, a1] ** 2 + d[:, a2] ** 2 < pd["r0"] ** 2)
+        vol = np.pi * pd["r0"] ** 2 * pd["length"]
+    else:
+        ax = pd["axis"]
+        inside = (np.abs(d[:, ax]) < 0.5 * pd["width"]) & (np.abs(d[:, 1 - ax]) < 0.5 * pd["length"])
+        vol = pd["width"] * pd["length"]
+    return p_box, (2 * k[inside].sum() + w[inside].sum()) / (dim * vol), int(inside.sum())
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_virial_pressure_box_and_pore(algo):
+    # NEXT-2 (PAPER.md:47-51): P = (2K + W) / (d V) over the box and over the particles inside the pore volume
+    for cfg, n in ((I.config4(12), 60), (I.config1(n_vapor=4096), 40)):
+        ref = O.run(cfg, n, cells=True)
+        p_box, p_pore, n_pore = _oracle_pressure(cfg, ref)
+        sim = make_sim(cfg, algo)
+        sim.step(n)
+        pr = sim.pressure()
+        assert pr["n_pore"] == n_pore and pr["step"] == n
+        assert abs(pr["P_box"] - p_box) <= 1e-8 * abs(p_box)
+        assert abs(pr["P_pore"] - p_pore) <= 1e-8 * max(abs(p_pore), abs(p_box))
+        sim.close()
+    # ideal gas limit: no forces -> P V = N T exactly (T = 2K / (d N))
+    cfg = dict(I.config4(10), eps=0.0, eps_w=0.0)
+    sim = make_sim(cfg, algo)
+    pr, en = sim.pressure(), sim.energy()
+    assert abs(pr["P_box"] * pr["V_box"] - 2 * en["K"] / 3) < 1e-9 * en["K"]
+    sim.close()
+    nopore = I.small_case(3, 50, (10.0, 10.0, 10.0), (0, 0, 1), seed=3)
+    sim = make_sim(nopore, algo)
+    with pytest.raises(md.MDError) as e:
+        sim.pressure()
+    assert e.value.code == md.MD_ERR_UNSUPPORTED
+    sim.close()
