@@ -48,7 +48,7 @@ def measure(cfg, algo, precision, n_steps, torch, md, peaks):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--configs", default="0,1,2,3,4")
+    ap.add_argument("--configs", default="0,1,2,3,4,5", help="0-4: BASELINE.json configs; 5: the paper's problem sizes")
     ap.add_argument("--max-log2n", type=int, default=20)
     ap.add_argument("--json", default="")
     args = ap.parse_args()
@@ -86,6 +86,11 @@ def main():
         for shape in ("cone", "inkbottle", "slit"):
             cfg = I.config3(shape)
             for algo in ("cells", "verlet"):
+                add(cfg, algo, 64, 2000)
+    if 5 in want:      # the paper's own problem sizes, context for its Tables 1 and 4
+        for dim in (2, 3):
+            cfg = I.paper_size(dim)
+            for algo in ("allpairs", "cells", "verlet"):
                 add(cfg, algo, 64, 2000)
     if 4 in want:
         for log2n in range(10, args.max_log2n + 1, 2):
