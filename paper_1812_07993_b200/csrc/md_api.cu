@@ -463,6 +463,16 @@ struct Sim : md_sim {
             out->launches[3] = n > 0 ? 1 : 0;
             out->steps = n; out->rebuilds = rebuilds_seen - r0;
             step_no += n;
+            if (getenv("MD_DEBUG_BUILD") && rebuilds_seen > r0 && out->rebuilds == 0) {
+                // only meaningful right after a rebuild (positions still wrapped, cell order current): n = 0 calls
+            }
+            if (getenv("MD_DEBUG_BUILD")) {
+                for (int k = 0; k < 3; ++k) {
+                    if (dim == 3) md::k_dbg_build<T, 9><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur);
+                    else md::k_dbg_build<T, 3><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur);
+                }
+                CK(cudaStreamSynchronize(stream));
+            }
             return MD_OK;
         }
         for (long long k = 0; k < n; ++k) {

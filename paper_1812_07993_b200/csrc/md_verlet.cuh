@@ -507,6 +507,14 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
     if (gtid == 0) { v.flags[VF_CUR] = c; v.flags[VF_CURV] = cv; v.times[3] += now_ns() - t0; }
 }
 
+// Diagnostics only (MD_DEBUG_BUILD=1 in md_profile_step): the list-build phase as a kernel of its own, so that ncu can
+// attribute its stalls.  It rebuilds the list from the current cell order, which is what the list already holds.
+template <typename T, int ROWS>
+__global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_build(Params<T> p, Verlet<T> v, int c)
+{
+    phase_build<T, ROWS>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+
 // a5 energy pass over the neighbour list (ordinary launch; the host passes the buffer parities).
 template <typename T>
 __global__ void __launch_bounds__(VL_THREADS) k_verlet_energy(Params<T> p, Verlet<T> v, int c, EnergyOut eo)
