@@ -128,6 +128,14 @@ int md_energy(md_sim*, md_energy_out* out);
  * MD_ERR_UNSUPPORTED if no monitored pore kind was given (pressure_box is still filled). */
 int md_pressure(md_sim*, md_pressure_out* out);
 
+/* Vapor density profiles about the pore given to md_create, histogrammed on the device at the current step
+ * (NEXT-4; the long-run comparison of north_star).  axial[n_axial]: particle counts in equal slabs of the whole box
+ * length along pore.axis.  radial[n_radial]: counts in equal-width shells 0 <= rho < r_max about the axis line through
+ * pore.center, restricted to |along - center| < length/2 (3D cylinder; in 2D rho = |r[axis] - center[axis]| with axis
+ * the wall normal and the restriction along the other dimension).  Host int64 arrays, either may be NULL.
+ * MD_ERR_UNSUPPORTED without a monitored pore kind. */
+int md_density_profile(md_sim*, int n_axial, long long* axial, int n_radial, double r_max, long long* radial);
+
 /* Like md_step but synchronous, one launch at a time with CUDA events around every kernel. */
 int md_profile_step(md_sim*, long long n_steps, md_kernel_times* out);
 

@@ -127,6 +127,7 @@ struct Layout {
     double *stage0, *stage1, *wstage;
     int *nbr, *ncnt, *vflags;   // VERLET: neighbour list, counts, flags
     unsigned long long *vtimes, *vbar;
+    unsigned long long* hist;   // density-profile bins
     double* vksum;              // VERLET thermostat: rotating kinetic-energy accumulators
     md::Vec4<T> *jv, *jw;       // ALLPAIRS: j lists (entries + ghosts) of the dot-product kernels
     int *jv_id, *jw_id;         // fp32: original index of every entry
@@ -180,6 +181,7 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.vtimes = c.take<unsigned long long>(8 + 8192);
     l.vbar = c.take<unsigned long long>(2);
     l.vksum = c.take<double>(4);
+    l.hist = c.take<unsigned long long>(md::HIST_MAX_BINS);
     l.stage0 = c.take<double>(n * dim);
     l.stage1 = c.take<double>(n * dim);
     l.wstage = c.take<double>(m * dim);
@@ -199,6 +201,7 @@ struct md_sim {
     virtual int pair_tests(long long* tests) = 0;
     virtual void info(int* algo, int nc[3], int* kps) const = 0;
     virtual int pressure(md_pressure_out* out) = 0;
+    virtual int density(int n_axial, long long* axial, int n_radial, double r_max, long long* radial) = 0;
     md_pore pore = {};
     md_box box = {};
 };
@@ -604,6 +607,42 @@ struct Sim : md_sim {
         return MD_OK;
     }
 
+    bool pore_region(md::PoreRegion& g) const
+    {
+        g = md::PoreRegion{};
+        if (pore.kind == MD_PORE_SLIT && dim == 2 && (pore.axis == 0 || pore.axis == 1)) g.kind = 1;
+        else if (pore.kind == MD_PORE_CYLINDER && dim == 3 && pore.axis >= 0 && pore.axis < 3) g.kind = 2;
+        g.axis = pore.axis;
+        for (int k = 0; k < 3; ++k) g.c[k] = pore.center[k];
+        g.half_len = 0.5 * pore.length; g.r0sq = pore.r0 * pore.r0; g.half_width = 0.5 * pore.width;
+        return g.kind != 0;
+    }
+
+    int density(int n_axial, long long* axial, int n_radial, double r_max, long long* radial) override
+    {
+        if (n_axial < 0 || n_radial < 0 || n_axial + n_radial > md::HIST_MAX_BINS || (n_radial > 0 && !(r_max > 0)) ||
+            (n_axial > 0 && !axial) || (n_radial > 0 && !radial)) { err = "bad histogram arguments"; return MD_ERR_INVALID_ARG; }
+        md::PoreRegion g;
+        if (!pore_region(g)) { err = "no monitored pore region (MD_PORE_SLIT in 2D or MD_PORE_CYLINDER in 3D)"; return MD_ERR_UNSUPPORTED; }
+        int rc = check_err_flag();
+        if (rc) return rc;
+        const int nb = n_axial + n_radial;
+        if (nb == 0) return MD_OK;
+        // profiles run along the pore: the cylinder axis, or (2D slit) the dimension the slit extends in
+        const int along = g.kind == 2 ? g.axis : 1 - g.axis;
+        unsigned long long* d_out = l.hist;
+        CK(cudaMemsetAsync(d_out, 0, sizeof(unsigned long long) * nb, stream));
+        md::k_density_profile<T><<<std::min(blocks(256), 296), 256, 0, stream>>>(p, view(), g, along, box.len[along], n_axial,
+                                                                              n_radial, r_max > 0 ? r_max : 1.0, d_out);
+        std::vector<unsigned long long> h((size_t)nb);
+        CK(cudaMemcpyAsync(h.data(), d_out, sizeof(unsigned long long) * nb, cudaMemcpyDeviceToHost, stream));
+        CK(cudaStreamSynchronize(stream));
+        CK(cudaGetLastError());
+        for (int k = 0; k < n_axial; ++k) axial[k] = (long long)h[k];
+        for (int k = 0; k < n_radial; ++k) radial[k] = (long long)h[n_axial + k];
+        return MD_OK;
+    }
+
     int pressure(md_pressure_out* out) override
     {
         if (!out) { err = "out is NULL"; return MD_ERR_INVALID_ARG; }
@@ -928,6 +967,10 @@ int md_energy(md_sim* s, md_energy_out* out) { return s ? s->energy(out) : MD_ER
 int md_profile_step(md_sim* s, long long n, md_kernel_times* out) { return s ? s->profile(n, out) : MD_ERR_INVALID_ARG; }
 int md_pair_tests(md_sim* s, long long* t) { return s ? s->pair_tests(t) : MD_ERR_INVALID_ARG; }
 int md_pressure(md_sim* s, md_pressure_out* out) { return s ? s->pressure(out) : MD_ERR_INVALID_ARG; }
+int md_density_profile(md_sim* s, int na, long long* axial, int nr, double r_max, long long* radial)
+{
+    return s ? s->density(na, axial, nr, r_max, radial) : MD_ERR_INVALID_ARG;
+}
 int md_info(const md_sim* s, int* algo, int nc[3], int* kps)
 {
     if (!s) return MD_ERR_INVALID_ARG;

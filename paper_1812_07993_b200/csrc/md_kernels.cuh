@@ -639,6 +639,48 @@ __global__ void __launch_bounds__(RED_THREADS) k_pressure_partial(Params<T> p, S
     block_sum6(v, part + blockIdx.x, gridDim.x);
 }
 
+// NEXT-4: density profiles about the pore, integer histograms (shared-memory bins, then global atomics).
+constexpr int HIST_MAX_BINS = 1024;
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_density_profile(Params<T> p, State<T> s, PoreRegion g, int along_dim, double box_len,
+                                                         int n_axial, int n_radial, double r_max,
+                                                         unsigned long long* __restrict__ out)
+{
+    __shared__ unsigned int bins[HIST_MAX_BINS];
+    const int nb = n_axial + n_radial;
+    for (int k = threadIdx.x; k < nb; k += blockDim.x) bins[k] = 0;
+    __syncthreads();
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < p.nv; i += gridDim.x * blockDim.x) {
+        Vec4<T> ri = s.r[i];
+        T dummy = T(0);
+        int err = 0;
+        boundary(ri.x, dummy, p.L[0], p.bc[0] == BC_PERIODIC ? BC_PERIODIC : BC_NONE, &err);
+        boundary(ri.y, dummy, p.L[1], p.bc[1] == BC_PERIODIC ? BC_PERIODIC : BC_NONE, &err);
+        boundary(ri.z, dummy, p.L[2], p.bc[2] == BC_PERIODIC ? BC_PERIODIC : BC_NONE, &err);
+        const double x[3] = {(double)ri.x, (double)ri.y, (double)ri.z};
+        if (n_axial > 0) {
+            const int b = min(max((int)floor(x[along_dim] / box_len * n_axial), 0), n_axial - 1);
+            atomicAdd(&bins[b], 1u);
+        }
+        if (n_radial > 0) {
+            const double d[3] = {x[0] - g.c[0], x[1] - g.c[1], x[2] - g.c[2]};
+            double rho;
+            bool in;
+            if (g.kind == 1) { rho = fabs(d[g.axis]); in = fabs(d[1 - g.axis]) < g.half_len; }
+            else {
+                const int a1 = (g.axis + 1) % 3, a2 = (g.axis + 2) % 3;
+                rho = sqrt(d[a1] * d[a1] + d[a2] * d[a2]); in = fabs(d[g.axis]) < g.half_len;
+            }
+            const int b = (int)floor(rho / r_max * n_radial);
+            if (in && b >= 0 && b < n_radial) atomicAdd(&bins[n_axial + b], 1u);
+        }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < nb; k += blockDim.x)
+        if (bins[k]) atomicAdd(&out[k], (unsigned long long)bins[k]);
+}
+
 // ---------------------------------------------------------------------------
 // F4, Berendsen thermostat for the multi-kernel paths: block partial sums of K, then every
 // block re-sums the partials in the same fixed order, forms lambda and rescales its velocities.

@@ -20,7 +20,7 @@ MD_BC_PERIODIC, MD_BC_REFLECT = 0, 1
 MD_FORCE_AUTO, MD_FORCE_ALLPAIRS, MD_FORCE_CELLS, MD_FORCE_VERLET = 0, 1, 2, 3
 _ALGO = {"auto": MD_FORCE_AUTO, "allpairs": MD_FORCE_ALLPAIRS, "cells": MD_FORCE_CELLS, "verlet": MD_FORCE_VERLET}
 
-EXPORTS = ["md_workspace_bytes", "md_create", "md_step", "md_get_state", "md_energy", "md_pressure", "md_profile_step",
+EXPORTS = ["md_workspace_bytes", "md_create", "md_step", "md_get_state", "md_energy", "md_pressure", "md_density_profile", "md_profile_step",
            "md_pair_tests", "md_info", "md_measure_peaks", "md_destroy", "md_last_error"]
 
 
@@ -97,6 +97,9 @@ def load_library():
         lib.md_energy.argtypes = [C.c_void_p, C.POINTER(md_energy_out)]
         lib.md_pressure.restype = C.c_int
         lib.md_pressure.argtypes = [C.c_void_p, C.POINTER(md_pressure_out)]
+        lib.md_density_profile.restype = C.c_int
+        lib.md_density_profile.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong), C.c_int, C.c_double,
+                                           C.POINTER(C.c_longlong)]
         lib.md_profile_step.restype = C.c_int
         lib.md_profile_step.argtypes = [C.c_void_p, C.c_longlong, C.POINTER(md_kernel_times)]
         lib.md_pair_tests.restype = C.c_int
@@ -207,6 +210,15 @@ class Simulation:
         self._check(self._lib.md_pressure(self._h, C.byref(o)))
         return dict(P_box=o.pressure_box, V_box=o.volume_box, P_pore=o.pressure_pore, V_pore=o.volume_pore,
                     K_pore=o.kinetic_pore, W_pore=o.virial_pore, n_pore=o.n_pore, step=o.step)
+
+    def density_profile(self, n_axial: int, n_radial: int, r_max: float):
+        """(axial counts, radial counts) about the pore of cfg["pore"], histogrammed on the device."""
+        ax = np.zeros(max(n_axial, 1), dtype=np.int64)
+        ra = np.zeros(max(n_radial, 1), dtype=np.int64)
+        lp = C.POINTER(C.c_longlong)
+        self._check(self._lib.md_density_profile(self._h, int(n_axial), ax.ctypes.data_as(lp), int(n_radial), float(r_max),
+                                                 ra.ctypes.data_as(lp)))
+        return ax[:n_axial], ra[:n_radial]
 
     def profile_step(self, n_steps: int):
         t = md_kernel_times()

@@ -419,3 +419,28 @@ def test_virial_pressure_box_and_pore(algo):
         sim.pressure()
     assert e.value.code == md.MD_ERR_UNSUPPORTED
     sim.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_device_density_profile_is_bit_exact(algo):
+    # NEXT-4: integer work -> bit-exact against the same histogram taken on the host from md_get_state
+    for cfg, n_ax, n_r, r_max in ((I.config4(12), 11, 10, 10.0), (I.config1(n_vapor=4096), 16, 8, 12.0)):
+        sim = make_sim(cfg, algo)
+        sim.step(37)
+        pos = sim.get_state(vel=False, force=False, pe=False)["pos"]
+        ax, ra = sim.density_profile(n_ax, n_r, r_max)
+        pd, dim = cfg["pore"], cfg["dim"]
+        L = np.array(cfg["box_len"][:dim])
+        d = pos - np.array(pd["center"][:dim])
+        if pd["kind"] == "cylinder":
+            along, a1, a2 = pd["axis"], (pd["axis"] + 1) % 3, (pd["axis"] + 2) % 3
+            rho = np.sqrt(d[:, a1] ** 2 + d[:, a2] ** 2)
+        else:
+            along = 1 - pd["axis"]
+            rho = np.abs(d[:, pd["axis"]])
+        inside = np.abs(d[:, along]) < 0.5 * pd["length"]
+        ax_ref = np.bincount(np.clip(np.floor(pos[:, along] / L[along] * n_ax).astype(int), 0, n_ax - 1), minlength=n_ax)
+        b = np.floor(rho / r_max * n_r).astype(int)
+        ra_ref = np.bincount(b[inside & (b < n_r)], minlength=n_r)
+        assert ax.sum() == cfg["n_vapor"] and np.array_equal(ax, ax_ref) and np.array_equal(ra, ra_ref)
+        sim.close()
