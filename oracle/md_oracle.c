@@ -39,6 +39,11 @@ typedef struct {
     int shift_energy;   /* 1: u(r) - u(r_c) inside the cut-off (reading A2) */
     double dt, mass;
     double tau_b, t_target; /* Berendsen thermostat F4: rise time (<= 0: off), T_0 */
+    /* NEXT-3, the paper's own pore: an axis-aligned box whose faces reflect from both sides, except the face at
+     * +prism_axis, which is open (2D: square pore with three closed sides; 3D: prism with five
+     * isolated walls and one open).  prism = 0: none. */
+    int prism, prism_axis;
+    double prism_c[3], prism_h[3]; /* centre, half sizes */
 } orc_params;
 
 /* ---- c.1 definitions ------------------------------------------------- */
@@ -293,9 +298,30 @@ int orc_run(const orc_params *p, int use_cells, long nv, double *pos, double *ve
         if (step == n_steps) break;
         int bad = 0;
         for (long i = 0; i < nv; ++i) {
+            double ro[3] = {0, 0, 0}, rn[3] = {0, 0, 0}, vh[3] = {0, 0, 0};
             for (int a = 0; a < dim; ++a) {
-                double v = vel[i * dim + a] + hk * f[i * dim + a];      /* F2: v(t + dt/2) */
-                double r = pos[i * dim + a] + p->dt * v;                /* F2: r(t + dt)   */
+                ro[a] = pos[i * dim + a];
+                vh[a] = vel[i * dim + a] + hk * f[i * dim + a];             /* F2: v(t + dt/2) */
+                rn[a] = ro[a] + p->dt * vh[a];                              /* F2: r(t + dt)   */
+            }
+            if (p->prism) {
+                /* geometric pore walls: one specular bounce per closed face whose rectangle the straight path
+                 * r(t) -> r(t + dt) crosses; faces are visited in the order -x, +x, -y, +y, (-z, +z) */
+                for (int a = 0; a < dim; ++a)
+                    for (int sgn = -1; sgn <= 1; sgn += 2) {
+                        if (a == p->prism_axis && sgn == 1) continue;             /* the open face */
+                        const double w = p->prism_c[a] + sgn * p->prism_h[a];
+                        if ((ro[a] - w) * (rn[a] - w) < 0.0) {
+                            const double t = (w - ro[a]) / (rn[a] - ro[a]);
+                            int inside = 1;
+                            for (int b = 0; b < dim; ++b)
+                                if (b != a && fabs(ro[b] + t * (rn[b] - ro[b]) - p->prism_c[b]) > p->prism_h[b]) inside = 0;
+                            if (inside) { rn[a] = 2.0 * w - rn[a]; vh[a] = -vh[a]; }
+                        }
+                    }
+            }
+            for (int a = 0; a < dim; ++a) {
+                double v = vh[a], r = rn[a];
                 const double L = p->L[a];
                 if (p->bc[a] == 0) {                                    /* periodic wrap into [0, L) */
                     r = r - L * floor(r / L);

@@ -17,7 +17,8 @@ class OrcParams(C.Structure):
     _fields_ = [("dim", C.c_int), ("L", C.c_double * 3), ("bc", C.c_int * 3), ("eps", C.c_double),
                 ("sigma", C.c_double), ("eps_w", C.c_double), ("sigma_w", C.c_double), ("r_cut", C.c_double),
                 ("shift_energy", C.c_int), ("dt", C.c_double), ("mass", C.c_double), ("tau_b", C.c_double),
-                ("t_target", C.c_double)]
+                ("t_target", C.c_double), ("prism", C.c_int), ("prism_axis", C.c_int), ("prism_c", C.c_double * 3),
+                ("prism_h", C.c_double * 3)]
 
 
 _lib = None
@@ -55,6 +56,12 @@ def params(cfg) -> OrcParams:
     p.shift_energy = int(cfg.get("shift_energy", 1))
     p.dt, p.mass = float(cfg["dt"]), float(cfg["mass"])
     p.tau_b, p.t_target = float(cfg.get("tau_b", 0.0)), float(cfg.get("t_target", 1.0))
+    pd = cfg.get("pore")
+    if pd and pd["kind"] == "prism":         # geometric walls: centre, length along axis, width across
+        p.prism, p.prism_axis = 1, int(pd["axis"])
+        for a in range(p.dim):
+            p.prism_c[a] = float(pd["center"][a])
+            p.prism_h[a] = 0.5 * float(pd["length"] if a == p.prism_axis else pd["width"])
     return p
 
 

@@ -334,3 +334,47 @@ def test_berendsen_thermostat_closed_forms():
     hh = O.run(cold, 300, history=True)["hist"]
     tt = 2.0 * hh[:, 0] / (3 * 150)
     assert tt[0] > 0.9 and np.abs(tt[50:] - 0.3).max() < 0.06
+
+
+def _prism_cfg(dim, pos, vel, axis=0, center=None, length=6.0, width=4.0, box=20.0, dt=0.01):
+    cfg = base_cfg(dim, box=(box,) * dim, bc=(0,) * dim, pos=np.array(pos, dtype=float), vel=np.array(vel, dtype=float), dt=dt)
+    cfg["eps"] = cfg["eps_w"] = 0.0
+    cfg["pore"] = dict(kind="prism", axis=axis, center=center or [10.0] * dim, length=length, width=width)
+    return cfg
+
+
+def test_geometric_prism_pore_free_flight():
+    # NEXT-3: the paper's pore: closed faces reflect from both sides, the +axis face is open.
+    # 2D pore [7, 13] x [8, 12], open at x = 13.  Free flight => closed forms.
+    # (a) bouncing between the side walls y = 8 and y = 12: triangular wave, |v| unchanged, x untouched
+    cfg = _prism_cfg(2, [[9.0, 10.0]], [[0.0, 3.0]])
+    out = O.run(cfg, 1000)
+    t = 1000 * 0.01
+    y = (10.0 - 8.0 + 3.0 * t) % 8.0
+    y = 8.0 + (y if y <= 4.0 else 8.0 - y)
+    assert abs(out["pos"][0, 1] - y) < 1e-10 and abs(out["pos"][0, 0] - 9.0) < 1e-12 and abs(abs(out["vel"][0, 1]) - 3.0) < 1e-14
+    # (b) towards the closed end x = 7: comes back and leaves through the open mouth at x = 13, then keeps going
+    cfg = _prism_cfg(2, [[9.0, 10.0]], [[-2.0, 0.0]])
+    out = O.run(cfg, 250)                                   # 2.5 time units: 1 to the wall, 1.5 back => x = 7 + 3 = 10
+    assert abs(out["pos"][0, 0] - 10.0) < 1e-10 and out["vel"][0, 0] == 2.0
+    out = O.run(cfg, 500)
+    assert abs(out["pos"][0, 0] - 15.0) < 1e-10            # x = 7 + 2 * 4: no wall at the mouth (x = 13)
+    # (c) from outside: hits the side wall y = 12 from above and bounces back; beside the pore it flies on
+    cfg = _prism_cfg(2, [[10.0, 14.0], [4.0, 14.0]], [[0.0, -1.0], [0.0, -1.0]])
+    out = O.run(cfg, 400)
+    assert abs(out["pos"][0, 1] - 14.0) < 1e-10 and out["vel"][0, 1] == 1.0     # 2 down, 2 back up
+    assert abs(out["pos"][1, 1] - 10.0) < 1e-10 and out["vel"][1, 1] == -1.0    # x = 4 is outside [7, 13]
+    # (d) enters through the mouth from the right and is turned round at the closed end
+    cfg = _prism_cfg(2, [[16.0, 10.5]], [[-3.0, 0.0]])
+    out = O.run(cfg, 500)                                   # 15 units of path: 9 to x = 7, 6 back => x = 13
+    assert abs(out["pos"][0, 0] - 13.0) < 1e-10 and out["vel"][0, 0] == 3.0
+    # (e) 3D prism along z, open at +z: corner bounce flips two components in one step
+    cfg = _prism_cfg(3, [[11.9, 11.9, 10.0]], [[2.0, 2.0, 0.0]], axis=2, dt=0.1)
+    out = O.run(cfg, 1)
+    assert np.allclose(out["pos"][0], [11.9, 11.9, 10.0], atol=1e-12) and np.array_equal(out["vel"][0], [-2.0, -2.0, 0.0])
+    # (f) with interactions on, the walls do no work: energy drift stays at the NVE level
+    lj = I.small_case(2, 30, (20.0, 20.0), (0, 0), seed=5, min_sep=1.0)
+    lj["pore"] = dict(kind="prism", axis=0, center=[10.0, 10.0], length=8.0, width=6.0)
+    h = O.run(lj, 2000, history=True)["hist"]
+    e = h[:, 0] + h[:, 1] + h[:, 2]
+    assert np.abs(e - e[0]).max() < 2e-3 * h[0, 0]
