@@ -55,7 +55,10 @@ typedef struct { int dim; double len[3]; int bc[3]; } md_box;
 /* Pore region.  The hot path sees wall PARTICLES, not shapes; the descriptor only selects the volume md_pressure
  * monitors: MD_PORE_CYLINDER (3D): distance from the axis line through `center` along dimension `axis` < r0 and
  * |along - center[axis]| < length/2; MD_PORE_SLIT (2D): |r[axis] - center[axis]| < width/2 (axis = wall normal) and
- * |r[1-axis] - center[1-axis]| < length/2.  Other kinds are stored but not monitored. */
+ * |r[1-axis] - center[1-axis]| < length/2.  MD_PORE_PRISM switches on GEOMETRIC walls (the paper's own pore,
+ * PAPER.md:115-121, :186): the axis-aligned box of size `length` along `axis` and `width` across, centred at `center`,
+ * reflects particles specularly from both sides of every face except the open one at +axis; it must lie at least one
+ * length unit inside the simulation box.  Other kinds are stored but neither monitored nor active. */
 typedef struct { int kind, axis; double center[3], length, r0, r1, neck_len, width; } md_pore;
 
 /* 12-6 Lennard-Jones: u(r) = 4 eps [(sigma/r)^12 - (sigma/r)^6] for r < r_cut, else 0 (strict <);

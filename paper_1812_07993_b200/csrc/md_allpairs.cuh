@@ -66,7 +66,12 @@ __global__ void __launch_bounds__(256) k_ap_kick_drift_list(Params<double> p, St
         double vx = s.vx[i] + p.hk * f.fx[i];
         double vy = s.vy[i] + p.hk * f.fy[i];
         double vz = s.vz[i] + p.hk * f.fz[i];
-        ri.x += p.dt * vx; ri.y += p.dt * vy; ri.z += p.dt * vz;
+        {
+            const double ro[3] = {ri.x, ri.y, ri.z};
+            double rn[3] = {ri.x + p.dt * vx, ri.y + p.dt * vy, ri.z + p.dt * vz}, vh[3] = {vx, vy, vz};
+            if (p.prism) prism_reflect(p, ro, rn, vh);
+            ri.x = rn[0]; ri.y = rn[1]; ri.z = rn[2]; vx = vh[0]; vy = vh[1]; vz = vh[2];
+        }
         boundary(ri.x, vx, p.L[0], p.bc[0], err);
         boundary(ri.y, vy, p.L[1], p.bc[1], err);
         boundary(ri.z, vz, p.L[2], p.bc[2], err);
@@ -262,7 +267,12 @@ __global__ void __launch_bounds__(256) k_apf_kick_drift_list(Params<float> p, St
         float vx = s.vx[i] + p.hk * f.fx[i];
         float vy = s.vy[i] + p.hk * f.fy[i];
         float vz = s.vz[i] + p.hk * f.fz[i];
-        ri.x += p.dt * vx; ri.y += p.dt * vy; ri.z += p.dt * vz;
+        {
+            const float ro[3] = {ri.x, ri.y, ri.z};
+            float rn[3] = {ri.x + p.dt * vx, ri.y + p.dt * vy, ri.z + p.dt * vz}, vh[3] = {vx, vy, vz};
+            if (p.prism) prism_reflect(p, ro, rn, vh);
+            ri.x = rn[0]; ri.y = rn[1]; ri.z = rn[2]; vx = vh[0]; vy = vh[1]; vz = vh[2];
+        }
         boundary(ri.x, vx, p.L[0], p.bc[0], err);
         boundary(ri.y, vy, p.L[1], p.bc[1], err);
         boundary(ri.z, vz, p.L[2], p.bc[2], err);

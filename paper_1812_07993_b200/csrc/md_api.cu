@@ -795,7 +795,7 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
 }
 
 template <typename T>
-int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o, long long nv, const double* pos,
+int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& lj, const md_opts& o, long long nv, const double* pos,
              const double* vel, long long nw, const double* wall, void* ws, size_t ws_bytes, void* stream,
              const GridSpec& g, int algo)
 {
@@ -832,6 +832,13 @@ int create_t(md_sim** out, const md_box& box, const md_lj& lj, const md_opts& o,
     p.sig2_vw = (T)(lj.sigma_w * lj.sigma_w); p.e24_vw = (T)(24.0 * lj.eps_w); p.e4_vw = (T)(4.0 * lj.eps_w);
     p.uc_vw = (T)ucut(lj.eps_w, lj.sigma_w);
     p.dt = (T)o.dt; p.hk = (T)(o.dt / (2.0 * o.mass)); p.mass = o.mass;
+    p.prism = pore && pore->kind == MD_PORE_PRISM;
+    p.prism_axis = p.prism ? pore->axis : 0;
+    for (int a = 0; a < 3; ++a) {
+        const bool on = p.prism && a < box.dim;
+        p.prism_c[a] = on ? (T)pore->center[a] : T(0);
+        p.prism_h[a] = on ? (T)(0.5 * (a == pore->axis ? pore->length : pore->width)) : T(1);
+    }
     p.thermo_rate = o.tau_b > 0 ? o.dt / o.tau_b : 0.0; p.t_target = o.t_target; p.dof = (double)box.dim * (double)nv;
     if (algo == MD_FORCE_ALLPAIRS) {
         // dot-product kernel: needs at most one periodic image per dimension inside r_c + margin of a face
@@ -945,6 +952,20 @@ int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj*
     int algo = pick_algo(*box, *lj, *o, nv, nw);
     if (algo < 0) { g_create_error = "cell list needs >= 3 cells in every periodic dimension"; return MD_ERR_UNSUPPORTED; }
     GridSpec g = grid_for(*box, *lj, *o, algo);
+    if (pore && pore->kind == MD_PORE_PRISM) {
+        // geometric walls must sit inside the box with a margin (VERLET keeps periodic coordinates unwrapped by < skin)
+        if (pore->axis < 0 || pore->axis >= dim || !(pore->length > 0) || !(pore->width > 0)) {
+            g_create_error = "prism pore needs 0 <= axis < dim, length > 0, width > 0";
+            return MD_ERR_INVALID_ARG;
+        }
+        for (int a = 0; a < dim; ++a) {
+            const double h = 0.5 * (a == pore->axis ? pore->length : pore->width);
+            if (!(pore->center[a] - h >= 1.0) || !(pore->center[a] + h <= box->len[a] - 1.0)) {
+                g_create_error = "prism pore must lie at least 1 length unit inside the box";
+                return MD_ERR_INVALID_ARG;
+            }
+        }
+    }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         cudaGetLastError();
@@ -952,8 +973,8 @@ int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj*
         return MD_ERR_CUDA;
     }
     int rc = o->precision == 64
-                 ? create_t<double>(out, *box, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo)
-                 : create_t<float>(out, *box, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo);
+                 ? create_t<double>(out, *box, pore, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo)
+                 : create_t<float>(out, *box, pore, *lj, *o, nv, pos, vel, nw, wall, ws, ws_bytes, stream, g, algo);
     if (rc == MD_OK && pore) (*out)->pore = *pore;
     return rc;
 }

@@ -24,6 +24,8 @@ struct Params {
     T dt, hk; // hk = dt / (2 m)
     double mass;
     double thermo_rate, t_target, dof;   // Berendsen F4: dt / tau_B (0 = off), T_0, dim * n_vapor
+    int prism, prism_axis;               // NEXT-3: geometric pore walls (closed faces reflect, +axis face open)
+    T prism_c[3], prism_h[3];            // centre, half sizes (unused dimensions: c = 0, h = 1)
 };
 
 // Packed position: one 4-wide vector load per neighbour (w is spare; the cell path keeps the
@@ -100,6 +102,28 @@ __device__ __forceinline__ void boundary(T& r, T& v, T L, int bc, int* err)
     }
 }
 
+// Geometric pore walls (the paper's own pore): one specular bounce per closed face whose
+// rectangle the straight path r(t) -> r(t + dt) crosses, faces visited in the order -x, +x, -y, +y, -z, +z.
+template <typename T>
+__device__ __forceinline__ void prism_reflect(const Params<T>& p, const T (&ro)[3], T (&rn)[3], T (&vh)[3])
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int sgn = -1; sgn <= 1; sgn += 2) {
+            if (a == p.prism_axis && sgn == 1) continue;                 // the open face
+            const T w = p.prism_c[a] + T(sgn) * p.prism_h[a];
+            if ((ro[a] - w) * (rn[a] - w) < T(0)) {
+                const T t = (w - ro[a]) / (rn[a] - ro[a]);
+                bool inside = true;
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+                    if (b != a && fabs(ro[b] + t * (rn[b] - ro[b]) - p.prism_c[b]) > p.prism_h[b]) inside = false;
+                if (inside) { rn[a] = T(2) * w - rn[a]; vh[a] = -vh[a]; }
+            }
+        }
+}
+
 template <typename T, bool MOVE, bool BIN>
 __global__ void __launch_bounds__(256) k_kick_drift_bin(Params<T> p, State<T> s, Force<T> f, int* __restrict__ count,
                                                         int* __restrict__ cell, int* __restrict__ slot,
@@ -116,6 +140,12 @@ __global__ void __launch_bounds__(256) k_kick_drift_bin(Params<T> p, State<T> s,
         x = x + p.dt * vx;
         y = y + p.dt * vy;
         z = z + p.dt * vz;
+        if (p.prism) {
+            const T ro[3] = {ri.x, ri.y, ri.z};
+            T rn[3] = {x, y, z}, vh[3] = {vx, vy, vz};
+            prism_reflect(p, ro, rn, vh);
+            x = rn[0]; y = rn[1]; z = rn[2]; vx = vh[0]; vy = vh[1]; vz = vh[2];
+        }
         boundary(x, vx, p.L[0], p.bc[0], err);
         boundary(y, vy, p.L[1], p.bc[1], err);
         boundary(z, vz, p.L[2], p.bc[2], err);

@@ -209,6 +209,12 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             const T sx = p.dt * vx, sy = p.dt * vy, sz = p.dt * vz;
             Vec4<T> rn;
             rn.x = ri.x + sx; rn.y = ri.y + sy; rn.z = ri.z + sz;
+            if (p.prism) {
+                const T ro[3] = {ri.x, ri.y, ri.z};
+                T rr[3] = {rn.x, rn.y, rn.z}, vh[3] = {vx, vy, vz};
+                prism_reflect(p, ro, rr, vh);
+                rn.x = rr[0]; rn.y = rr[1]; rn.z = rr[2]; vx = vh[0]; vy = vh[1]; vz = vh[2];
+            }
             // periodic dimensions are left unwrapped until the next rebuild; reflection is immediate
             int* err = v.flags + VF_ESCAPE;
             if (p.bc[0] == BC_REFLECT) boundary(rn.x, vx, p.L[0], BC_REFLECT, err);

@@ -264,6 +264,44 @@ def paper_size(dim, seed=BASE_SEED + 9):
                    "allpairs")
 
 
+def paper_geometry(dim, seed=BASE_SEED + 20):
+    """The paper's own runs in reduced units (NEXT-3; readings A16 of DESIGN.md): a pore with GEOMETRIC reflecting walls
+    (no wall particles), open at +x into an outer space with periodic boundaries, pore : outside density 5 : 1.
+    2D: square pore 1 um x 1 um with 420 molecules, outer space 1764, 35 C.
+    3D: prism 500 x 50 x 50 nm with 1000 molecules, outer space 1800 with 9x the volume, 25 C.
+    dt = 0.016 ps = 0.00959 tau.  The gas is so dilute (4e-5 sigma^-2) that a cell grid would hold ~1e7 empty cells:
+    the all-pairs kernel is the one to use, as in the paper."""
+    from . import units
+
+    rng = SplitMix64(seed + dim)
+    if dim == 2:
+        l = units.length_reduced(1.0e-6)
+        n_in, n_out, t_star = 420, 1764, units.temperature_reduced(35.0)
+        box = (4.0 * l + 4.0, 7.0 * l)                              # pore + k = 3 pore widths of outer space, 2k + 1 tall
+        lo, hi = np.array([2.0, 3.0 * l]), np.array([2.0 + l, 4.0 * l])
+    else:
+        lx, lw = units.length_reduced(500e-9), units.length_reduced(50e-9)
+        n_in, n_out, t_star = 1000, 1800, units.temperature_reduced(25.0)
+        box = (10.0 * lx + 4.0, lw + 4.0, lw + 4.0)                 # outer space: same cross-section, 9x the length
+        lo, hi = np.array([2.0, 2.0, 2.0]), np.array([2.0 + lx, 2.0 + lw, 2.0 + lw])
+    L = np.array(box)
+    inside = lo + rng.uniform(n_in * dim).reshape(n_in, dim) * (hi - lo)
+    outside = []
+    while len(outside) < n_out:                                      # uniform in the box, outside the pore
+        q = rng.uniform(dim) * L
+        if not ((q > lo - 1.0) & (q < hi + 1.0)).all():
+            outside.append(q)
+    pos = np.ascontiguousarray(np.concatenate([inside, np.array(outside)]))
+    vel = maxwell_boltzmann(rng, n_in + n_out, dim, t_star)
+    Lp = [float(x) for x in box] + [1.0] * (3 - dim)
+    return dict(name="paper_geometry_%dd_%d" % (dim, n_in + n_out), seed=seed, dim=dim, box_len=Lp,
+                bc=[BC_PERIODIC] * 3, eps=1.0, sigma=1.0, eps_w=2.0, sigma_w=1.0, r_cut=2.5, shift_energy=1,
+                dt=units.PAPER_DT, mass=1.0, pos=pos, vel=vel, wall=np.zeros((0, dim)), n_vapor=n_in + n_out, n_wall=0,
+                steps=2000, algo="allpairs", t_star=t_star,
+                pore=dict(kind="prism", axis=0, center=list(0.5 * (lo + hi)), length=float(hi[0] - lo[0]),
+                          width=float(hi[1] - lo[1])))
+
+
 def small_case(dim, n_vapor, box, bc, n_wall=0, seed=7, t_star=1.0, min_sep=0.9):
     """Small random dense-ish cases for tests: uniform positions with a minimum separation."""
     rng = SplitMix64(seed)

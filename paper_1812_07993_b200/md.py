@@ -168,7 +168,7 @@ class Simulation:
         if cfg.get("pore"):                       # dict(kind="cylinder"|"slit", axis, center, length, r0 | width)
             pd = cfg["pore"]
             pore = md_pore()
-            pore.kind = {"slit": 1, "cylinder": 2}[pd["kind"]]
+            pore.kind = {"slit": 1, "cylinder": 2, "prism": 5}[pd["kind"]]
             pore.axis = int(pd["axis"])
             for a, c in enumerate(pd["center"]):
                 pore.center[a] = float(c)

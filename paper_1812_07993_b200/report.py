@@ -92,6 +92,7 @@ def main():
             cfg = I.paper_size(dim)
             for algo in ("allpairs", "cells", "verlet"):
                 add(cfg, algo, 64, 2000)
+            add(I.paper_geometry(dim), "allpairs", 64, 2000)      # the paper's geometry, units and 2000 steps (NEXT-3)
     if 4 in want:
         for log2n in range(10, args.max_log2n + 1, 2):
             cfg = I.config4(log2n)

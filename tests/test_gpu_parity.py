@@ -444,3 +444,42 @@ def test_device_density_profile_is_bit_exact(algo):
         ra_ref = np.bincount(b[inside & (b < n_r)], minlength=n_r)
         assert ax.sum() == cfg["n_vapor"] and np.array_equal(ax, ax_ref) and np.array_equal(ra, ra_ref)
         sim.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_geometric_prism_pore_matches_oracle(algo):
+    # NEXT-3: the paper's own pore geometry (closed faces reflect, +axis face open), gas inside and outside
+    for dim, box, axis in ((3, (16.0, 15.0, 14.0), 2), (2, (24.0, 20.0), 0)):
+        nv = 220 if dim == 3 else 90
+        cfg = I.small_case(dim, nv, box, (0,) * dim, n_wall=0, seed=12 + dim, min_sep=1.0, t_star=2.0)
+        cfg["pore"] = dict(kind="prism", axis=axis, center=[0.5 * b for b in box], length=7.0, width=5.0)
+        cfg["dt"] = 0.01
+        ref = O.run(cfg, 150, cells=False)
+        assert not np.allclose(ref["pos"], O.run(dict(cfg, pore=None), 150)["pos"])      # the walls did act
+        sim = make_sim(cfg, algo)
+        sim.step(75)
+        sim.step(75)
+        st = sim.get_state()
+        assert traj_error(st["pos"], ref["pos"], cfg["box_len"], cfg["bc"]) <= TRAJ_TOL
+        assert np.abs(st["vel"] - ref["vel"]).max() <= 1e-7
+        sim.close()
+    bad = dict(cfg)
+    bad["pore"] = dict(kind="prism", axis=0, center=[2.0, 10.0], length=7.0, width=5.0)     # sticks out of the box
+    with pytest.raises(md.MDError) as e:
+        md.Simulation(bad, algo=algo)
+    assert e.value.code == md.MD_ERR_INVALID_ARG
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_paper_geometry_and_units_match_oracle(dim):
+    # NEXT-3: the paper's own runs in reduced units, geometric walls, all-pairs
+    cfg = I.paper_geometry(dim)
+    assert cfg["n_vapor"] == (2184 if dim == 2 else 2800) and abs(cfg["dt"] - 0.00959) < 1e-5
+    ref = O.run(cfg, 200)
+    assert not np.array_equal(np.sign(ref["vel"]), np.sign(cfg["vel"]))          # some molecules did bounce
+    sim = md.Simulation(cfg, algo="allpairs")
+    sim.step(200)
+    st = sim.get_state()
+    assert traj_error(st["pos"], ref["pos"], cfg["box_len"], cfg["bc"]) <= TRAJ_TOL
+    assert np.abs(st["vel"] - ref["vel"]).max() <= 1e-7
+    sim.close()
