@@ -474,6 +474,7 @@ struct Sim : md_sim {
                     if (dim == 3) md::k_dbg_build<T, 9><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur);
                     else md::k_dbg_build<T, 3><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur);
                 }
+                for (int k = 0; k < 3; ++k) md::k_dbg_force<T><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur, curv);
                 CK(cudaStreamSynchronize(stream));
             }
             return MD_OK;

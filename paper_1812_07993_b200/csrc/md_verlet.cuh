@@ -521,6 +521,13 @@ __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_build(Params<T> p, Verlet
     phase_build<T, ROWS>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 
+// Diagnostics only (MD_DEBUG_BUILD=1): the force part of the step phase as a kernel of its own (recomputes f(t)).
+template <typename T>
+__global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_force(Params<T> p, Verlet<T> v, int c, int cv)
+{
+    phase_step<T>(p, v, c, cv, true, false, false, 0, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+
 // a5 energy pass over the neighbour list (ordinary launch; the host passes the buffer parities).
 template <typename T>
 __global__ void __launch_bounds__(VL_THREADS) k_verlet_energy(Params<T> p, Verlet<T> v, int c, EnergyOut eo)
