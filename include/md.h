@@ -106,7 +106,8 @@ size_t md_workspace_bytes(const md_box*, const md_lj*, const md_opts*, long long
  * [n_wall][dim], may be NULL iff n_wall == 0), bins, evaluates f(0).  device_workspace: device
  * memory of >= md_workspace_bytes bytes, 256-byte aligned.  cuda_stream: a cudaStream_t (NULL =
  * default stream).  pore may be NULL.  Invalid: dim not 2/3, n_vapor < 1, n_wall < 0, dt <= 0,
- * mass <= 0, r_cut <= 0, non-finite or out-of-box positions, a periodic length < 2 r_cut.
+ * mass <= 0, r_cut <= 0, non-finite or out-of-box positions, a periodic length < 2 r_cut, skin < 0, a thermostat
+ * with tau_b < dt or t_target <= 0, a prism pore not inside the box.
  * MD_ERR_UNSUPPORTED: MD_FORCE_CELLS with a periodic dimension shorter than 3 cells (AUTO falls
  * back to all-pairs).  On failure *out = NULL and md_last_error(NULL) has the reason. */
 int md_create(md_sim** out, const md_box*, const md_pore*, const md_lj*, const md_opts*,
@@ -146,7 +147,8 @@ int md_profile_step(md_sim*, long long n_steps, md_kernel_times* out);
  * (vapor-vapor + vapor-wall), counted by an untimed instrumented pass. */
 int md_pair_tests(md_sim*, long long* tests);
 
-/* Which force kernel the handle uses (MD_FORCE_ALLPAIRS / MD_FORCE_CELLS), its grid, kernels/step. */
+/* Which force path the handle uses (MD_FORCE_ALLPAIRS / MD_FORCE_CELLS / MD_FORCE_VERLET), its cell grid, and the
+ * kernels launched per time step (VERLET: 1 = the whole md_step batch is one persistent launch). */
 int md_info(const md_sim*, int* force_algo, int n_cells[3], int* kernels_per_step);
 
 /* DFMA / FFMA chains on every SM and a device copy; scratch = device memory, >= 64 MiB for a
