@@ -19,7 +19,8 @@
 namespace md {
 
 constexpr int AD_THREADS = 128;   // threads per block = entries per shared-memory tile
-constexpr int AD_IB = 4;          // particles i per thread
+constexpr int AD_IB = 4;          // particles i per thread for large N; 1 below AD_SMALL_N (more, shorter blocks: the
+constexpr int AD_SMALL_N = 8192;  // kernel is latency-bound there, profiles/r01_final_cfg2.md)
 constexpr int AD_UNROLL = 8;      // tests per i between two candidate checks
 
 struct AllPairsDot {
@@ -133,28 +134,28 @@ __device__ __forceinline__ void ap_exact(const Params<double>& p, bool wall, dou
     }
 }
 
-// grid = (i blocks, j slices).  Block (bi, sj) owns particles [bi * 512, bi * 512 + 512) (thread t: i = base +
-// t + 128 b, b < 4) and the tiles t with t % gridDim.y == sj of the j lists (vapor + ghosts, then walls).
+// grid = (i blocks, j slices).  Block (bi, sj) owns particles [bi * 128 IB, (bi + 1) * 128 IB) (thread t: i = base +
+// t + 128 b, b < IB) and the tiles t with t % gridDim.y == sj of the j lists (vapor + ghosts, then walls).
 // Forces are accumulated with fp64 atomics (f was cleared by k_ap_kick_drift_list); ENERGY instead
 // accumulates pe, pe_w, virial and hit counts (cleared by the host) and leaves f alone.
-template <bool ENERGY>
+template <bool ENERGY, int IB>
 __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double> p, AllPairsDot a, Force<double> f,
                                                                    EnergyOut eo)
 {
     __shared__ Vec4<double> sj[AD_THREADS];
-    const int base = blockIdx.x * (AD_THREADS * AD_IB) + threadIdx.x;
-    double ax[AD_IB], ay[AD_IB], az[AD_IB], si[AD_IB];      // -2 x_i, -2 y_i, -2 z_i, |r_i|^2
-    int idx[AD_IB];
+    const int base = blockIdx.x * (AD_THREADS * IB) + threadIdx.x;
+    double ax[IB], ay[IB], az[IB], si[IB];      // -2 x_i, -2 y_i, -2 z_i, |r_i|^2
+    int idx[IB];
 #pragma unroll
-    for (int b = 0; b < AD_IB; ++b) {
+    for (int b = 0; b < IB; ++b) {
         idx[b] = base + b * AD_THREADS;
         // particles beyond nv: parked far away so that they never pass the filter
         Vec4<double> e = {1.0e9, 1.0e9, 1.0e9, 3.0e18};
         if (idx[b] < p.nv) e = a.jv[idx[b]];
         ax[b] = -2.0 * e.x; ay[b] = -2.0 * e.y; az[b] = -2.0 * e.z; si[b] = e.w;
     }
-    double fx[AD_IB] = {}, fy[AD_IB] = {}, fz[AD_IB] = {}, uv[AD_IB] = {}, uw[AD_IB] = {}, wv[AD_IB] = {}, ww[AD_IB] = {};
-    int cv[AD_IB] = {}, cw[AD_IB] = {};
+    double fx[IB] = {}, fy[IB] = {}, fz[IB] = {}, uv[IB] = {}, uw[IB] = {}, wv[IB] = {}, ww[IB] = {};
+    int cv[IB] = {}, cw[IB] = {};
     bool any = false;
     const int nvj = p.nv + *a.ghost_count;
     const int tiles_v = (nvj + AD_THREADS - 1) / AD_THREADS, tiles_w = (a.nwg + AD_THREADS - 1) / AD_THREADS;
@@ -176,7 +177,7 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double
             for (int u = 0; u < AD_UNROLL; ++u) {
                 const Vec4<double> q = sj[k0 + u];
 #pragma unroll
-                for (int b = 0; b < AD_IB; ++b) {
+                for (int b = 0; b < IB; ++b) {
                     const double r2 = fma(ax[b], q.x, fma(ay[b], q.y, fma(az[b], q.z, si[b] + q.w)));
                     cand |= (__double2hiint(r2) < thr);
                 }
@@ -185,7 +186,7 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double
                 for (int u = 0; u < AD_UNROLL; ++u) {
                     const Vec4<double> q = sj[k0 + u];
 #pragma unroll
-                    for (int b = 0; b < AD_IB; ++b) {
+                    for (int b = 0; b < IB; ++b) {
                         const double r2 = fma(ax[b], q.x, fma(ay[b], q.y, fma(az[b], q.z, si[b] + q.w)));
                         if (__double2hiint(r2) >= thr) continue;               // same filter value as above
                         if (!wall && j0 + k0 + u == idx[b]) continue;          // j == i skipped by index
@@ -199,7 +200,7 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double
     }
     if (!any) return;
 #pragma unroll
-    for (int b = 0; b < AD_IB; ++b) {
+    for (int b = 0; b < IB; ++b) {
         const int i = idx[b];
         if (i >= p.nv) continue;
         if (!ENERGY) {
@@ -300,25 +301,25 @@ __global__ void k_apf_wall_list(Params<float> p, AllPairsDotF a, int* __restrict
     push_images_f(p, a, e.x, e.y, e.z, i, a.jw, a.jw_id, p.nw, counter);
 }
 
-template <bool ENERGY>
+template <bool ENERGY, int IB>
 __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dotf(Params<float> p, State<float> s, AllPairsDotF a,
                                                                     Force<float> f, EnergyOut eo)
 {
     __shared__ Vec4<float> sj[AD_THREADS];
     __shared__ int sid[AD_THREADS];
-    const int base = blockIdx.x * (AD_THREADS * AD_IB) + threadIdx.x;
-    float ax[AD_IB], ay[AD_IB], az[AD_IB], si[AD_IB];
-    Vec4<float> ro[AD_IB];                                    // original positions, for the exact path
-    int idx[AD_IB];
+    const int base = blockIdx.x * (AD_THREADS * IB) + threadIdx.x;
+    float ax[IB], ay[IB], az[IB], si[IB];
+    Vec4<float> ro[IB];                                    // original positions, for the exact path
+    int idx[IB];
 #pragma unroll
-    for (int b = 0; b < AD_IB; ++b) {
+    for (int b = 0; b < IB; ++b) {
         idx[b] = base + b * AD_THREADS;
         Vec4<float> e = {1.0e9f, 1.0e9f, 1.0e9f, 3.0e18f};
         ro[b] = e;
         if (idx[b] < p.nv) { e = a.jv[idx[b]]; ro[b] = s.r[idx[b]]; }
         ax[b] = -2.f * e.x; ay[b] = -2.f * e.y; az[b] = -2.f * e.z; si[b] = e.w;
     }
-    Acc<float, ENERGY> av[AD_IB], aw[AD_IB];
+    Acc<float, ENERGY> av[IB], aw[IB];
     bool any = false;
     const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
     const int nvj = p.nv + *a.ghost_count;
@@ -343,7 +344,7 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dotf(Params<float
             for (int u = 0; u < AD_UNROLL; ++u) {
                 const Vec4<float> q = sj[k0 + u];
 #pragma unroll
-                for (int b = 0; b < AD_IB; ++b)
+                for (int b = 0; b < IB; ++b)
                     cand |= fmaf(ax[b], q.x, fmaf(ay[b], q.y, fmaf(az[b], q.z, si[b] + q.w))) < thr;
             }
             if (cand) {
@@ -351,7 +352,7 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dotf(Params<float
                     const Vec4<float> q = sj[k0 + u];
                     const int jo = sid[k0 + u];
 #pragma unroll
-                    for (int b = 0; b < AD_IB; ++b) {
+                    for (int b = 0; b < IB; ++b) {
                         if (!(fmaf(ax[b], q.x, fmaf(ay[b], q.y, fmaf(az[b], q.z, si[b] + q.w))) < thr)) continue;
                         if (jo < 0 || idx[b] >= p.nv || (!wall && jo == idx[b])) continue;
                         const Vec4<float> rj = wall ? a.wr[jo] : s.r[jo];
@@ -369,7 +370,7 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dotf(Params<float
     }
     if (!any) return;
 #pragma unroll
-    for (int b = 0; b < AD_IB; ++b) {
+    for (int b = 0; b < IB; ++b) {
         const int i = idx[b];
         if (i >= p.nv) continue;
         const float fx = av[b].fx + aw[b].fx, fy = av[b].fy + aw[b].fy, fz = av[b].fz + aw[b].fz;

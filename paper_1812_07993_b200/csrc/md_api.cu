@@ -239,7 +239,7 @@ struct Sim : md_sim {
     md::AllPairsDot ad;
     md::AllPairsDotF adf;
     bool dot = false;           // all-pairs through the dot-product kernels (md_allpairs.cuh)
-    int ad_slices = 1;
+    int ad_slices = 1, ad_ib = md::AD_IB;
     int gpar = 0;               // which of the two ghost counters describes the current j list
 
     bool verlet() const { return algo == MD_FORCE_VERLET; }
@@ -336,11 +336,14 @@ struct Sim : md_sim {
                     cudaMemsetAsync(l.eo.cvv, 0, n * sizeof(int), stream);
                     cudaMemsetAsync(l.eo.cvw, 0, n * sizeof(int), stream);
                 }
-                const dim3 grid(cdiv(p.nv, md::AD_THREADS * md::AD_IB), ad_slices);
-                if constexpr (std::is_same<T, double>::value)
-                    md::k_force_allpairs_dot<ENERGY><<<grid, md::AD_THREADS, 0, stream>>>(p, ad, l.f, l.eo);
-                else
-                    md::k_force_allpairs_dotf<ENERGY><<<grid, md::AD_THREADS, 0, stream>>>(p, l.st[cur], adf, l.f, l.eo);
+                const dim3 grid(cdiv(p.nv, md::AD_THREADS * ad_ib), ad_slices);
+                if constexpr (std::is_same<T, double>::value) {
+                    if (ad_ib == 1) md::k_force_allpairs_dot<ENERGY, 1><<<grid, md::AD_THREADS, 0, stream>>>(p, ad, l.f, l.eo);
+                    else md::k_force_allpairs_dot<ENERGY, md::AD_IB><<<grid, md::AD_THREADS, 0, stream>>>(p, ad, l.f, l.eo);
+                } else {
+                    if (ad_ib == 1) md::k_force_allpairs_dotf<ENERGY, 1><<<grid, md::AD_THREADS, 0, stream>>>(p, l.st[cur], adf, l.f, l.eo);
+                    else md::k_force_allpairs_dotf<ENERGY, md::AD_IB><<<grid, md::AD_THREADS, 0, stream>>>(p, l.st[cur], adf, l.f, l.eo);
+                }
                 // the second half-kick also clears the OTHER ghost counter, which the next step's list will fill
                 if (KICK) md::k_ap_kick<T><<<blocks(256), 256, 0, stream>>>(p, l.st[cur], l.f, l.ghost_count + (gpar ^ 1));
             }
@@ -772,11 +775,12 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
             int dev = 0, sms = 148, nb = 4;
             cudaGetDevice(&dev);
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            ad_ib = nv < md::AD_SMALL_N ? 1 : md::AD_IB;
             if constexpr (std::is_same<T, double>::value)
-                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, md::k_force_allpairs_dot<false>, md::AD_THREADS, 0);
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, md::k_force_allpairs_dot<false, md::AD_IB>, md::AD_THREADS, 0);
             else
-                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, md::k_force_allpairs_dotf<false>, md::AD_THREADS, 0);
-            const int slots = std::max(1, nb * sms), ib = cdiv(nv, md::AD_THREADS * md::AD_IB);
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, md::k_force_allpairs_dotf<false, md::AD_IB>, md::AD_THREADS, 0);
+            const int slots = std::max(1, nb * sms), ib = cdiv(nv, md::AD_THREADS * ad_ib);
             double best = -1.0;
             for (int sl = 1; sl <= std::min(tiles, 96); ++sl) {
                 const double waves = (double)ib * sl / slots;
