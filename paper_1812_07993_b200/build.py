@@ -4,7 +4,8 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRCS = [os.path.join(HERE, "csrc", "md_api.cu")]
-DEPS = SRCS + [os.path.join(HERE, "csrc", "md_kernels.cuh"), os.path.join(HERE, "..", "include", "md.h")]
+DEPS = SRCS + [os.path.join(HERE, "csrc", h) for h in ("md_kernels.cuh", "md_allpairs.cuh", "md_verlet.cuh")] + [
+    os.path.join(HERE, "..", "include", "md.h")]
 LIB = os.path.join(HERE, "libmd_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 

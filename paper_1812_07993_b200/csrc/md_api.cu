@@ -268,6 +268,9 @@ struct Sim : md_sim {
             // one thread per particle; whole multiples of the SM count keep the SMs evenly loaded
             const int want = cdiv(cdiv(p.nv, md::VL_THREADS), sms) * sms;
             coop_grid = std::max(1, std::min(nb * sms, p.nv <= md::VL_THREADS * sms ? cdiv(p.nv, md::VL_THREADS) : want));
+            // lane groups for long lists pay while the particles fit one wave (measured: -13 % per step at 2^16,
+            // +1..2 % at 2^18 and 2^20, profiles/r01_heavy_groups.md)
+            if (!getenv("MD_HEAVY_T")) vl.heavy_t = p.nv <= coop_grid * md::VL_THREADS ? 12 : md::VL_MAXN;
         }
         CK(cudaMemsetAsync(l.vflags + md::VF_REQ0, 0, 3 * sizeof(int), stream));   // rebuild-request slots
         CK(cudaMemsetAsync(l.vbar, 0, 2 * sizeof(unsigned long long), stream));        // grid barrier counter
@@ -459,6 +462,11 @@ struct Sim : md_sim {
                 for (int k = 0; k < nwarp && k < 8192; ++k) { mx = std::max(mx, w[k]); sm += w[k]; }
                 fprintf(stderr, "\n[md] max %.0f us mean %.0f us\n", mx * 1e-3, sm * 1e-3 / nwarp);
             }
+            if (getenv("MD_DEBUG_TIMES")) {
+                int nh = 0;
+                CK(cudaMemcpy(&nh, l.vflags + md::VF_NHEAVY, sizeof(int), cudaMemcpyDeviceToHost));
+                fprintf(stderr, "[md] heavy particles (list > %d entries) after the last rebuild: %d\n", vl.heavy_t, nh);
+            }
             if (getenv("MD_DEBUG_TIMES"))
                 fprintf(stderr, "[md] cumulative ns: step %llu barrier %llu rebuild %llu final %llu | bin %llu scan %llu "
                         "scatter %llu build %llu\n", t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7]);
@@ -598,7 +606,7 @@ struct Sim : md_sim {
             CK(cudaMemcpyAsync(h.data(), l.ncnt, sizeof(int) * h.size(), cudaMemcpyDeviceToHost, stream));
             CK(cudaStreamSynchronize(stream));
             long long t = 0;
-            for (int c : h) t += c & (md::VL_FOLD - 1);
+            for (int c : h) t += c & md::VL_NMASK;
             *tests = t;
             return MD_OK;
         }
@@ -885,6 +893,7 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
         v.cell = s->l.cell; v.slot = s->l.slot; v.count = s->l.count; v.start = s->l.start; v.tile_sum = s->l.tile_sum;
         v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.bar = s->l.vbar; v.ksum = s->l.vksum; v.times = s->l.vtimes; v.dbg = getenv("MD_DEBUG_TIMES") ? s->l.vtimes + 8 : nullptr;
         v.rl2 = (T)(rl * rl); v.half_skin = (T)(0.5 * skin);
+        v.heavy_t = getenv("MD_HEAVY_T") ? atoi(getenv("MD_HEAVY_T")) : 12;
     }
     int rc = s->init(box, lj, o, nv, pos, vel, nw, wall);
     if (rc != MD_OK) {

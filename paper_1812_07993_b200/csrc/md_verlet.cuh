@@ -25,7 +25,7 @@ constexpr int VL_MAXN = 128;   // neighbour-list stride (entries per particle)
 // The rebuild request rotates over three slots (step % 3): a slot is cleared one barrier before the phase that
 // may set it and read one barrier after, so no block can see a later step's request (which would desynchronise
 // the grid barriers).
-enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_COUNT = 8 };
+enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_COUNT = 9 };
 
 template <typename T>
 struct Verlet {
@@ -45,6 +45,9 @@ struct Verlet {
     unsigned long long* times; // [8] ns seen by thread 0: step phases, step barriers, rebuilds, final phase,
                                // rebuild split: bin, scan, scatter, list build (each with its barrier)
     T rl2, half_skin;          // (r_c + skin)^2, skin / 2
+    int heavy_t;               // particles whose list is longer than this are "heavy": in the step phase an 8-lane
+                               // group shares one such list (indices in `cell`, ncnt words in `slot` -- both free
+                               // between rebuilds; their number in flags[VF_NHEAVY])
 };
 
 // d = a - b folded to the nearest image by comparison (|true d| < r_c + skin < L/2).  fp32: the shift
@@ -97,6 +100,12 @@ __device__ __forceinline__ unsigned long long now_ns()
 // built: only such particles can have a neighbour across the face, all others skip the image folding.
 // Entries are consumed four at a time: four index loads, then four position loads, are in flight together.
 constexpr int VL_FOLD = 1 << 30;
+constexpr int VL_HEAVY = 1 << 29;      // list longer than Verlet::heavy_t (see phase_step)
+constexpr int VL_NMASK = (1 << 16) - 1;
+#ifndef MD_VL_GROUP
+#define MD_VL_GROUP 8
+#endif
+constexpr int VL_GROUP = MD_VL_GROUP;   // lanes sharing one heavy particle's list
 
 // 1 / x without the division's special-case branch: hardware seed (>= 20 bits) + two Newton steps.
 __device__ __forceinline__ double rcp_fast(double x)
@@ -171,8 +180,36 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
 #pragma unroll
     for (int u = 0; u < 4; ++u) j0[u] = lst[(size_t)u * v.stride];       // in flight together with ncnt (and r_i, v_i)
     const int raw = v.ncnt[i];
-    if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & (VL_FOLD - 1), r, ri, j0, av, aw);
-    else list_loop<T, ENERGY, false>(p, lst, v.stride, raw, r, ri, j0, av, aw);
+    if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
+    else list_loop<T, ENERGY, false>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
+}
+
+// A heavy particle's list shared by the VL_GROUP lanes of a group: lane `sub` takes entries sub, sub + 8, sub + 16,
+// ... of every 4 * VL_GROUP (one batch of four covers lists of up to that many entries); the caller sums the lanes' partial forces.
+template <typename T, bool FOLD>
+__device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* __restrict__ lst, size_t stride, int n,
+                                                int sub, const Vec4<T>* __restrict__ r, const Vec4<T>& ri,
+                                                Acc<T, false>& av, Acc<T, false>& aw)
+{
+    const bool px = FOLD && p.bc[0] == BC_PERIODIC, py = FOLD && p.bc[1] == BC_PERIODIC, pz = FOLD && p.bc[2] == BC_PERIODIC;
+    for (int k = 0; k < n; k += 4 * VL_GROUP) {
+        int j[4];
+        Vec4<T> rj[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int kk = k + sub + VL_GROUP * u;
+            j[u] = kk < n ? lst[(size_t)kk * stride] : -1;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) rj[u] = r[max(j[u], 0)];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
+            const T dy = py ? fold(ri.y, rj[u].y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj[u].y;
+            const T dz = pz ? fold(ri.z, rj[u].z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj[u].z;
+            pair_term_nb<T, false>(p, j[u] >= 0, j[u] >= p.nv, dx, dy, dz, av, aw);
+        }
+    }
 }
 
 // ---- phase: [forces] -> [kick completing the step] -> [kick + drift of the next step] -----------
@@ -187,19 +224,8 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
     Vec4<T>* __restrict__ rnew = v.st[c ^ 1].r;
     const State<T>& s = v.st[cv];
     double kacc = 0.0;
-    for (int i = gtid; i < p.nv; i += gthreads) {
-        const Vec4<T> ri = rcur[i];
-        T vx = s.vx[i], vy = s.vy[i], vz = s.vz[i];      // issued early, consumed after the force loop
-        vx = lam * vx; vy = lam * vy; vz = lam * vz;     // F4 of the step just completed (lam = 1 without thermostat)
-        T fx, fy, fz;
-        if (force) {
-            Acc<T, false> av, aw;
-            list_force<T, false>(p, v, rcur, i, ri, av, aw);
-            fx = av.fx + aw.fx; fy = av.fy + aw.fy; fz = av.fz + aw.fz;
-            v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz;
-        } else {
-            fx = v.f.fx[i]; fy = v.f.fy[i]; fz = v.f.fz[i];
-        }
+    // F3 / F2 of particle i once its force is known (v already carries F4's factor)
+    auto integrate = [&](int i, const Vec4<T>& ri, T vx, T vy, T vz, T fx, T fy, T fz) {
         if (kick) {                                    // F3: v(t) = v(t - dt/2) + (dt/2m) f(t)
             vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
         }
@@ -225,6 +251,56 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             rnew[i] = rn;
         }
         if (kick || drift || lam != T(1)) { s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz; }
+    };
+    for (int i = gtid; i < p.nv; i += gthreads) {
+        const Vec4<T> ri = rcur[i];
+        T vx = s.vx[i], vy = s.vy[i], vz = s.vz[i];      // issued early, consumed after the force loop
+        vx = lam * vx; vy = lam * vy; vz = lam * vz;     // F4 of the step just completed (lam = 1 without thermostat)
+        T fx, fy, fz;
+        if (force) {
+            if (v.ncnt[i] & VL_HEAVY) continue;          // the whole particle belongs to a lane group below
+            Acc<T, false> av, aw;
+            list_force<T, false>(p, v, rcur, i, ri, av, aw);
+            fx = av.fx + aw.fx; fy = av.fy + aw.fy; fz = av.fz + aw.fz;
+            v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz;
+        } else {
+            fx = v.f.fx[i]; fy = v.f.fy[i]; fz = v.f.fz[i];
+        }
+        integrate(i, ri, vx, vy, vz, fx, fy, fz);
+    }
+    if (force) {
+        // Heavy particles (list longer than heavy_t: next to a wall, inside a cluster): one per group of VL_GROUP
+        // lanes, so that no warp walks a list several times the typical length while the grid waits at the
+        // barrier.  Group slots are numbered so that the blocks past the last particle (idle when the particles
+        // fill less than one wave) take this work first and the rest is dealt round-robin over the other blocks,
+        // one group per block and warp at a time.
+        const int nh = v.flags[VF_NHEAVY];
+        const int lane = threadIdx.x & 31, sub = lane & (VL_GROUP - 1);
+        const unsigned gmask = ((1u << VL_GROUP) - 1u) << (lane & ~(VL_GROUP - 1));
+        constexpr int GPW = 32 / VL_GROUP, GPB = VL_THREADS / VL_GROUP;         // groups per warp, per block
+        const int nbl = min((int)gridDim.x, (p.nv + VL_THREADS - 1) / VL_THREADS), nsp = (int)gridDim.x - nbl;
+        const int b = blockIdx.x, q = (lane / VL_GROUP) * (VL_THREADS / 32) + (threadIdx.x >> 5);
+        const int slot = b >= nbl ? (b - nbl) + nsp * ((threadIdx.x >> 5) * GPW + lane / VL_GROUP) : nsp * GPB + q * nbl + b;
+        for (int h = slot; h < nh; h += gthreads / VL_GROUP) {
+            const int i = v.cell[h], raw = v.slot[h];
+            const Vec4<T> ri = rcur[i];
+            T vx = T(0), vy = T(0), vz = T(0);
+            if (sub == 0) { vx = lam * s.vx[i]; vy = lam * s.vy[i]; vz = lam * s.vz[i]; }
+            Acc<T, false> av, aw;
+            if (raw & VL_FOLD) list_loop_group<T, true>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, av, aw);
+            else list_loop_group<T, false>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, av, aw);
+            T fx = av.fx + aw.fx, fy = av.fy + aw.fy, fz = av.fz + aw.fz;
+#pragma unroll
+            for (int o = 1; o < VL_GROUP; o <<= 1) {
+                fx += __shfl_xor_sync(gmask, fx, o);
+                fy += __shfl_xor_sync(gmask, fy, o);
+                fz += __shfl_xor_sync(gmask, fz, o);
+            }
+            if (sub == 0) {
+                v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz;
+                integrate(i, ri, vx, vy, vz, fx, fy, fz);
+            }
+        }
     }
     if (ksum) {                                        // thermostat: this thread's share of K(t), one atomic per warp
         kacc = warp_sum_d(kacc);
@@ -432,7 +508,13 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
             const bool face = (p.bc[0] == BC_PERIODIC && (cx == 0 || cx == nx - 1)) ||
                               (p.bc[1] == BC_PERIODIC && (cy == 0 || cy == ny - 1)) ||
                               (p.bc[2] == BC_PERIODIC && (cz == 0 || cz == nz - 1));
-            v.ncnt[i] = min(n, VL_MAXN) | (face ? VL_FOLD : 0);
+            const bool heavy = n > v.heavy_t;
+            const int raw = min(n, VL_MAXN) | (face ? VL_FOLD : 0) | (heavy ? VL_HEAVY : 0);
+            if (heavy) {                                   // `cell` and `slot` are free until the next rebuild
+                const int h = atomicAdd(v.flags + VF_NHEAVY, 1);
+                v.cell[h] = i; v.slot[h] = raw;
+            }
+            v.ncnt[i] = raw;
             if (n > VL_MAXN) v.flags[VF_OVERFLOW] = 1;
         }
         __syncwarp();
@@ -458,6 +540,7 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
     for (long long s = 0;; ++s) {
         if (rebuild) {
             unsigned long long u0 = gtid == 0 ? now_ns() : 0ull, u1;
+            if (gtid == 0) v.flags[VF_NHEAVY] = 0;
             phase_bin<T>(p, v, c, gtid, gthreads);
             grid_barrier(v.bar, bar_target);
             if (gtid == 0) { u1 = now_ns(); v.times[4] += u1 - u0; u0 = u1; }
