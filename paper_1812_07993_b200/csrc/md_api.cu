@@ -11,6 +11,7 @@
 #include <cstring>
 #include <string>
 #include <type_traits>
+#include <algorithm>
 #include <vector>
 
 namespace {
@@ -460,7 +461,14 @@ struct Sim : md_sim {
                 for (int k = 0; k < nwarp && k < 8192; k += 37) fprintf(stderr, " %.0f", w[k] * 1e-3);
                 unsigned long long mx = 0, sm = 0;
                 for (int k = 0; k < nwarp && k < 8192; ++k) { mx = std::max(mx, w[k]); sm += w[k]; }
-                fprintf(stderr, "\n[md] max %.0f us mean %.0f us\n", mx * 1e-3, sm * 1e-3 / nwarp);
+                fprintf(stderr, "\n[md] max %.0f us mean %.0f us; slowest warps:", mx * 1e-3, sm * 1e-3 / nwarp);
+                std::vector<int> order(std::min(nwarp, 8192));
+                for (size_t k = 0; k < order.size(); ++k) order[k] = (int)k;
+                std::partial_sort(order.begin(), order.begin() + std::min<size_t>(12, order.size()), order.end(),
+                                  [&](int x, int y) { return w[x] > w[y]; });
+                for (size_t k = 0; k < std::min<size_t>(12, order.size()); ++k)
+                    fprintf(stderr, " %d:%.0f", order[k], w[order[k]] * 1e-3);
+                fprintf(stderr, "\n");
             }
             if (getenv("MD_DEBUG_TIMES")) {
                 int nh = 0;

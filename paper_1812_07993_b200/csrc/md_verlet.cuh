@@ -103,7 +103,7 @@ constexpr int VL_FOLD = 1 << 30;
 constexpr int VL_HEAVY = 1 << 29;      // list longer than Verlet::heavy_t (see phase_step)
 constexpr int VL_NMASK = (1 << 16) - 1;
 #ifndef MD_VL_GROUP
-#define MD_VL_GROUP 8
+#define MD_VL_GROUP 4
 #endif
 constexpr int VL_GROUP = MD_VL_GROUP;   // lanes sharing one heavy particle's list
 
@@ -132,8 +132,12 @@ __device__ __forceinline__ void pair_term_nb(const Params<T>& p, bool valid, boo
     const T s6 = s3 * s3;
     const T g = hit ? (wall ? p.e24_vw : p.e24_vv) * inv * (T(2) * s6 - s3) : T(0);
     const T gw = wall ? g : T(0), gv = wall ? T(0) : g;
-    av.fx = fma_(gv, dx, av.fx); av.fy = fma_(gv, dy, av.fy); av.fz = fma_(gv, dz, av.fz);
-    aw.fx = fma_(gw, dx, aw.fx); aw.fy = fma_(gw, dy, aw.fy); aw.fz = fma_(gw, dz, aw.fz);
+    if (ENERGY) {                                           // U_vv and U_vw are reported separately
+        av.fx = fma_(gv, dx, av.fx); av.fy = fma_(gv, dy, av.fy); av.fz = fma_(gv, dz, av.fz);
+        aw.fx = fma_(gw, dx, aw.fx); aw.fy = fma_(gw, dy, aw.fy); aw.fz = fma_(gw, dz, aw.fz);
+    } else {                                                // time loop: one accumulator (aw stays 0)
+        av.fx = fma_(g, dx, av.fx); av.fy = fma_(g, dy, av.fy); av.fz = fma_(g, dz, av.fz);
+    }
     if (ENERGY) {
         const double u = hit ? (double)((wall ? p.e4_vw : p.e4_vv) * (s6 - s3) - (wall ? p.uc_vw : p.uc_vv)) : 0.0;
         const double w = (double)(g * r2);
@@ -142,27 +146,32 @@ __device__ __forceinline__ void pair_term_nb(const Params<T>& p, bool valid, boo
     }
 }
 
-// Batches of four list entries; while batch b is evaluated the indices of batch b + 1 are in flight.  The first
+// Batches of VL_BATCH list entries; while batch b is evaluated the indices of batch b + 1 are in flight.  The first
 // index loads do not wait for the list length (rows beyond it are allocated; their values are masked), so the
 // first positions are requested one round trip after the thread starts.
+#ifndef MD_VL_BATCH
+#define MD_VL_BATCH 4
+#endif
+constexpr int VL_BATCH = MD_VL_BATCH;
 template <typename T, bool ENERGY, bool FOLD>
 __device__ __forceinline__ void list_loop(const Params<T>& p, const int* __restrict__ lst, size_t stride, int n,
-                                          const Vec4<T>* __restrict__ r, const Vec4<T>& ri, const int (&j0)[4],
+                                          const Vec4<T>* __restrict__ r, const Vec4<T>& ri, const int (&j0)[VL_BATCH],
                                           Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
     const bool px = FOLD && p.bc[0] == BC_PERIODIC, py = FOLD && p.bc[1] == BC_PERIODIC, pz = FOLD && p.bc[2] == BC_PERIODIC;
-    int jn[4];
+    int jn[VL_BATCH];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) jn[u] = u < n ? j0[u] : -1;
-    for (int k = 0; k < n; k += 4) {
-        int j[4];
-        Vec4<T> rj[4];
+    for (int u = 0; u < VL_BATCH; ++u) jn[u] = u < n ? j0[u] : -1;
+    for (int k = 0; k < n; k += VL_BATCH) {
+        int j[VL_BATCH];
+        Vec4<T> rj[VL_BATCH];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { j[u] = jn[u]; rj[u] = r[max(j[u], 0)]; }
+        for (int u = 0; u < VL_BATCH; ++u) { j[u] = jn[u]; rj[u] = r[max(j[u], 0)]; }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) jn[u] = k + 4 + u < n ? lst[(size_t)(k + 4 + u) * stride] : -1;   // next batch
+        for (int u = 0; u < VL_BATCH; ++u)
+            jn[u] = k + VL_BATCH + u < n ? lst[(size_t)(k + VL_BATCH + u) * stride] : -1;   // next batch
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < VL_BATCH; ++u) {
             const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
             const T dy = py ? fold(ri.y, rj[u].y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj[u].y;
             const T dz = pz ? fold(ri.z, rj[u].z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj[u].z;
@@ -176,9 +185,9 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
                                            const Vec4<T>& ri, Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
     const int* __restrict__ lst = v.nbr + i;
-    int j0[4];
+    int j0[VL_BATCH];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) j0[u] = lst[(size_t)u * v.stride];       // in flight together with ncnt (and r_i, v_i)
+    for (int u = 0; u < VL_BATCH; ++u) j0[u] = lst[(size_t)u * v.stride];   // in flight together with ncnt (and r_i, v_i)
     const int raw = v.ncnt[i];
     if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
     else list_loop<T, ENERGY, false>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
