@@ -232,7 +232,7 @@ struct Sim : md_sim {
     double e_host[6];
     // VERLET (persistent kernel): device-side buffer parities are mirrored here by refresh()
     md::Verlet<T> vl;
-    int curv = 0, coop_grid = 0;
+    int curv = 0, coop_grid = 0, coop_base = 0, coop_max = 0, heavy_seen = 0;
     int minb3_threshold = getenv("MD_MINB3_THRESHOLD") ? atoi(getenv("MD_MINB3_THRESHOLD")) : 500000;
     long long rebuilds_seen = 0;
     unsigned long long phase_seen[4] = {0, 0, 0, 0}, phase_ns[4] = {0, 0, 0, 0};
@@ -258,7 +258,7 @@ struct Sim : md_sim {
         const bool big = p.nv > minb3_threshold;
         void* kernel = dim == 3 ? (big ? (void*)md::k_md_run<T, 9, 3> : (void*)md::k_md_run<T, 9, 2>)
                                 : (big ? (void*)md::k_md_run<T, 3, 3> : (void*)md::k_md_run<T, 3, 2>);
-        if (!coop_grid) {
+        if (!coop_max) {
             int dev = 0, sms = 0, coop = 0, nb = 0;
             CK(cudaGetDevice(&dev));
             CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
@@ -266,13 +266,19 @@ struct Sim : md_sim {
             CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
             CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, md::VL_THREADS, 0));
             if (nb < 1) { err = "persistent kernel does not fit on an SM"; return MD_ERR_CUDA; }
+            coop_max = nb * sms;
             // one thread per particle; whole multiples of the SM count keep the SMs evenly loaded
             const int want = cdiv(cdiv(p.nv, md::VL_THREADS), sms) * sms;
-            coop_grid = std::max(1, std::min(nb * sms, p.nv <= md::VL_THREADS * sms ? cdiv(p.nv, md::VL_THREADS) : want));
-            // lane groups for long lists pay while the particles fit one wave (measured: -13 % per step at 2^16,
-            // +1..2 % at 2^18 and 2^20, profiles/r01_heavy_groups.md)
-            if (!getenv("MD_HEAVY_T")) vl.heavy_t = p.nv <= coop_grid * md::VL_THREADS ? 12 : md::VL_MAXN;
+            coop_base = std::max(1, std::min(coop_max, p.nv <= md::VL_THREADS * sms ? cdiv(p.nv, md::VL_THREADS) : want));
         }
+        // Blocks past the last particle serve the lane groups of the particles with long lists (the kernel hands
+        // out only as many as those blocks hold: measured -13 % per step at 2^16 with them, +1..2 % at 2^18 and
+        // 2^20 where the work would land on busy blocks, profiles/r01_heavy_groups.md): an eighth of the particle
+        // blocks, or what the last list this handle has seen asked for (refresh() mirrors the count) plus a quarter.
+        const int light = cdiv(p.nv, md::VL_THREADS);
+        coop_grid = coop_base;
+        if (light < coop_max)
+            coop_grid = std::min(coop_max, std::max(coop_base, light + std::max(light / 8, cdiv(heavy_seen * md::VL_GROUP * 5 / 4, md::VL_THREADS)) + 1));
         CK(cudaMemsetAsync(l.vflags + md::VF_REQ0, 0, 3 * sizeof(int), stream));   // rebuild-request slots
         CK(cudaMemsetAsync(l.vbar, 0, 2 * sizeof(unsigned long long), stream));        // grid barrier counter
         CK(cudaMemsetAsync(l.vksum, 0, 4 * sizeof(double), stream));
@@ -289,7 +295,7 @@ struct Sim : md_sim {
         CK(cudaMemcpyAsync(h, l.vflags, sizeof(h), cudaMemcpyDeviceToHost, stream));
         CK(cudaStreamSynchronize(stream));
         CK(cudaGetLastError());
-        cur = h[md::VF_CUR]; curv = h[md::VF_CURV]; rebuilds_seen = h[md::VF_NREBUILD];
+        cur = h[md::VF_CUR]; curv = h[md::VF_CURV]; rebuilds_seen = h[md::VF_NREBUILD]; heavy_seen = h[md::VF_NHEAVY];
         if (h[md::VF_ESCAPE]) { err = "a particle left a reflecting box (more than one bounce in a step)"; return MD_ERR_STATE; }
         if (h[md::VF_OVERFLOW]) { err = "neighbour list overflow (> 128 neighbours within r_cut + skin)"; return MD_ERR_WORKSPACE; }
         return MD_OK;

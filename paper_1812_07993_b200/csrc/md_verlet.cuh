@@ -21,11 +21,12 @@ namespace cg = cooperative_groups;
 constexpr int VL_THREADS = 256;
 constexpr int VL_MAXN = 128;   // neighbour-list stride (entries per particle)
 
-// flags: rebuild request, list overflow, position-buffer parity, velocity/id-buffer parity, rebuild count, escape
+// flags: rebuild request, list overflow, position-buffer parity, velocity/id-buffer parity, rebuild count, escape,
+// particles with a long list at the last rebuild (demand), how many of them the idle blocks' lane groups took (capacity)
 // The rebuild request rotates over three slots (step % 3): a slot is cleared one barrier before the phase that
 // may set it and read one barrier after, so no block can see a later step's request (which would desynchronise
 // the grid barriers).
-enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_COUNT = 9 };
+enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_HCAP = 9, VF_COUNT = 10 };
 
 template <typename T>
 struct Verlet {
@@ -283,7 +284,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         // barrier.  Group slots are numbered so that the blocks past the last particle (idle when the particles
         // fill less than one wave) take this work first and the rest is dealt round-robin over the other blocks,
         // one group per block and warp at a time.
-        const int nh = v.flags[VF_NHEAVY];
+        const int nh = min(v.flags[VF_NHEAVY], v.flags[VF_HCAP]);
         const int lane = threadIdx.x & 31, sub = lane & (VL_GROUP - 1);
         const unsigned gmask = ((1u << VL_GROUP) - 1u) << (lane & ~(VL_GROUP - 1));
         constexpr int GPW = 32 / VL_GROUP, GPB = VL_THREADS / VL_GROUP;         // groups per warp, per block
@@ -463,7 +464,7 @@ __device__ __forceinline__ void list_range(const Params<T>& p, const Vec4<T>* __
 }
 
 template <typename T, int ROWS>
-__device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>& v, int c, int gtid, int gthreads)
+__device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>& v, int c, int gtid, int gthreads, int hcap)
 {
     constexpr int PPW = 32 / ROWS;                       // particles per warp
     __shared__ int s_cnt[(VL_THREADS / 32) * PPW];
@@ -517,11 +518,12 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
             const bool face = (p.bc[0] == BC_PERIODIC && (cx == 0 || cx == nx - 1)) ||
                               (p.bc[1] == BC_PERIODIC && (cy == 0 || cy == ny - 1)) ||
                               (p.bc[2] == BC_PERIODIC && (cz == 0 || cz == nz - 1));
-            const bool heavy = n > v.heavy_t;
-            const int raw = min(n, VL_MAXN) | (face ? VL_FOLD : 0) | (heavy ? VL_HEAVY : 0);
-            if (heavy) {                                   // `cell` and `slot` are free until the next rebuild
+            // a long list goes to a lane group while the idle blocks have groups left (the counter keeps the
+            // demand; the host sizes the next launch by it); `cell` and `slot` are free until the next rebuild
+            int raw = min(n, VL_MAXN) | (face ? VL_FOLD : 0);
+            if (n > v.heavy_t) {
                 const int h = atomicAdd(v.flags + VF_NHEAVY, 1);
-                v.cell[h] = i; v.slot[h] = raw;
+                if (h < hcap) { raw |= VL_HEAVY; v.cell[h] = i; v.slot[h] = raw; }
             }
             v.ncnt[i] = raw;
             if (n > VL_MAXN) v.flags[VF_OVERFLOW] = 1;
@@ -545,11 +547,13 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
     const int gthreads = gridDim.x * blockDim.x;
     int c = v.flags[VF_CUR], cv = v.flags[VF_CURV];
     bool rebuild = force_rebuild != 0;
+    // lane groups in the blocks past the last particle (none once the particles fill the grid)
+    const int hcap = max((int)gridDim.x - (p.nv + VL_THREADS - 1) / VL_THREADS, 0) * (VL_THREADS / VL_GROUP);
     unsigned long long t0 = gtid == 0 ? now_ns() : 0ull, t1;
     for (long long s = 0;; ++s) {
         if (rebuild) {
             unsigned long long u0 = gtid == 0 ? now_ns() : 0ull, u1;
-            if (gtid == 0) v.flags[VF_NHEAVY] = 0;
+            if (gtid == 0) { v.flags[VF_NHEAVY] = 0; v.flags[VF_HCAP] = hcap; }
             phase_bin<T>(p, v, c, gtid, gthreads);
             grid_barrier(v.bar, bar_target);
             if (gtid == 0) { u1 = now_ns(); v.times[4] += u1 - u0; u0 = u1; }
@@ -565,7 +569,7 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
             grid_barrier(v.bar, bar_target);
             if (gtid == 0) { u1 = now_ns(); v.times[6] += u1 - u0; u0 = u1; }
             c ^= 1; cv ^= 1;
-            phase_build<T, ROWS>(p, v, c, gtid, gthreads);
+            phase_build<T, ROWS>(p, v, c, gtid, gthreads, hcap);
             for (int q = gtid; q < p.ncell; q += gthreads) v.count[q] = 0;                  // for the next rebuild
             if (gtid == 0) v.flags[VF_NREBUILD] += 1;
             grid_barrier(v.bar, bar_target);
@@ -610,7 +614,7 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
 template <typename T, int ROWS>
 __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_build(Params<T> p, Verlet<T> v, int c)
 {
-    phase_build<T, ROWS>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+    phase_build<T, ROWS>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, v.flags[VF_HCAP]);
 }
 
 // Diagnostics only (MD_DEBUG_BUILD=1): the force part of the step phase as a kernel of its own (recomputes f(t)).
