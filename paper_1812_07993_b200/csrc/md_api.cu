@@ -908,6 +908,7 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
         v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.bar = s->l.vbar; v.ksum = s->l.vksum; v.times = s->l.vtimes; v.dbg = getenv("MD_DEBUG_TIMES") ? s->l.vtimes + 8 : nullptr;
         v.rl2 = (T)(rl * rl); v.half_skin = (T)(0.5 * skin);
         v.heavy_t = getenv("MD_HEAVY_T") ? atoi(getenv("MD_HEAVY_T")) : 12;
+        v.carry = getenv("MD_NO_CARRY") ? 0 : 1;
     }
     int rc = s->init(box, lj, o, nv, pos, vel, nw, wall);
     if (rc != MD_OK) {

@@ -46,6 +46,7 @@ struct Verlet {
     unsigned long long* times; // [8] ns seen by thread 0: step phases, step barriers, rebuilds, final phase,
                                // rebuild split: bin, scan, scatter, list build (each with its barrier)
     T rl2, half_skin;          // (r_c + skin)^2, skin / 2
+    int carry;                 // 0: reload own state every step (diagnostic A/B, MD_NO_CARRY)
     int heavy_t;               // particles whose list is longer than this are "heavy": in the step phase an 8-lane
                                // group shares one such list (indices in `cell`, ncnt words in `slot` -- both free
                                // between rebuilds; their number in flags[VF_NHEAVY])
@@ -183,15 +184,22 @@ __device__ __forceinline__ void list_loop(const Params<T>& p, const int* __restr
 
 template <typename T, bool ENERGY>
 __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& v, const Vec4<T>* __restrict__ r, int i,
-                                           const Vec4<T>& ri, Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
+                                           const Vec4<T>& ri, int raw, const int (&j0)[VL_BATCH],
+                                           Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
     const int* __restrict__ lst = v.nbr + i;
-    int j0[VL_BATCH];
-#pragma unroll
-    for (int u = 0; u < VL_BATCH; ++u) j0[u] = lst[(size_t)u * v.stride];   // in flight together with ncnt (and r_i, v_i)
-    const int raw = v.ncnt[i];
     if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
     else list_loop<T, ENERGY, false>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
+}
+
+template <typename T, bool ENERGY>
+__device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& v, const Vec4<T>* __restrict__ r, int i,
+                                           const Vec4<T>& ri, Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
+{
+    int j0[VL_BATCH];
+#pragma unroll
+    for (int u = 0; u < VL_BATCH; ++u) j0[u] = v.nbr[(size_t)u * v.stride + i];   // in flight together with ncnt (and r_i, v_i)
+    list_force<T, ENERGY>(p, v, r, i, ri, v.ncnt[i], j0, av, aw);
 }
 
 // A heavy particle's list shared by the VL_GROUP lanes of a group: lane `sub` takes entries sub, sub + 8, sub + 16,
@@ -199,19 +207,22 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
 template <typename T, bool FOLD>
 __device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* __restrict__ lst, size_t stride, int n,
                                                 int sub, const Vec4<T>* __restrict__ r, const Vec4<T>& ri,
-                                                Acc<T, false>& av, Acc<T, false>& aw)
+                                                const int (&j0)[4], Acc<T, false>& av, Acc<T, false>& aw)
 {
     const bool px = FOLD && p.bc[0] == BC_PERIODIC, py = FOLD && p.bc[1] == BC_PERIODIC, pz = FOLD && p.bc[2] == BC_PERIODIC;
+    int jn[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) jn[u] = sub + VL_GROUP * u < n ? j0[u] : -1;
     for (int k = 0; k < n; k += 4 * VL_GROUP) {
         int j[4];
         Vec4<T> rj[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int kk = k + sub + VL_GROUP * u;
-            j[u] = kk < n ? lst[(size_t)kk * stride] : -1;
-        }
+        for (int u = 0; u < 4; ++u) { j[u] = jn[u]; rj[u] = r[max(j[u], 0)]; }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) rj[u] = r[max(j[u], 0)];
+        for (int u = 0; u < 4; ++u) {
+            const int kk = k + 4 * VL_GROUP + sub + VL_GROUP * u;
+            jn[u] = kk < n ? lst[(size_t)kk * stride] : -1;
+        }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
@@ -222,20 +233,35 @@ __device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* _
     }
 }
 
+// What a thread keeps in registers across the grid barrier while it owns the same particle from step to step (the
+// particles fit one wave, no rebuild in between): the position and velocity it has just written and the static head
+// of the list, so that the next phase starts with the neighbours' position loads instead of a round trip of its own;
+// likewise the particle, list head and (lane 0) velocity of the lane group's first heavy particle.
+template <typename T>
+struct Carry {
+    Vec4<T> r;
+    T vx, vy, vz;
+    int raw, j0[VL_BATCH];
+    bool valid = false;
+    int nh, hi, hraw, hj[4];
+    T hvx, hvy, hvz;
+    bool nhvalid = false, hvalid = false;
+};
+
 // ---- phase: [forces] -> [kick completing the step] -> [kick + drift of the next step] -----------
 // force: compute f from the list (else use the stored f(t));  kick: complete the current step (F3);
 // drift: start the next step (F2).
 template <typename T>
 __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& v, int c, int cv, bool force,
                                            bool kick, bool drift, int req, int gtid, int gthreads,
-                                           T lam = T(1), double* ksum = nullptr)
+                                           T lam, double* ksum, Carry<T>& cy, const bool cyon)
 {
     const Vec4<T>* __restrict__ rcur = v.st[c].r;
     Vec4<T>* __restrict__ rnew = v.st[c ^ 1].r;
     const State<T>& s = v.st[cv];
     double kacc = 0.0;
-    // F3 / F2 of particle i once its force is known (v already carries F4's factor)
-    auto integrate = [&](int i, const Vec4<T>& ri, T vx, T vy, T vz, T fx, T fy, T fz) {
+    // F3 / F2 of particle i once its force is known (v already carries F4's factor); v and rn return what was stored
+    auto integrate = [&](int i, const Vec4<T>& ri, T& vx, T& vy, T& vz, T fx, T fy, T fz, Vec4<T>& rn) {
         if (kick) {                                    // F3: v(t) = v(t - dt/2) + (dt/2m) f(t)
             vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
         }
@@ -243,7 +269,6 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         if (drift) {                                   // F2: v(t + dt/2), r(t + dt)
             vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
             const T sx = p.dt * vx, sy = p.dt * vy, sz = p.dt * vz;
-            Vec4<T> rn;
             rn.x = ri.x + sx; rn.y = ri.y + sy; rn.z = ri.z + sz;
             if (p.prism) {
                 const T ro[3] = {ri.x, ri.y, ri.z};
@@ -263,20 +288,43 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         if (kick || drift || lam != T(1)) { s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz; }
     };
     for (int i = gtid; i < p.nv; i += gthreads) {
-        const Vec4<T> ri = rcur[i];
-        T vx = s.vx[i], vy = s.vy[i], vz = s.vz[i];      // issued early, consumed after the force loop
+        const bool kept = cyon && cy.valid;               // cyon only when this loop runs at most once
+        Vec4<T> ri;
+        T vx, vy, vz;
+        int raw = 0, j0[VL_BATCH];
+        if (kept) {
+            ri = cy.r; vx = cy.vx; vy = cy.vy; vz = cy.vz; raw = cy.raw;
+#pragma unroll
+            for (int u = 0; u < VL_BATCH; ++u) j0[u] = cy.j0[u];
+        } else {
+            ri = rcur[i];
+            vx = s.vx[i]; vy = s.vy[i]; vz = s.vz[i];    // issued early, consumed after the force loop
+#pragma unroll
+            for (int u = 0; u < VL_BATCH; ++u) j0[u] = force ? v.nbr[(size_t)u * v.stride + i] : 0;   // in flight together
+            if (force) raw = v.ncnt[i];
+        }
         vx = lam * vx; vy = lam * vy; vz = lam * vz;     // F4 of the step just completed (lam = 1 without thermostat)
         T fx, fy, fz;
         if (force) {
-            if (v.ncnt[i] & VL_HEAVY) continue;          // the whole particle belongs to a lane group below
+            if (raw & VL_HEAVY) {                        // the whole particle belongs to a lane group below
+                if (cyon) { cy.raw = raw; cy.valid = drift; }
+                continue;
+            }
             Acc<T, false> av, aw;
-            list_force<T, false>(p, v, rcur, i, ri, av, aw);
+            list_force<T, false>(p, v, rcur, i, ri, raw, j0, av, aw);
             fx = av.fx + aw.fx; fy = av.fy + aw.fy; fz = av.fz + aw.fz;
             v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz;
         } else {
             fx = v.f.fx[i]; fy = v.f.fy[i]; fz = v.f.fz[i];
         }
-        integrate(i, ri, vx, vy, vz, fx, fy, fz);
+        Vec4<T> rn = ri;
+        integrate(i, ri, vx, vy, vz, fx, fy, fz, rn);
+        if (cyon && force) {
+            cy.r = rn; cy.vx = vx; cy.vy = vy; cy.vz = vz; cy.raw = raw;
+#pragma unroll
+            for (int u = 0; u < VL_BATCH; ++u) cy.j0[u] = j0[u];
+            cy.valid = drift;
+        }
     }
     if (force) {
         // Heavy particles (list longer than heavy_t: next to a wall, inside a cluster): one per group of VL_GROUP
@@ -284,7 +332,12 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         // barrier.  Group slots are numbered so that the blocks past the last particle (idle when the particles
         // fill less than one wave) take this work first and the rest is dealt round-robin over the other blocks,
         // one group per block and warp at a time.
-        const int nh = min(v.flags[VF_NHEAVY], v.flags[VF_HCAP]);
+        int nh;
+        if (cyon && cy.nhvalid) nh = cy.nh;
+        else {
+            nh = min(v.flags[VF_NHEAVY], v.flags[VF_HCAP]);
+            if (cyon) { cy.nh = nh; cy.nhvalid = true; }
+        }
         const int lane = threadIdx.x & 31, sub = lane & (VL_GROUP - 1);
         const unsigned gmask = ((1u << VL_GROUP) - 1u) << (lane & ~(VL_GROUP - 1));
         constexpr int GPW = 32 / VL_GROUP, GPB = VL_THREADS / VL_GROUP;         // groups per warp, per block
@@ -292,13 +345,24 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         const int b = blockIdx.x, q = (lane / VL_GROUP) * (VL_THREADS / 32) + (threadIdx.x >> 5);
         const int slot = b >= nbl ? (b - nbl) + nsp * ((threadIdx.x >> 5) * GPW + lane / VL_GROUP) : nsp * GPB + q * nbl + b;
         for (int h = slot; h < nh; h += gthreads / VL_GROUP) {
-            const int i = v.cell[h], raw = v.slot[h];
-            const Vec4<T> ri = rcur[i];
+            const bool first = h == slot, kept = cyon && first && cy.hvalid;
+            int i, raw, j0[4];
             T vx = T(0), vy = T(0), vz = T(0);
-            if (sub == 0) { vx = lam * s.vx[i]; vy = lam * s.vy[i]; vz = lam * s.vz[i]; }
+            if (kept) {
+                i = cy.hi; raw = cy.hraw; vx = cy.hvx; vy = cy.hvy; vz = cy.hvz;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) j0[u] = cy.hj[u];
+            } else {
+                i = v.cell[h]; raw = v.slot[h];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) j0[u] = v.nbr[(size_t)(sub + VL_GROUP * u) * v.stride + i];
+                if (sub == 0) { vx = s.vx[i]; vy = s.vy[i]; vz = s.vz[i]; }
+            }
+            const Vec4<T> ri = rcur[i];
+            vx = lam * vx; vy = lam * vy; vz = lam * vz;
             Acc<T, false> av, aw;
-            if (raw & VL_FOLD) list_loop_group<T, true>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, av, aw);
-            else list_loop_group<T, false>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, av, aw);
+            if (raw & VL_FOLD) list_loop_group<T, true>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, j0, av, aw);
+            else list_loop_group<T, false>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, j0, av, aw);
             T fx = av.fx + aw.fx, fy = av.fy + aw.fy, fz = av.fz + aw.fz;
 #pragma unroll
             for (int o = 1; o < VL_GROUP; o <<= 1) {
@@ -308,7 +372,14 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             }
             if (sub == 0) {
                 v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz;
-                integrate(i, ri, vx, vy, vz, fx, fy, fz);
+                Vec4<T> rn = ri;
+                integrate(i, ri, vx, vy, vz, fx, fy, fz, rn);
+            }
+            if (cyon && first) {
+                cy.hi = i; cy.hraw = raw; cy.hvx = vx; cy.hvy = vy; cy.hvz = vz;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) cy.hj[u] = j0[u];
+                cy.hvalid = drift;
             }
         }
     }
@@ -316,6 +387,15 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         kacc = warp_sum_d(kacc);
         if ((threadIdx.x & 31) == 0 && kacc != 0.0) atomicAdd(ksum, kacc);
     }
+}
+
+template <typename T>
+__device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& v, int c, int cv, bool force,
+                                           bool kick, bool drift, int req, int gtid, int gthreads,
+                                           T lam = T(1), double* ksum = nullptr)
+{
+    Carry<T> none;
+    phase_step<T>(p, v, c, cv, force, kick, drift, req, gtid, gthreads, lam, ksum, none, false);
 }
 
 // ---- rebuild phases (a2 inside the persistent kernel) -------------------------------------------
@@ -547,6 +627,8 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
     const int gthreads = gridDim.x * blockDim.x;
     int c = v.flags[VF_CUR], cv = v.flags[VF_CURV];
     bool rebuild = force_rebuild != 0;
+    Carry<T> carry;
+    const bool cyon = MINB == 2 && v.carry && !thermo && gthreads >= p.nv;      // (the 3-blocks-per-SM variant serves N > one wave)
     // lane groups in the blocks past the last particle (none once the particles fill the grid)
     const int hcap = max((int)gridDim.x - (p.nv + VL_THREADS - 1) / VL_THREADS, 0) * (VL_THREADS / VL_GROUP);
     unsigned long long t0 = gtid == 0 ? now_ns() : 0ull, t1;
@@ -574,6 +656,7 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
             if (gtid == 0) v.flags[VF_NREBUILD] += 1;
             grid_barrier(v.bar, bar_target);
             if (gtid == 0) { t1 = now_ns(); v.times[2] += t1 - t0; t0 = t1; v.times[7] += t1 - u0; }
+            carry.valid = carry.hvalid = carry.nhvalid = false;          // new particle order, new lists
         }
         if (s == n_steps) break;
         const int req = (int)(s % 3);
@@ -581,7 +664,7 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
         unsigned long long dbg0 = 0;
         if (v.dbg) dbg0 = now_ns();
         if (!thermo || s == 0) {
-            phase_step<T>(p, v, c, cv, s > 0, s > 0, true, req, gtid, gthreads);
+            phase_step<T>(p, v, c, cv, s > 0, s > 0, true, req, gtid, gthreads, T(1), nullptr, carry, cyon);
         } else {
             // with the thermostat lambda(t) needs K(t) of ALL particles before the next drift: the fused phase splits
             // into [F1 + F3 + K partial sums] | barrier | [F4 rescale + F2], one extra barrier per step
