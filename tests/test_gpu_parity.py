@@ -177,6 +177,27 @@ def test_config2_step0_brute_sample_and_cells():
     check_traj(cfg, "verlet", 100, cells_oracle=True)
 
 
+def test_config2_bench_launch_configuration_2000_steps():
+    """Full size, the launch bench.py times (MD_FORCE_VERLET, md_step(2000) = one persistent launch, then md_energy).
+    After 2000 steps trajectories are chaotic, so what holds at any size is checked: the step counter, energy
+    conservation (max-excursion reading of A8, bound 1e-3 K(0): a dropped or doubled pair term drifts far more) and
+    the oracle's K, U and pair counts at the same step within the 1/sqrt(N) fluctuation (2 %)."""
+    cfg = I.config2()
+    sim = md.Simulation(cfg, algo="verlet")
+    e0 = sim.energy()
+    sim.step(2000)
+    e1 = sim.energy()
+    assert e1["step"] == 2000
+    assert abs((e1["K"] + e1["U"]) - (e0["K"] + e0["U"])) <= 1e-3 * e0["K"]
+    ref = O.run(cfg, 2000, cells=True)
+    assert abs(e1["K"] - ref["K"]) <= 0.02 * ref["K"]
+    assert abs(e1["U"] - ref["U"]) <= 0.02 * abs(ref["U"])
+    f = O.forces(dict(cfg, pos=ref["pos"]), cells=True)
+    assert abs(e1["pairs_vv"] - f["pairs_vv"]) <= 0.02 * f["pairs_vv"]
+    assert abs(e1["pairs_vw"] - f["pairs_vw"]) <= 0.05 * f["pairs_vw"] + 50
+    sim.close()
+
+
 @pytest.mark.parametrize("shape", ["cone", "inkbottle", "slit"])
 def test_config3_shapes_step0(shape):
     cfg = I.config3(shape)
