@@ -188,7 +188,11 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
                                            Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
     const int* __restrict__ lst = v.nbr + i;
-    if (raw & VL_FOLD) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
+    // one loop per warp: if any lane's particle sits in a face cell every lane folds (the comparisons never fire
+    // for the others); a per-lane choice would run the two loops one after the other in most warps, because a
+    // warp's 32 cell-ordered particles span most of an x row and so nearly always include a face cell
+    const bool fold = __any_sync(__activemask(), (raw & VL_FOLD) != 0) || (raw & VL_FOLD);
+    if (fold) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
     else list_loop<T, ENERGY, false>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
 }
 
@@ -361,7 +365,8 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             const Vec4<T> ri = rcur[i];
             vx = lam * vx; vy = lam * vy; vz = lam * vz;
             Acc<T, false> av, aw;
-            if (raw & VL_FOLD) list_loop_group<T, true>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, j0, av, aw);
+            const bool fold = __any_sync(__activemask(), (raw & VL_FOLD) != 0) || (raw & VL_FOLD);
+            if (fold) list_loop_group<T, true>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, j0, av, aw);
             else list_loop_group<T, false>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, j0, av, aw);
             T fx = av.fx + aw.fx, fy = av.fy + aw.fy, fz = av.fz + aw.fz;
 #pragma unroll
