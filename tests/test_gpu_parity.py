@@ -240,8 +240,10 @@ def test_fp32_mode_forces():
 def test_energy_drift_and_long_run_statistics_dilute_gas(algo):
     # long runs are chaotic: compare the drift statistic (reading A8: wall-free dilute 3D gas, shifted energy,
     # |<E>_{9000..10000} - <E>_{1000..2000}| / K(0)) and the temperature with the oracle's, not trajectories
-    # N = 16384: the statistic is a random walk of r_c-crossing kinks whose relative size falls as 1/sqrt(N)
-    cfg = I.cylinder_config(16384, 4242, "drift", box=(16384 / 0.05) ** (1 / 3), length=0)
+    # The statistic is a random walk of r_c-crossing kinks whose relative size falls as 1/sqrt(N), and the GPU's
+    # summation order (atomics) makes every run another realisation of it: measured over 12 runs 2e-6 .. 7e-5 at
+    # N = 16384 (a tail beyond the 1e-4 bound) and 2e-7 .. 2e-5 at N = 65536, so the check runs at 65536
+    cfg = I.cylinder_config(65536, 4242, "drift", box=(65536 / 0.05) ** (1 / 3), length=0)
     sim = md.Simulation(cfg, algo=algo)
     e0 = sim.energy()
 
