@@ -219,11 +219,12 @@ def run_ours(args):
     if persistent:
         # one launch = prof_steps time steps of k_md_run (force from the list + both half-kicks + drift, and the
         # in-kernel re-bin / list rebuilds); algorithmic bytes per particle-step, fp64:
-        # r 32 + v 24 read, r' 32 + v' 24 + f 24 written, list count 4 + 4 per list entry read
+        # r 32 + v 24 read, r' 32 + v' 24 written (f is stored only by the last phase of a launch), list count 4 +
+        # 4 per list entry read
         prof_steps = 2000
         sim.profile_step(200)
         kt = sim.profile_step(prof_steps)
-        per_step = nv * (136 + 4) + 4 * tests
+        per_step = nv * (112 + 4) + 4 * tests
         top_name, t_top, alg = "k_md_run (persistent: %d time steps per launch)" % prof_steps, kt["ms"][3] * 1e-3, per_step * prof_steps
         shares = {"k_md_run": 1.0}
         # DRAM traffic of k_md_run from the committed ncu --set full capture (profiles/r01_v7_cfg2.md):

@@ -858,6 +858,8 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
     p.uc_vv = (T)ucut(lj.eps, lj.sigma);
     p.sig2_vw = (T)(lj.sigma_w * lj.sigma_w); p.e24_vw = (T)(24.0 * lj.eps_w); p.e4_vw = (T)(4.0 * lj.eps_w);
     p.uc_vw = (T)ucut(lj.eps_w, lj.sigma_w);
+    p.c12_vv = (T)(48.0 * lj.eps * pow(lj.sigma, 12)); p.c6_vv = (T)(24.0 * lj.eps * pow(lj.sigma, 6));
+    p.c12_vw = (T)(48.0 * lj.eps_w * pow(lj.sigma_w, 12)); p.c6_vw = (T)(24.0 * lj.eps_w * pow(lj.sigma_w, 6));
     p.dt = (T)o.dt; p.hk = (T)(o.dt / (2.0 * o.mass)); p.mass = o.mass;
     p.prism = pore && pore->kind == MD_PORE_PRISM;
     p.prism_axis = p.prism ? pore->axis : 0;

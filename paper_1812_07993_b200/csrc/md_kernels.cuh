@@ -21,6 +21,7 @@ struct Params {
     T rc2;
     T sig2_vv, e24_vv, e4_vv, uc_vv;
     T sig2_vw, e24_vw, e4_vw, uc_vw;
+    T c12_vv, c6_vv, c12_vw, c6_vw;       // 48 eps sigma^12, 24 eps sigma^6: g = (c12 / r^6 - c6) / r^8 (time loop)
     T dt, hk; // hk = dt / (2 m)
     double mass;
     double thermo_rate, t_target, dof;   // Berendsen F4: dt / tau_B (0 = off), T_0, dim * n_vapor

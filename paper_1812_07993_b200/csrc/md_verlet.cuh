@@ -125,6 +125,11 @@ __device__ __forceinline__ double rcp_fast(double x)
 }
 __device__ __forceinline__ float rcp_fast(float x) { return 1.0f / x; }
 
+// |step| rounded UP for the path-length bound: the fp32 square root with a 1e-6 margin covers its own and the
+// conversion's rounding and spares the FP64 pipe the ~10 instructions of a double-precision sqrt per particle-step.
+__device__ __forceinline__ double step_len(double s2) { return (double)(sqrtf((float)s2) * 1.000001f); }
+__device__ __forceinline__ float step_len(float s2) { return sqrtf(s2); }
+
 // Branch-free pair term: the four pairs of a batch form four independent dependency chains.
 template <typename T, bool ENERGY>
 __device__ __forceinline__ void pair_term_nb(const Params<T>& p, bool valid, bool wall, T dx, T dy, T dz,
@@ -133,10 +138,16 @@ __device__ __forceinline__ void pair_term_nb(const Params<T>& p, bool valid, boo
     const T r2 = fma_(dz, dz, fma_(dy, dy, dx * dx));
     const bool hit = valid && r2 < p.rc2;                   // strict, same r^2 arithmetic as every other path
     const T inv = rcp_fast(hit ? r2 : T(1));
-    const T s = (wall ? p.sig2_vw : p.sig2_vv) * inv;
-    const T s3 = s * s * s;
-    const T s6 = s3 * s3;
-    const T g = hit ? (wall ? p.e24_vw : p.e24_vv) * inv * (T(2) * s6 - s3) : T(0);
+    T s3, s6, g;
+    if (ENERGY) {
+        const T s = (wall ? p.sig2_vw : p.sig2_vv) * inv;
+        s3 = s * s * s;
+        s6 = s3 * s3;
+        g = hit ? (wall ? p.e24_vw : p.e24_vv) * inv * (T(2) * s6 - s3) : T(0);
+    } else {                                                // time loop: 5 instead of 7 operations after 1 / r^2
+        const T i3 = inv * inv * inv;
+        g = hit ? fma_(wall ? p.c12_vw : p.c12_vv, i3, -(wall ? p.c6_vw : p.c6_vv)) * i3 * inv : T(0);
+    }
     const T gw = wall ? g : T(0), gv = wall ? T(0) : g;
     if (ENERGY) {                                           // U_vv and U_vw are reported separately
         av.fx = fma_(gv, dx, av.fx); av.fy = fma_(gv, dy, av.fy); av.fz = fma_(gv, dz, av.fz);
@@ -289,7 +300,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             if (p.bc[0] == BC_REFLECT) boundary(rn.x, vx, p.L[0], BC_REFLECT, err);
             if (p.bc[1] == BC_REFLECT) boundary(rn.y, vy, p.L[1], BC_REFLECT, err);
             if (p.bc[2] == BC_REFLECT) boundary(rn.z, vz, p.L[2], BC_REFLECT, err);
-            rn.w = ri.w + sqrt(sx * sx + sy * sy + sz * sz);      // path length >= displacement
+            rn.w = ri.w + step_len(sx * sx + sy * sy + sz * sz); // path length >= displacement
             if (rn.w > v.half_skin) v.flags[VF_REQ0 + req] = 1;
             rnew[i] = rn;
         }
@@ -321,7 +332,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             Acc<T, false> av, aw;
             list_force<T, false>(p, v, rcur, i, ri, raw, j0, av, aw);
             fx = av.fx + aw.fx; fy = av.fy + aw.fy; fz = av.fz + aw.fz;
-            v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz;
+            if (!drift) { v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz; }   // f is read back only after a phase without drift
         } else {
             fx = v.f.fx[i]; fy = v.f.fy[i]; fz = v.f.fz[i];
         }
@@ -380,7 +391,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
                 fz += __shfl_xor_sync(gmask, fz, o);
             }
             if (sub == 0) {
-                v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz;
+                if (!drift) { v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz; }
                 Vec4<T> rn = ri;
                 integrate(i, ri, vx, vy, vz, fx, fy, fz, rn);
             }
