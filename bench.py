@@ -227,9 +227,9 @@ def run_ours(args):
         per_step = nv * (112 + 4) + 4 * tests
         top_name, t_top, alg = "k_md_run (persistent: %d time steps per launch)" % prof_steps, kt["ms"][3] * 1e-3, per_step * prof_steps
         shares = {"k_md_run": 1.0}
-        # DRAM traffic of k_md_run from the committed ncu --set full capture (profiles/r01_v7_cfg2.md):
-        # dram__bytes_read.sum + dram__bytes_write.sum = 11.93 MB for a 200-step launch = 59.6 KB per time step
-        traffic = 59.6e3 * prof_steps
+        # DRAM traffic of k_md_run from the committed ncu --set full capture (profiles/r01_v8_cfg2.md):
+        # dram__bytes_read.sum + dram__bytes_write.sum = 11.86 MB for a 200-step launch = 59.3 KB per time step
+        traffic = 59.3e3 * prof_steps
         extra = {"time_steps_per_launch": prof_steps, "rebuilds_in_launch": kt["rebuilds"],
                  "us_per_time_step": kt["ms"][3] * 1e3 / prof_steps}
     else:
