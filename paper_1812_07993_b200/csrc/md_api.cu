@@ -233,7 +233,7 @@ struct Sim : md_sim {
     // VERLET (persistent kernel): device-side buffer parities are mirrored here by refresh()
     md::Verlet<T> vl;
     int curv = 0, coop_grid = 0, coop_base = 0, coop_max = 0, heavy_seen = 0;
-    int minb3_threshold = getenv("MD_MINB3_THRESHOLD") ? atoi(getenv("MD_MINB3_THRESHOLD")) : 500000;
+    int minb3_threshold = getenv("MD_MINB3_THRESHOLD") ? atoi(getenv("MD_MINB3_THRESHOLD")) : -1;   // -1: set at the first launch
     long long rebuilds_seen = 0;
     unsigned long long phase_seen[4] = {0, 0, 0, 0}, phase_ns[4] = {0, 0, 0, 0};
 
@@ -255,6 +255,16 @@ struct Sim : md_sim {
 
     int launch_run(long long n, int force_rebuild)
     {
+        if (minb3_threshold < 0) {
+            // Two resident blocks per SM (128 registers, state carried in registers across the barrier) while the
+            // particles fit that grid with one thread each; beyond it three blocks of the 80-register variant:
+            // measured 13.4 vs 18.0 us per step at N = 80,000, 21.0 vs 23.9 at 2^17, 31.6 vs 34.4 at 2^18, 104 vs
+            // 127 at 2^20, and 12.1 vs 11.9 at 2^16 (profiles/r01_heavy_groups.md)
+            int dev = 0, sms = 0;
+            CK(cudaGetDevice(&dev));
+            CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            minb3_threshold = 2 * sms * md::VL_THREADS;
+        }
         const bool big = p.nv > minb3_threshold;
         void* kernel = dim == 3 ? (big ? (void*)md::k_md_run<T, 9, 3> : (void*)md::k_md_run<T, 9, 2>)
                                 : (big ? (void*)md::k_md_run<T, 3, 3> : (void*)md::k_md_run<T, 3, 2>);
