@@ -34,9 +34,13 @@ def measure(cfg, algo, precision, n_steps, torch, md, peaks):
     e = sim.energy()
     tests = sim.pair_tests()
     inter = 2 * e["pairs_vv"] + e["pairs_vw"]
-    row = dict(config=cfg["name"], n_vapor=cfg["n_vapor"], n_wall=cfg["n_wall"], algo=sim.info()["algo"], precision=precision,
+    nv, nw = cfg["n_vapor"], cfg["n_wall"]
+    # compulsory state traffic of a fully fused step: read r, v and write r', v' = 4 * dim reals per particle
+    state_bytes = 4 * cfg["dim"] * (precision // 8) * nv
+    row = dict(config=cfg["name"], n_vapor=nv, n_wall=nw, algo=sim.info()["algo"], precision=precision,
                steps_timed=n_steps, md_steps_per_s=1.0 / sec, pair_interactions_per_s=inter / sec,
-               pair_tests_per_s=tests / sec, us_per_step=sec * 1e6)
+               pair_tests_per_s=tests / sec, allpairs_equivalent_per_s=nv * (nv - 1.0 + nw) / sec, us_per_step=sec * 1e6,
+               state_gbs=state_bytes / sec * 1e-9, state_frac_of_copy_peak=state_bytes / sec * 1e-9 / peaks["copy_gbs"])
     if algo == "allpairs":
         flops = 7.0                                   # executed per test (1 add + 3 fma): DESIGN.md section 5
         peak = peaks["fp64_tflops"] if precision == 64 else peaks["fp32_tflops"]
@@ -50,6 +54,10 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", default="0,1,2,3,4,5", help="0-4: BASELINE.json configs; 5: the paper's problem sizes")
     ap.add_argument("--max-log2n", type=int, default=20)
+    ap.add_argument("--min-log2n", type=int, default=10)
+    ap.add_argument("--paths", default="allpairs,cells,verlet", help="force paths to run (subset)")
+    ap.add_argument("--precisions", default="64,32", help="config 4 precisions to run (subset)")
+    ap.add_argument("--steps", type=int, default=0, help="override the number of timed steps of every row (0: per-config defaults)")
     ap.add_argument("--json", default="")
     args = ap.parse_args()
     import torch
@@ -63,8 +71,13 @@ def main():
     want = {int(x) for x in args.configs.split(",")}
     rows = []
 
+    paths = set(args.paths.split(","))
+    precisions = {int(x) for x in args.precisions.split(",")}
+
     def add(cfg, algo, precision, n_steps):
-        r = measure(cfg, algo, precision, n_steps, torch, md, peaks)
+        if algo not in paths or precision not in precisions:
+            return
+        r = measure(cfg, algo, precision, args.steps or n_steps, torch, md, peaks)
         if r:
             rows.append(r)
             print("  %-22s %-8s fp%d  %10.0f steps/s" % (r["config"], r["algo"], precision, r["md_steps_per_s"]), file=sys.stderr)
@@ -94,7 +107,7 @@ def main():
                 add(cfg, algo, 64, 2000)
             add(I.paper_geometry(dim), "allpairs", 64, 2000)      # the paper's geometry, units and 2000 steps (NEXT-3)
     if 4 in want:
-        for log2n in range(10, args.max_log2n + 1, 2):
+        for log2n in range(args.min_log2n, args.max_log2n + 1, 2):
             cfg = I.config4(log2n)
             for precision in (64, 32):
                 for algo in ("cells", "verlet"):
@@ -104,13 +117,19 @@ def main():
                 add(cfg, "allpairs", precision, ap_steps)
     print("peaks measured in this run: FP64 %.1f TFLOP/s, FP32 %.1f TFLOP/s, copy %.0f GB/s\n" %
           (peaks["fp64_tflops"], peaks["fp32_tflops"], peaks["copy_gbs"]))
-    print("| config | N_v | N_w | path | fp | steps timed | MD steps/s | pair-interactions/s | pair tests/s | ALU TFLOP/s (frac of measured peak) |")
-    print("|---|---|---|---|---|---|---|---|---|---|")
+    print("Rates (SURVEY 8(d)): pair-interactions/s = ordered within-cut-off evaluations; pair tests/s = ordered distance tests "
+          "executed; all-pairs-equivalent/s = N_v (N_v - 1 + N_w) x steps/s (comparable with the paper's derived 1-2.8e9); "
+          "state GB/s = compulsory bytes of a fully fused step (read r, v; write r', v': 96 B per particle in 3D fp64) x steps/s, "
+          "against the device-copy GB/s measured in this run.\n")
+    print("| config | N_v | N_w | path | fp | steps timed | MD steps/s | us/step | pair-interactions/s | pair tests/s | all-pairs-equivalent/s | "
+          "state GB/s (frac of copy peak) | ALU TFLOP/s (frac of measured peak) |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     for r in rows:
         alu = "%.2f (%.3f)" % (r["alu_tflops"], r["alu_frac_of_measured_peak"]) if "alu_tflops" in r else ""
-        print("| %s | %d | %d | %s | %d | %d | %.4g | %.4g | %.4g | %s |" %
+        print("| %s | %d | %d | %s | %d | %d | %.4g | %.4g | %.4g | %.4g | %.4g | %.1f (%.3f) | %s |" %
               (r["config"], r["n_vapor"], r["n_wall"], r["algo"], r["precision"], r["steps_timed"], r["md_steps_per_s"],
-               r["pair_interactions_per_s"], r["pair_tests_per_s"], alu))
+               r["us_per_step"], r["pair_interactions_per_s"], r["pair_tests_per_s"], r["allpairs_equivalent_per_s"],
+               r["state_gbs"], r["state_frac_of_copy_peak"], alu))
     if args.json:
         with open(args.json, "w") as fh:
             json.dump(dict(peaks=peaks, rows=rows), fh)

@@ -33,29 +33,53 @@ def make_sim(cfg, algo, precision=64):
         raise
 
 
-def check_step0(cfg, algo, ref=None, precision=64, ftol=FTOL):
+def _cutoff_bracket(cfg, cells):
+    """fp32 mode takes the strict r^2 < r_c^2 decision in fp32 (the kernel's precision), the oracle in fp64: a pair whose
+    r^2 lies within the fp32 rounding of r_c^2 (three roundings of 2^-24 in the fma chain; the differences themselves are
+    exact) may fall on either side, and the force jumps by 0.039 eps/sigma there.  The oracle evaluated with
+    r_c (1 -+ 2e-7) brackets every such decision: particles whose oracle force differs between the two are the
+    ambiguous ones (about one pair in 2e6 at density 0.05)."""
+    lo = O.forces(dict(cfg, r_cut=cfg["r_cut"] * (1 - 2e-7)), cells=cells)
+    hi = O.forces(dict(cfg, r_cut=cfg["r_cut"] * (1 + 2e-7)), cells=cells)
+    amb = (lo["f"] != hi["f"]).any(axis=1)
+    return lo, hi, amb
+
+
+def check_step0(cfg, algo, ref=None, precision=64, ftol=FTOL, bracket=None):
     sim = make_sim(cfg, algo, precision)
     ref = ref if ref is not None else O.forces(cfg, cells=cfg["n_vapor"] > 20000)
     st = sim.get_state()
     en = sim.energy()
     assert sim.info()["algo"] == algo
     assert np.array_equal(st["pos"], cfg["pos"]) or precision == 32
-    assert en["pairs_vv"] == ref["pairs_vv"] and en["pairs_vw"] == ref["pairs_vw"]
-    assert force_error(st["f"], ref["f"]) <= ftol
-    assert scalar_error(st["pe"], ref["pe"]) <= ftol
     k_ref = O.kinetic(cfg, cfg["vel"])
-    assert abs(en["K"] - k_ref) <= 1e-12 * k_ref or precision == 32
     scale = max(abs(ref["U"]), k_ref)
+    if bracket is None:
+        assert en["pairs_vv"] == ref["pairs_vv"] and en["pairs_vw"] == ref["pairs_vw"]
+        assert force_error(st["f"], ref["f"]) <= ftol
+        assert scalar_error(st["pe"], ref["pe"]) <= ftol
+    else:
+        # fp32 mode: counts inside the bracket; unambiguous particles against the oracle, ambiguous ones against
+        # whichever side of the bracket the kernel's fp32 decision took
+        lo, hi, amb = bracket
+        assert lo["pairs_vv"] <= en["pairs_vv"] <= hi["pairs_vv"] and lo["pairs_vw"] <= en["pairs_vw"] <= hi["pairs_vw"]
+        ok = ~amb
+        assert force_error(st["f"][ok], ref["f"][ok]) <= ftol
+        assert scalar_error(st["pe"][ok], ref["pe"][ok]) <= ftol
+        for i in np.nonzero(amb)[0]:
+            assert min(force_error(st["f"][i:i + 1], side["f"][i:i + 1]) for side in (lo, hi)) <= 10 * ftol
+    assert abs(en["K"] - k_ref) <= 1e-12 * k_ref or precision == 32
     assert abs(en["U"] - ref["U"]) <= ftol * scale
     assert abs(en["U_vw"] - ref["U_vw"]) <= ftol * scale
-    assert abs(en["virial"] - ref["vir"].sum()) <= ftol * max(abs(ref["vir"].sum()), k_ref)
+    vir_amb = 0.0 if bracket is None else 0.1 * 2.5 * max(1, int(bracket[2].sum()))   # g r^2 = 0.039 * 2.5 per flipped pair
+    assert abs(en["virial"] - ref["vir"].sum()) <= ftol * max(abs(ref["vir"].sum()), k_ref) + vir_amb
     sim.close()
     return ref
 
 
-def check_traj(cfg, algo, n_steps=100, cells_oracle=False, chunks=(37, 63)):
+def check_traj(cfg, algo, n_steps=100, cells_oracle=False, chunks=(37, 63), ref=None):
     sim = make_sim(cfg, algo)
-    ref = O.run(cfg, n_steps, cells=cells_oracle)
+    ref = ref if ref is not None else O.run(cfg, n_steps, cells=cells_oracle)
     assert sum(chunks) == n_steps
     for c in chunks:                      # odd + odd chunk sizes exercise both graph parities
         sim.step(c)
@@ -85,7 +109,10 @@ def test_config0_forces_and_trajectory(algo):
     (3, (8.0, 9.3, 7.6), (0, 0, 0), 40, 1), (3, (8.1, 7.5, 5.2), (0, 0, 1), 40, 2), (3, (4.0, 8.0, 8.0), (1, 0, 0), 0, 3),
     (2, (13.7, 9.9), (0, 1), 12, 4), (2, (7.5, 7.5), (0, 0), 12, 5), (2, (2.6, 30.0), (1, 0), 5, 6),
     (3, (3.0, 3.0, 3.0), (1, 1, 1), 2, 7), (3, (9.6, 10.5, 9.9), (0, 0, 0), 30, 8), (3, (9.5, 9.6, 5.2), (0, 0, 1), 30, 9),
-    (2, (12.0, 9.6), (0, 0), 10, 10)])
+    (2, (12.0, 9.6), (0, 0), 10, 10),
+    # a periodic length in [2 r_c, 2.2 r_c): more than one image per dimension can sit within r_c + margin of a face,
+    # so all-pairs runs the per-pair minimum-image kernel k_force_allpairs (cells / verlet: box too small, skipped)
+    (3, (5.2, 9.0, 8.0), (0, 0, 0), 20, 13), (2, (5.3, 12.0), (0, 0), 8, 14), (3, (5.05, 5.4, 5.49), (0, 0, 0), 6, 15)])
 @pytest.mark.parametrize("algo", ALGOS)
 def test_small_ragged_cases(dim, box, bc, nw, seed, algo):
     vol = float(np.prod(box))
@@ -210,11 +237,15 @@ def test_verlet_three_blocks_per_sm_variant_trajectory(n_vapor):
 
 
 @pytest.mark.parametrize("shape", ["cone", "inkbottle", "slit"])
-def test_config3_shapes_step0(shape):
+def test_config3_shapes_step0_and_100_steps(shape):
+    # BASELINE.json configs[3]: 262,144 vapor particles, three pore shapes; oracle = its CPU cell-list variant
     cfg = I.config3(shape)
     ref = O.forces(cfg, cells=True)
     check_step0(cfg, "cells", ref=ref)
     check_step0(cfg, "verlet", ref=ref)
+    traj = O.run(cfg, 100, cells=True)
+    check_traj(cfg, "cells", 100, ref=traj)
+    check_traj(cfg, "verlet", 100, ref=traj)
 
 
 @pytest.mark.parametrize("log2n", [10, 12, 14])
@@ -228,23 +259,40 @@ def test_config4_sizes_both_kernels(log2n):
     check_traj(cfg, "verlet", 100, cells_oracle=True)
 
 
-def test_config4_2p20_cells_step0():
-    cfg = I.config4(20)
+@pytest.mark.parametrize("log2n", [16, 18, 20])
+def test_config4_large_sizes_all_paths(log2n):
+    # BASELINE.json configs[4] with its own seeds: step 0 on all three paths (all-pairs at 2^20: 1.1e12 tests per
+    # evaluation), 100-step trajectories on the two cell-based paths (and all-pairs at 2^16: 4.4e9 tests per step)
+    cfg = I.config4(log2n)
     ref = O.forces(cfg, cells=True)
-    check_step0(cfg, "cells", ref=ref)
-    check_step0(cfg, "verlet", ref=ref)
+    for algo in ALGOS:
+        check_step0(cfg, algo, ref=ref)
+    traj = O.run(cfg, 100, cells=True)
+    check_traj(cfg, "cells", 100, ref=traj)
+    check_traj(cfg, "verlet", 100, ref=traj, chunks=(1, 42, 57))
+    if log2n == 16:
+        check_traj(cfg, "allpairs", 100, ref=traj)
 
 
-def test_fp32_mode_forces():
-    # reading A12: fp32 state/arithmetic; compared with the oracle fed the same float-rounded inputs
-    cfg = I.config4(12)
+def _float_rounded(cfg, keys=("pos", "wall")):
     c32 = dict(cfg)
-    c32["pos"] = cfg["pos"].astype(np.float32).astype(np.float64)
-    c32["wall"] = cfg["wall"].astype(np.float32).astype(np.float64)
+    for k in keys:
+        c32[k] = cfg[k].astype(np.float32).astype(np.float64)
     c32["box_len"] = [float(np.float32(x)) for x in cfg["box_len"]]
-    ref = O.forces(c32)
+    return c32
+
+
+@pytest.mark.parametrize("log2n", [12, 16, 20])
+def test_fp32_mode_forces(log2n):
+    # reading A12: fp32 state/arithmetic; compared with the oracle fed the same float-rounded inputs.  BASELINE.json
+    # configs[4] runs every size in fp32 too: in the 276 sigma box of 2^20 one ulp of a coordinate is 3e-5 sigma, so the
+    # <= 1e-4 bound only holds because differences are formed exactly (image shift on the particle at the top of the box)
+    cfg = I.config4(log2n)
+    c32 = _float_rounded(cfg)
+    ref = O.forces(c32, cells=log2n > 14)
+    bracket = _cutoff_bracket(c32, cells=log2n > 14)
     for algo in ("cells", "allpairs", "verlet"):
-        check_step0(c32, algo, ref=ref, precision=32, ftol=1e-4)
+        check_step0(c32, algo, ref=ref, precision=32, ftol=1e-4, bracket=bracket)
 
 
 @pytest.mark.parametrize("algo", ["cells", "verlet"])
@@ -385,10 +433,7 @@ def test_fp32_trajectory_stays_close(algo):
     # fp32 mode over 100 steps against the fp64 oracle on the float-rounded input: rounding of the state
     # (ulp(L) ~ 4e-6 per step in position) bounds the agreement, not the force law
     cfg = I.config4(12)
-    c32 = dict(cfg)
-    for k in ("pos", "wall", "vel"):
-        c32[k] = cfg[k].astype(np.float32).astype(np.float64)
-    c32["box_len"] = [float(np.float32(x)) for x in cfg["box_len"]]
+    c32 = _float_rounded(cfg, ("pos", "wall", "vel"))
     ref = O.run(c32, 100, cells=True)
     sim = make_sim(c32, algo, precision=32)
     sim.step(100)
@@ -532,4 +577,115 @@ def test_paper_geometry_and_units_match_oracle(dim):
     st = sim.get_state()
     assert traj_error(st["pos"], ref["pos"], cfg["box_len"], cfg["bc"]) <= TRAJ_TOL
     assert np.abs(st["vel"] - ref["vel"]).max() <= 1e-7
+    sim.close()
+
+
+def _nonunit(cfg, sig=1.3, eps=0.7, sig_w=1.1, eps_w=1.6, mass=2.5, r_cut=3.0):
+    """cfg with its geometry scaled by sig and every model parameter away from 1 (m_i, sigma, eps are
+    parameters).  r_cut and sigma_w are NOT the scaled values, so this is not the reduced-unit system in disguise."""
+    c = dict(cfg, pos=cfg["pos"] * sig, wall=cfg["wall"] * sig, box_len=[x * sig for x in cfg["box_len"]],
+             sigma=sig, eps=eps, sigma_w=sig_w, eps_w=eps_w, mass=mass, r_cut=r_cut)
+    if cfg.get("pore"):
+        pd = dict(cfg["pore"])
+        pd["center"] = [x * sig for x in pd["center"]]
+        for k in ("length", "r0", "width"):
+            if k in pd:
+                pd[k] = pd[k] * sig
+        c["pore"] = pd
+    return c
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("thermostat", [False, True])
+def test_parameters_away_from_one(algo, thermostat):
+    """mass = 2.5, sigma = 1.3, eps = 0.7, sigma_w = 1.1, eps_w = 1.6, r_cut = 3: the first time the time loop's own
+    coefficients (c12 = 48 eps sigma^12, c6 = 24 eps sigma^6), hk = dt / 2m, K = m v^2 / 2 and the thermostat's
+    temperature see anything but 1 (the oracle's side is pinned by tests/test_oracle_pins.py::test_scaled_* and
+    ::test_dimensional_scaling_*)."""
+    extra = dict(tau_b=0.08, t_target=0.7) if thermostat else {}
+    for base, cells in ((I.config4(12), True), (I.small_case(2, 90, (13.7, 9.9), (0, 1), n_wall=12, seed=4, min_sep=0.9), False),
+                        (I.small_case(3, 200, (9.6, 10.5, 9.9), (0, 0, 1), n_wall=30, seed=8, min_sep=0.9), False)):
+        cfg = dict(_nonunit(base), **extra)
+        check_step0(cfg, algo, ref=O.forces(cfg, cells=cells))
+        ref = O.run(cfg, 100, cells=cells)
+        sim = make_sim(cfg, algo)
+        for c in (1, 36, 63):
+            sim.step(c)
+        st, en = sim.get_state(), sim.energy()
+        assert traj_error(st["pos"], ref["pos"], cfg["box_len"], cfg["bc"]) <= TRAJ_TOL
+        assert np.abs(st["vel"] - ref["vel"]).max() <= 1e-7
+        scale = max(abs(ref["U"]), ref["K"])
+        assert abs(en["K"] - ref["K"]) <= 1e-8 * scale and abs(en["U"] - ref["U"]) <= 1e-8 * scale
+        if cfg.get("pore"):                                  # K with the mass in it also feeds the pressure monitor
+            pr = sim.pressure()
+            p_box, p_pore, n_pore = _oracle_pressure(cfg, ref)
+            assert pr["n_pore"] == n_pore and abs(pr["P_box"] - p_box) <= 1e-7 * abs(p_box)
+        sim.close()
+
+
+def _drift_statistic(e, k0):
+    """Reading A8: (<E> over the last 1000 steps - <E> over steps 1000..2000) / K(0), signed."""
+    return (e[-1000:].mean() - e[1000:2000].mean()) / k0
+
+
+def test_energy_drift_distribution_matches_oracle_over_seeds():
+    """Reading A8 over several realisations instead of one pass/fail: the plainly truncated force makes every r_c
+    crossing a small energy kink, so the statistic is a zero-mean random walk whose rms falls as 1/sqrt(N) (oracle, 8
+    seeds each: rms 1.6e-4 at N = 1728, 1.1e-4 at N = 4096; A8).  GPU (Verlet path) and oracle are run on the
+    same 8 seeded inputs at N = 4096; trajectories decorrelate (chaos), so the two sets of 8 values are compared as
+    samples of one distribution: rms within a factor 3 of each other and of the 6.4e-3 / sqrt(N) law, no systematic
+    sign."""
+    n, seeds = 4096, range(4242, 4250)
+    gpu, orc = [], []
+    for seed in seeds:
+        cfg = I.cylinder_config(n, seed, "drift", box=(n / 0.05) ** (1 / 3), length=0)
+        h = O.run(cfg, 10000, cells=True, history=True)["hist"]
+        orc.append(_drift_statistic(h[:, 0] + h[:, 1] + h[:, 2], h[0, 0]))
+        sim = md.Simulation(cfg, algo="verlet")
+        k0 = sim.energy()["K"]
+        e = np.zeros(10001)                                  # E at steps 1000..1999 and 9001..10000, as the statistic reads
+        sim.step(1000)
+        for s in range(1000, 2000):
+            en = sim.energy()
+            e[s] = en["K"] + en["U"]
+            sim.step(1)
+        sim.step(7001)
+        for s in range(9001, 10001):
+            en = sim.energy()
+            e[s] = en["K"] + en["U"]
+            assert en["step"] == s
+            if s < 10000:
+                sim.step(1)
+        assert sim.energy()["step"] == 10000
+        gpu.append(_drift_statistic(e, k0))
+        sim.close()
+    gpu, orc = np.array(gpu), np.array(orc)
+    rms_g, rms_o, law = np.sqrt((gpu ** 2).mean()), np.sqrt((orc ** 2).mean()), 6.4e-3 / np.sqrt(n)
+    assert law / 3 <= rms_o <= 3 * law and law / 3 <= rms_g <= 3 * law and rms_o / 3 <= rms_g <= 3 * rms_o, (gpu, orc)
+    assert gpu.min() < 0 < gpu.max() and orc.min() < 0 < orc.max()               # a zero-mean random walk, not a trend
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_fp32_mode_monitors(algo):
+    # md_density_profile and md_pressure in fp32 mode: the histogram is integer work on the fp32 positions the handle
+    # itself reports (bit-exact); the pressure is compared with the oracle on the float-rounded input (<= 1e-4)
+    cfg = _float_rounded(I.config4(12), ("pos", "wall", "vel"))
+    sim = make_sim(cfg, algo, precision=32)
+    pr = sim.pressure()
+    ref = O.forces(cfg)
+    p_box, p_pore, n_pore = _oracle_pressure(cfg, dict(ref, pos=cfg["pos"], vel=cfg["vel"]))
+    assert pr["n_pore"] == n_pore
+    assert abs(pr["P_box"] - p_box) <= 1e-4 * abs(p_box) and abs(pr["P_pore"] - p_pore) <= 1e-4 * max(abs(p_pore), abs(p_box))
+    sim.step(37)
+    pos = sim.get_state(vel=False, force=False, pe=False)["pos"]
+    ax, ra = sim.density_profile(11, 10, 10.0)
+    pd = cfg["pore"]
+    L = np.array(cfg["box_len"])
+    d = pos - np.array(pd["center"])
+    rho = np.sqrt(d[:, 0] ** 2 + d[:, 1] ** 2)
+    inside = np.abs(d[:, 2]) < 0.5 * pd["length"]
+    ax_ref = np.bincount(np.clip(np.floor(pos[:, 2] / L[2] * 11).astype(int), 0, 10), minlength=11)
+    b = np.floor(rho / 10.0 * 10).astype(int)
+    ra_ref = np.bincount(b[inside & (b < 10)], minlength=10)
+    assert ax.sum() == cfg["n_vapor"] and np.array_equal(ax, ax_ref) and np.array_equal(ra, ra_ref)
     sim.close()

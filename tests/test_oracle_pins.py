@@ -297,14 +297,25 @@ def test_uniform_gas_pair_count_poisson():
 
 
 def test_energy_conservation_dilute_gas_10k_steps():
-    # reading A8: drift := |<E>_last1000 - <E>_{1000..2000}| / K(0) <= 1e-4 on the dilute 3D gas, shifted energy
-    cfg = I.cylinder_config(1728, 4242, "drift", box=(1728 / 0.05) ** (1 / 3), length=0)
-    assert cfg["n_wall"] == 0
-    h = O.run(cfg, 10000, cells=True, history=True)["hist"]
-    e = h[:, 0] + h[:, 1] + h[:, 2]
-    drift = abs(e[-1000:].mean() - e[1000:2000].mean()) / h[0, 0]
-    assert drift <= 1e-4, drift
-    assert np.abs(e - e[0]).max() / h[0, 0] < 1e-3
+    # reading A8: drift := (<E>_last1000 - <E>_{1000..2000}) / K(0) on the dilute 3D gas, shifted energy.  The force is
+    # plainly truncated (A2), so every r_c crossing leaves a small energy kink of either sign: the statistic is a
+    # zero-mean random walk whose rms over realisations falls as 1/sqrt(N) -- measured over 16 seeds at N = 1728: mean
+    # 5e-6, rms 1.5e-4 (rms sqrt(N) = 6.3e-3); 8 seeds at N = 4096: 1.1e-4.  north_star's "below 1e-4" is therefore a
+    # statement about large N (rms 2.5e-5 at the 65,536 particles of the metric's workload, checked on the GPU); a single
+    # realisation at N = 1728 (3.8e-5 for seed 4242) passing 1e-4 is luck, so the pin is on the distribution:
+    # six seeds, rms within a factor 3 of the law, both signs present, and no run wanders beyond 1e-3 K(0) at any step.
+    n, ds = 1728, []
+    for seed in range(4242, 4248):
+        cfg = I.cylinder_config(n, seed, "drift", box=(n / 0.05) ** (1 / 3), length=0)
+        assert cfg["n_wall"] == 0
+        h = O.run(cfg, 10000, cells=True, history=True)["hist"]
+        e = h[:, 0] + h[:, 1] + h[:, 2]
+        ds.append((e[-1000:].mean() - e[1000:2000].mean()) / h[0, 0])
+        assert np.abs(e - e[0]).max() / h[0, 0] < 1e-3
+    ds = np.array(ds)
+    rms, law = np.sqrt((ds ** 2).mean()), 6.4e-3 / math.sqrt(n)
+    assert law / 3 <= rms <= 3 * law, ds
+    assert ds.min() < 0 < ds.max(), ds
 
 
 def test_berendsen_thermostat_closed_forms():
@@ -378,3 +389,114 @@ def test_geometric_prism_pore_free_flight():
     h = O.run(lj, 2000, history=True)["hist"]
     e = h[:, 0] + h[:, 1] + h[:, 2]
     assert np.abs(e - e[0]).max() < 2e-3 * h[0, 0]
+
+
+# ---- parameters away from 1 (m_i, sigma and epsilon are parameters of the model) ---------------------
+# Every pin above runs with mass = sigma = eps = 1, where a slip such as hk = dt*m/2, K = v^2/2 or a wrong power of
+# sigma in g is invisible.  The pins below use m = 2.5, sigma = 1.3, eps = 0.7, sigma_w = 1.1, eps_w = 1.6.
+M, SIG, EPS, SIGW, EPSW = 2.5, 1.3, 0.7, 1.1, 1.6
+
+
+def test_scaled_parameters_pair_closed_form():
+    # U(r; eps, sigma) = eps U_1(r / sigma), F(r; eps, sigma) = (eps / sigma) F_1(r / sigma), virial = F r:
+    # golden rows (eps = sigma = 1) evaluated at r / sigma
+    for x, u1, f1 in golden_rows():
+        if x >= 2.5:
+            continue
+        for wall, eps, sig in ((False, EPS, SIG), (True, EPSW, SIGW)):
+            r = x * sig
+            fo, uo, out = pair(r, wall=wall, eps=EPS, sigma=SIG, eps_w=EPSW, sigma_w=SIGW, r_cut=4.0)
+            assert abs(uo - eps * u1) <= 4e-14 * max(1.0, abs(u1)), (x, wall)
+            assert abs(fo - eps / sig * f1) <= 4e-13 * max(1.0, abs(f1)), (x, wall)
+            w = out["vir"].sum()
+            assert abs(w - eps / sig * f1 * r) <= 1e-12 * max(1.0, abs(f1))
+    # zero force at r = 2^(1/6) sigma, for both pair types
+    for wall, sig in ((False, SIG), (True, SIGW)):
+        fo, _, _ = pair(2.0 ** (1.0 / 6.0) * sig, wall=wall, eps=EPS, sigma=SIG, eps_w=EPSW, sigma_w=SIGW, r_cut=4.0)
+        assert abs(fo) < 1e-13
+    # the shift is u(r_cut) of the same (eps, sigma): 4 eps [(sigma / r_c)^12 - (sigma / r_c)^6], by rational arithmetic
+    for wall, eps, sig in ((False, Fraction(7, 10), Fraction(13, 10)), (True, Fraction(8, 5), Fraction(11, 10))):
+        q = sig / Fraction(3)
+        uc = float(4 * eps * (q ** 12 - q ** 6))
+        kw = dict(wall=wall, eps=EPS, sigma=SIG, eps_w=EPSW, sigma_w=SIGW, r_cut=3.0)
+        _, u_un, _ = pair(2.0, shift_energy=0, **kw)
+        _, u_sh, _ = pair(2.0, shift_energy=1, **kw)
+        assert abs((u_un - u_sh) - uc) < 1e-15
+
+
+def test_kinetic_energy_and_first_step_with_mass():
+    # K = 1/2 m |v|^2 on hand-set velocities: 1/2 * 2.5 * (1 + 4 + 9) + 1/2 * 2.5 * 4 = 22.5
+    cfg = base_cfg(3, mass=M, pos=np.array([[5.0, 5.0, 5.0], [12.0, 5.0, 5.0]]), vel=np.array([[1.0, 2.0, 3.0], [0.0, -2.0, 0.0]]))
+    assert O.kinetic(cfg, cfg["vel"]) == 22.5
+    # one step from rest: v(dt/2) = (dt / 2m) F, r(dt) = r + dt v(dt/2) = r + dt^2 F / (2 m): F2 of PAPER.md:79-80 with
+    # a = F / m (Eq. (1)).  Two particles 1.5 sigma apart, eps = 0.7, sigma = 1.3.
+    r = 1.5 * SIG
+    f = EPS / SIG * golden_rows()[2][2]
+    dt = 0.005
+    cfg = base_cfg(3, mass=M, eps=EPS, sigma=SIG, r_cut=4.0, dt=dt, pos=np.array([[5.0 + r, 5.0, 5.0], [5.0, 5.0, 5.0]]),
+                   vel=np.zeros((2, 3)))
+    out = O.run(cfg, 1)
+    assert abs((out["pos"][0, 0] - (5.0 + r)) - dt * dt * f / (2 * M)) < 1e-15
+    assert abs((out["pos"][1, 0] - 5.0) + dt * dt * f / (2 * M)) < 1e-15
+    # after the step v(dt) = (dt / 2m)(F(0) + F(dt)), F(dt) from the closed form at the new separation
+    r1 = out["pos"][0, 0] - out["pos"][1, 0]
+    x = r1 / SIG
+    f_new = EPS / SIG * 24.0 * (2.0 * x ** -12 - x ** -6) / x
+    assert abs(out["vel"][0, 0] - dt / (2 * M) * (f + f_new)) < 1e-15
+
+
+def test_bound_pair_period_scales_with_mass_sigma_eps():
+    # omega = sqrt(U''(r_min) / mu), U''(r_min) = 72 * 2^(-1/3) eps / sigma^2: period proportional to sqrt(m sigma^2 / eps)
+    kpp = 72.0 * 2.0 ** (-1.0 / 3.0)
+    dt, delta = 0.005, 1e-3
+    for wall in (False, True):
+        eps, sig = (EPSW, SIGW) if wall else (EPS, SIG)
+        r0 = 2.0 ** (1.0 / 6.0) * sig
+        a = np.array([[5.0, 5.0, 5.0]])
+        b = np.array([[5.0 + r0 + delta, 5.0, 5.0]])
+        kw = dict(mass=M, eps=EPS, sigma=SIG, eps_w=EPSW, sigma_w=SIGW, r_cut=4.0, dt=dt)
+        if wall:
+            cfg = base_cfg(3, pos=b, vel=np.zeros((1, 3)), wall=a, **kw)
+            omega = math.sqrt(kpp * eps / sig ** 2 / M)
+        else:
+            cfg = base_cfg(3, pos=np.concatenate([a, b]), vel=np.zeros((2, 3)), **kw)
+            omega = math.sqrt(kpp * eps / sig ** 2 / (0.5 * M))
+        xs, pos, vel = [], cfg["pos"], cfg["vel"]
+        for _ in range(1400):
+            o = O.run(cfg, 1, pos=pos, vel=vel)
+            pos, vel = o["pos"], o["vel"]
+            xs.append(pos[-1, 0] - (5.0 if wall else pos[0, 0]))
+        T = _period(np.array(xs), dt)
+        assert abs(T - 2 * math.pi / omega) / T < 2e-3, (wall, T, 2 * math.pi / omega)
+
+
+def test_dimensional_scaling_maps_onto_reduced_units():
+    # Lengths x sigma, energies x eps, masses x m, times x sigma sqrt(m / eps): the run with (m, sigma, eps) on the
+    # scaled input is the reduced-unit run (which the pins above fix) scaled back.  Exact in real arithmetic, so the
+    # two differ by rounding only; any wrong power of m, sigma or eps in hk, K, g or u shows as an O(1) difference.
+    cfg = I.small_case(3, 120, (8.0, 9.0, 7.6), (0, 0, 1), n_wall=20, seed=31, min_sep=0.95)
+    cfg["eps_w"] = 1.6
+    tau = SIG * math.sqrt(M / EPS)
+    big = dict(cfg, pos=cfg["pos"] * SIG, wall=cfg["wall"] * SIG, vel=cfg["vel"] * SIG / tau,
+               box_len=[x * SIG for x in cfg["box_len"]], r_cut=cfg["r_cut"] * SIG, dt=cfg["dt"] * tau, mass=M,
+               eps=EPS, sigma=SIG, eps_w=1.6 * EPS, sigma_w=SIG)
+    n = 60
+    a, b = O.run(cfg, n, history=True), O.run(big, n, history=True)
+    assert np.abs(b["pos"] / SIG - a["pos"]).max() < 1e-9
+    assert np.abs(b["vel"] * tau / SIG - a["vel"]).max() < 1e-8
+    assert np.abs(b["f"] * SIG / EPS - a["f"]).max() <= 1e-8 * np.abs(a["f"]).max()
+    assert abs(b["K"] / EPS - a["K"]) < 1e-9 * a["K"] and abs(b["U"] / EPS - a["U"]) < 1e-9 * abs(a["U"])
+    assert np.array_equal(a["hist"][:, 3:], b["hist"][:, 3:])          # pair counts step by step
+    assert np.abs(b["vir"] / EPS - a["vir"]).max() < 1e-8 * np.abs(a["vir"]).max()
+    # and the thermostat's temperature uses K with the mass in it: T = 2K / (d N), same lambda in both unit systems
+    ta = O.run(dict(cfg, tau_b=0.05, t_target=0.5), n)
+    tb = O.run(dict(big, tau_b=0.05 * tau, t_target=0.5 * EPS), n)
+    assert np.abs(tb["vel"] * tau / SIG - ta["vel"]).max() < 1e-8
+
+
+def test_free_flight_is_independent_of_mass():
+    cfg = I.small_case(3, 40, (6.0, 7.0, 8.0), (0, 0, 1), n_wall=0, seed=3)
+    cfg["eps"] = cfg["eps_w"] = 0.0
+    a, b = O.run(cfg, 300), O.run(dict(cfg, mass=M), 300)
+    assert np.array_equal(a["pos"], b["pos"]) and np.array_equal(a["vel"], b["vel"])
+    assert abs(b["K"] - M * a["K"]) < 1e-12 * b["K"]
