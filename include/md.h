@@ -57,8 +57,8 @@ typedef struct { int dim; double len[3]; int bc[3]; } md_box;
  * |along - center[axis]| < length/2; MD_PORE_SLIT (2D): |r[axis] - center[axis]| < width/2 (axis = wall normal) and
  * |r[1-axis] - center[1-axis]| < length/2.  MD_PORE_PRISM switches on GEOMETRIC walls (the paper's own pore,
  * PAPER.md:115-121, :186): the axis-aligned box of size `length` along `axis` and `width` across, centred at `center`,
- * reflects particles specularly from both sides of every face except the open one at +axis; it must lie at least one
- * length unit inside the simulation box.  Other kinds are stored but neither monitored nor active. */
+ * reflects particles specularly from both sides of every face except the open one at +axis; it must lie at least
+ * max(1, skin) length units inside the simulation box.  Other kinds are stored but neither monitored nor active. */
 typedef struct { int kind, axis; double center[3], length, r0, r1, neck_len, width; } md_pore;
 
 /* 12-6 Lennard-Jones: u(r) = 4 eps [(sigma/r)^12 - (sigma/r)^6] for r < r_cut, else 0 (strict <);
@@ -75,10 +75,12 @@ typedef struct { double eps, sigma, eps_w, sigma_w, r_cut; int shift_energy; } m
  *             within r_cut is ever missed); the whole md_step batch is one persistent launch;
  *   AUTO      VERLET when the box holds >= 3 cells of side r_cut + skin per periodic dimension, else CELLS
  *             under the same rule with r_cut, else ALLPAIRS.
- * skin >= 0 is the VERLET list margin in length units; 0 selects the default 0.24 r_cut.
+ * 0 <= skin < r_cut is the VERLET list margin in length units; 0 selects the default 0.24 r_cut.
+ * heavy_list >= 0: VERLET lists of this many entries or more are walked by a group of four lanes instead of the
+ * particle's own thread (0 selects the default 13; a tuning knob, results do not depend on it).
  * tau_b > 0 switches on the Berendsen thermostat (the paper's kernel F4) after every step:
  * v <- lambda v, lambda = sqrt(1 + (dt / tau_b)(t_target / T - 1)), T = 2K / (dim n_vapor) (k_B = 1); tau_b <= 0: NVE. */
-typedef struct { double dt, mass; int precision, force_algo; double skin; double tau_b, t_target; } md_opts;
+typedef struct { double dt, mass; int precision, force_algo; double skin; double tau_b, t_target; int heavy_list; } md_opts;
 
 /* potential = potential_vv + potential_vw = sum_i pe_i; virial = sum over unordered vv pairs and
  * vw pairs of g.d (g = force on the vapor particle, d = r_i - r_j); pairs_* = pairs with r < r_cut. */
@@ -93,8 +95,10 @@ typedef struct { double pressure_box, volume_box, pressure_pore, volume_pore, ki
 
 /* Per-kernel device times of md_profile_step, milliseconds summed over the profiled steps, and
  * launch counts.  Index: 0 kick+drift(+bin count), 1 scan, 2 scatter, 3 force(+half-kick).  VERLET: the
- * whole batch is one launch, reported in slot 3; rebuilds = cell-list + neighbour-list rebuilds in it. */
-typedef struct { double ms[4]; long long launches[4]; double total_ms; long long steps, rebuilds; } md_kernel_times;
+ * whole batch is one launch, reported in slot 3 (slots 0-2: step phases, grid barriers, rebuilds as timed inside the
+ * kernel by its first thread); rebuilds = cell-list + neighbour-list rebuilds in it, rebuild_ms = their split into
+ * bin, scan, scatter and list build, each with the grid barrier that ends it (VERLET only, else 0). */
+typedef struct { double ms[4]; long long launches[4]; double total_ms; long long steps, rebuilds; double rebuild_ms[4]; } md_kernel_times;
 
 /* Peak micro-benchmarks run on the caller's stream (TFLOP/s count FMA = 2 flops; GB/s = read+write). */
 typedef struct { double fp64_tflops, fp32_tflops, copy_gbs; } md_peaks;
@@ -106,7 +110,7 @@ size_t md_workspace_bytes(const md_box*, const md_lj*, const md_opts*, long long
  * [n_wall][dim], may be NULL iff n_wall == 0), bins, evaluates f(0).  device_workspace: device
  * memory of >= md_workspace_bytes bytes, 256-byte aligned.  cuda_stream: a cudaStream_t (NULL =
  * default stream).  pore may be NULL.  Invalid: dim not 2/3, n_vapor < 1, n_wall < 0, dt <= 0,
- * mass <= 0, r_cut <= 0, non-finite or out-of-box positions, a periodic length < 2 r_cut, skin < 0, a thermostat
+ * mass <= 0, r_cut <= 0, non-finite or out-of-box positions, a periodic length < 2 r_cut, skin < 0 or >= r_cut, a thermostat
  * with tau_b < dt or t_target <= 0, a prism pore not inside the box.
  * MD_ERR_UNSUPPORTED: MD_FORCE_CELLS with a periodic dimension shorter than 3 cells (AUTO falls
  * back to all-pairs).  On failure *out = NULL and md_last_error(NULL) has the reason. */

@@ -17,6 +17,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
            "-Xcompiler", "-fPIC", "-shared"]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("MD_NVCC_FLAGS", "").split()       # e.g. -DMD_DIAGNOSTICS (debug timers, standalone phase kernels)
     cmd += SRCS + ["-o", LIB]
     subprocess.run(cmd, check=True)
     return LIB

@@ -72,6 +72,8 @@ const char* validate(const md_box* box, const md_lj* lj, const md_opts* o, long 
     if (o->precision != 64 && o->precision != 32) return "precision must be 64 or 32";
     if (o->force_algo < MD_FORCE_AUTO || o->force_algo > MD_FORCE_VERLET) return "unknown force_algo";
     if (!(o->skin >= 0) || !std::isfinite(o->skin)) return "skin must be >= 0";
+    if (o->skin >= lj->r_cut) return "skin must be < r_cut";
+    if (o->heavy_list < 0) return "heavy_list must be >= 0";
     if (!std::isfinite(o->tau_b) || !std::isfinite(o->t_target)) return "tau_b, t_target must be finite";
     if (o->tau_b > 0 && (o->tau_b < o->dt || !(o->t_target > 0))) return "thermostat needs tau_b >= dt and t_target > 0";
     if (!(lj->r_cut > 0) || !std::isfinite(lj->r_cut)) return "r_cut must be > 0";
@@ -118,6 +120,7 @@ struct Layout {
     md::State<T> st[2];
     md::Force<T> f;
     int *cell, *slot, *count, *start, *tile_sum;
+    unsigned long long* tile_agg;   // VERLET: in-kernel scan's published tile sums
     md::Vec4<T> *wr, *wtr;      // wall positions: cell order / caller's order
     int *wcell, *wslot, *wstart;
     uint8_t* wnear;
@@ -127,7 +130,9 @@ struct Layout {
     unsigned long long* tests;
     double *stage0, *stage1, *wstage;
     int *nbr, *ncnt, *vflags;   // VERLET: neighbour list, counts, flags
-    unsigned long long *vtimes, *vbar;
+    unsigned long long* vtimes;
+    unsigned long long* vbar;   // VERLET: grid-barrier arrival counter
+    md::F4* r32;                // VERLET fp64: fp32 shadow of the positions for the list build
     unsigned long long* hist;   // density-profile bins
     double* vksum;              // VERLET thermostat: rotating kinetic-energy accumulators
     md::Vec4<T> *jv, *jw;       // ALLPAIRS: j lists (entries + ghosts) of the dot-product kernels
@@ -137,8 +142,19 @@ struct Layout {
     size_t bytes;
 };
 
+// Image blocks of a VERLET position buffer (md_verlet.cuh): bit a of the block number = shifted in dimension a, so
+// the count is 1 + the sum of the periodic dimensions' bits; fp32 mode keeps block 0 only (it folds differences).
+int image_blocks(const md_box& box, int precision)
+{
+    int top = 0;
+    if (precision == 64)
+        for (int a = 0; a < box.dim; ++a)
+            if (box.bc[a] == MD_BC_PERIODIC) top |= 1 << a;
+    return top + 1;
+}
+
 template <typename T>
-Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell, int algo)
+Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell, int algo, int nimg)
 {
     Layout<T> l;
     Carver c(base);
@@ -146,7 +162,8 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     size_t n = (size_t)align_up((size_t)nv, 64);
     size_t m = (size_t)align_up((size_t)(nw > 0 ? nw : 1), 64);
     for (int b = 0; b < (cells ? 2 : 1); ++b) {
-        l.st[b].r = c.take<md::Vec4<T>>(verlet ? n + m : n);   // VERLET: walls appended at [nv, nv + nw)
+        // VERLET: nimg image blocks of nv + nw entries each (walls appended at [nv, nv + nw) of every block)
+        l.st[b].r = c.take<md::Vec4<T>>(verlet ? (size_t)nimg * (size_t)(nv + nw) + 64 : n);
         l.st[b].vx = c.take<T>(n); l.st[b].vy = c.take<T>(n); l.st[b].vz = c.take<T>(n);
         l.st[b].id = c.take<int>(n);
     }
@@ -173,6 +190,8 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.nbr = c.take<int>(verlet ? n * md::VL_MAXN : 1);
     l.ncnt = c.take<int>(verlet ? n : 1);
     l.vflags = c.take<int>(md::VF_COUNT);
+    l.r32 = c.take<md::F4>(verlet && sizeof(T) == 8 ? n + m : 1);
+    l.tile_agg = c.take<unsigned long long>(verlet ? (size_t)cdiv((long long)nc, md::SCAN_TILE) + 1 : 1);
     const bool dot = algo == MD_FORCE_ALLPAIRS;
     l.jv = c.take<md::Vec4<T>>(dot ? 8 * n : 1);          // <= 7 periodic images per particle
     l.jw = c.take<md::Vec4<T>>(dot ? 8 * m : 1);
@@ -203,6 +222,7 @@ struct md_sim {
     virtual void info(int* algo, int nc[3], int* kps) const = 0;
     virtual int pressure(md_pressure_out* out) = 0;
     virtual int density(int n_axial, long long* axial, int n_radial, double r_max, long long* radial) = 0;
+    virtual void drain() = 0;
     md_pore pore = {};
     md_box box = {};
 };
@@ -232,10 +252,10 @@ struct Sim : md_sim {
     double e_host[6];
     // VERLET (persistent kernel): device-side buffer parities are mirrored here by refresh()
     md::Verlet<T> vl;
-    int curv = 0, coop_grid = 0, coop_base = 0, coop_max = 0, heavy_seen = 0;
-    int minb3_threshold = getenv("MD_MINB3_THRESHOLD") ? atoi(getenv("MD_MINB3_THRESHOLD")) : -1;   // -1: set at the first launch
+    int curv = 0, coop_grid = 0, coop_base = 0, coop_max = 0, heavy_seen = 0, heavy32_seen = 0;
+    int minb3_threshold = -1;   // particles beyond which the 3-blocks-per-SM build runs; set at the first launch
     long long rebuilds_seen = 0;
-    unsigned long long phase_seen[4] = {0, 0, 0, 0}, phase_ns[4] = {0, 0, 0, 0};
+    unsigned long long phase_seen[8] = {}, phase_ns[8] = {};
 
     md::AllPairsDot ad;
     md::AllPairsDotF adf;
@@ -244,6 +264,7 @@ struct Sim : md_sim {
     int gpar = 0;               // which of the two ghost counters describes the current j list
 
     bool verlet() const { return algo == MD_FORCE_VERLET; }
+    void drain() override { cudaStreamSynchronize(stream); }
 
     // Particle state as the post-processing kernels see it (positions from `cur`, the rest from `curv`).
     md::State<T> view() const
@@ -255,6 +276,9 @@ struct Sim : md_sim {
 
     int launch_run(long long n, int force_rebuild)
     {
+#ifdef MD_DIAGNOSTICS
+        if (minb3_threshold < 0 && getenv("MD_MINB3_THRESHOLD")) minb3_threshold = atoi(getenv("MD_MINB3_THRESHOLD"));
+#endif
         if (minb3_threshold < 0) {
             // Two resident blocks per SM (128 registers, state carried in registers across the barrier) while the
             // particles fit that grid with one thread each; beyond it three blocks of the 80-register variant:
@@ -284,11 +308,15 @@ struct Sim : md_sim {
         // Blocks past the last particle serve the lane groups of the particles with long lists (the kernel hands
         // out only as many as those blocks hold: measured -13 % per step at 2^16 with them, +1..2 % at 2^18 and
         // 2^20 where the work would land on busy blocks, profiles/r01_heavy_groups.md): an eighth of the particle
-        // blocks, or what the last list this handle has seen asked for (refresh() mirrors the count) plus a quarter.
+        // blocks, or what the last list this handle has seen asked for (refresh() mirrors the counts) plus a quarter:
+        // four lanes per long list, a warp per VL_WARP_ROUNDS very long ones.
         const int light = cdiv(p.nv, md::VL_THREADS);
         coop_grid = coop_base;
-        if (light < coop_max)
-            coop_grid = std::min(coop_max, std::max(coop_base, light + std::max(light / 8, cdiv(heavy_seen * md::VL_GROUP * 5 / 4, md::VL_THREADS)) + 1));
+        if (light < coop_max) {
+            const int idle4 = cdiv(heavy_seen * md::VL_GROUP * 5 / 4, md::VL_THREADS);
+            const int idle32 = cdiv(heavy32_seen * 5 / 4, md::VL_WARP_ROUNDS * (md::VL_THREADS / 32));
+            coop_grid = std::min(coop_max, std::max(coop_base, light + std::max(light / 8, std::max(idle4, idle32)) + 1));
+        }
         CK(cudaMemsetAsync(l.vflags + md::VF_REQ0, 0, 3 * sizeof(int), stream));   // rebuild-request slots
         CK(cudaMemsetAsync(l.vbar, 0, 2 * sizeof(unsigned long long), stream));        // grid barrier counter
         CK(cudaMemsetAsync(l.vksum, 0, 4 * sizeof(double), stream));
@@ -305,7 +333,7 @@ struct Sim : md_sim {
         CK(cudaMemcpyAsync(h, l.vflags, sizeof(h), cudaMemcpyDeviceToHost, stream));
         CK(cudaStreamSynchronize(stream));
         CK(cudaGetLastError());
-        cur = h[md::VF_CUR]; curv = h[md::VF_CURV]; rebuilds_seen = h[md::VF_NREBUILD]; heavy_seen = h[md::VF_NHEAVY];
+        cur = h[md::VF_CUR]; curv = h[md::VF_CURV]; rebuilds_seen = h[md::VF_NREBUILD]; heavy_seen = h[md::VF_NHEAVY]; heavy32_seen = h[md::VF_NHEAVY32];
         if (h[md::VF_ESCAPE]) { err = "a particle left a reflecting box (more than one bounce in a step)"; return MD_ERR_STATE; }
         if (h[md::VF_OVERFLOW]) { err = "neighbour list overflow (> 128 neighbours within r_cut + skin)"; return MD_ERR_WORKSPACE; }
         return MD_OK;
@@ -469,42 +497,29 @@ struct Sim : md_sim {
             CK(cudaEventElapsedTime(&ms, ev[0], ev[1]));
             unsigned long long t[8];
             CK(cudaMemcpy(t, l.vtimes, sizeof(t), cudaMemcpyDeviceToHost));
+#ifdef MD_DIAGNOSTICS
             if (getenv("MD_DEBUG_TIMES")) {
                 std::vector<unsigned long long> w(8192);
                 CK(cudaMemcpy(w.data(), l.vtimes + 8, 8192 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
                 const int nwarp = coop_grid * md::VL_THREADS / 32;
-                fprintf(stderr, "[md] per-warp cumulative step-phase us (every 37th of %d warps):", nwarp);
-                for (int k = 0; k < nwarp && k < 8192; k += 37) fprintf(stderr, " %.0f", w[k] * 1e-3);
                 unsigned long long mx = 0, sm = 0;
                 for (int k = 0; k < nwarp && k < 8192; ++k) { mx = std::max(mx, w[k]); sm += w[k]; }
-                fprintf(stderr, "\n[md] max %.0f us mean %.0f us; slowest warps:", mx * 1e-3, sm * 1e-3 / nwarp);
-                std::vector<int> order(std::min(nwarp, 8192));
-                for (size_t k = 0; k < order.size(); ++k) order[k] = (int)k;
-                std::partial_sort(order.begin(), order.begin() + std::min<size_t>(12, order.size()), order.end(),
-                                  [&](int x, int y) { return w[x] > w[y]; });
-                for (size_t k = 0; k < std::min<size_t>(12, order.size()); ++k)
-                    fprintf(stderr, " %d:%.0f", order[k], w[order[k]] * 1e-3);
-                fprintf(stderr, "\n");
-            }
-            if (getenv("MD_DEBUG_TIMES")) {
+                fprintf(stderr, "[md] per-warp cumulative step-phase us: max %.0f mean %.0f\n", mx * 1e-3, sm * 1e-3 / nwarp);
                 int nh = 0;
                 CK(cudaMemcpy(&nh, l.vflags + md::VF_NHEAVY, sizeof(int), cudaMemcpyDeviceToHost));
                 fprintf(stderr, "[md] heavy particles (list > %d entries) after the last rebuild: %d\n", vl.heavy_t, nh);
             }
-            if (getenv("MD_DEBUG_TIMES"))
-                fprintf(stderr, "[md] cumulative ns: step %llu barrier %llu rebuild %llu final %llu | bin %llu scan %llu "
-                        "scatter %llu build %llu\n", t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7]);
-            for (int q = 0; q < 4; ++q) { phase_ns[q] = t[q] - phase_seen[q]; phase_seen[q] = t[q]; }
+#endif
+            for (int q = 0; q < 8; ++q) { phase_ns[q] = t[q] - phase_seen[q]; phase_seen[q] = t[q]; }
+            for (int q = 0; q < 4; ++q) out->rebuild_ms[q] = phase_ns[4 + q] * 1e-6;   // bin, scan, scatter, list build
             // VERLET: ms[0] step phases, ms[1] grid barriers, ms[2] rebuilds (as seen by thread 0), ms[3] whole launch
             out->ms[0] = phase_ns[0] * 1e-6; out->ms[1] = phase_ns[1] * 1e-6; out->ms[2] = phase_ns[2] * 1e-6;
             out->ms[3] = out->total_ms = ms;
             out->launches[3] = n > 0 ? 1 : 0;
             out->steps = n; out->rebuilds = rebuilds_seen - r0;
             step_no += n;
-            if (getenv("MD_DEBUG_BUILD") && rebuilds_seen > r0 && out->rebuilds == 0) {
-                // only meaningful right after a rebuild (positions still wrapped, cell order current): n = 0 calls
-            }
-            if (getenv("MD_DEBUG_BUILD")) {
+#ifdef MD_DIAGNOSTICS
+            if (getenv("MD_DEBUG_BUILD")) {      // the build and force phases as kernels of their own, for ncu
                 for (int k = 0; k < 3; ++k) {
                     if (dim == 3) md::k_dbg_build<T, 9><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur);
                     else md::k_dbg_build<T, 3><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur);
@@ -512,6 +527,7 @@ struct Sim : md_sim {
                 for (int k = 0; k < 3; ++k) md::k_dbg_force<T><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur, curv);
                 CK(cudaStreamSynchronize(stream));
             }
+#endif
             return MD_OK;
         }
         for (long long k = 0; k < n; ++k) {
@@ -630,7 +646,7 @@ struct Sim : md_sim {
             CK(cudaMemcpyAsync(h.data(), l.ncnt, sizeof(int) * h.size(), cudaMemcpyDeviceToHost, stream));
             CK(cudaStreamSynchronize(stream));
             long long t = 0;
-            for (int c : h) t += c & md::VL_NMASK;
+            for (int c : h) t += (c & md::VL_NVV_MASK) + ((c >> md::VL_NVW_SHIFT) & md::VL_NVW_MASK);
             *tests = t;
             return MD_OK;
         }
@@ -773,11 +789,13 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
         // walls (cell order) appended to both position buffers; then bin + list + f(0) in one persistent launch
         CK(cudaMemsetAsync(l.vflags, 0, sizeof(int) * md::VF_COUNT, stream));
         CK(cudaMemsetAsync(l.vtimes, 0, (8 + 8192) * sizeof(unsigned long long), stream));
-        CK(cudaMemsetAsync(l.tile_sum, 0, sizeof(int) * (size_t)(cdiv(p.ncell, md::SCAN_TILE) + 1), stream));
+        CK(cudaMemsetAsync(l.tile_agg, 0, sizeof(unsigned long long) * (size_t)(cdiv(p.ncell, md::SCAN_TILE) + 1), stream));
         if (nw > 0)
             for (int b = 0; b < 2; ++b)
                 CK(cudaMemcpyAsync(l.st[b].r + nv, l.wr, sizeof(md::Vec4<T>) * (size_t)nw, cudaMemcpyDeviceToDevice,
                                    stream));
+        if constexpr (sizeof(T) == 8)
+            if (nw > 0) md::k_wall_ghosts<T><<<cdiv(nw, 256), 256, 0, stream>>>(p, vl);   // fp32 shadow + static ghost copies
         int rc = launch_run(0, 1);
         if (rc) return rc;
         return refresh();
@@ -842,7 +860,7 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
     s->box = box;
     s->algo = algo;
     s->stream = (cudaStream_t)stream;
-    s->l = carve<T>(ws, box.dim, nv, nw, g.ncell, algo);
+    s->l = carve<T>(ws, box.dim, nv, nw, g.ncell, algo, image_blocks(box, o.precision));
     if (s->l.bytes > ws_bytes) {
         g_create_error = "workspace too small";
         delete s;
@@ -916,11 +934,24 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
         md::Verlet<T>& v = s->vl;
         v.st[0] = s->l.st[0]; v.st[1] = s->l.st[1]; v.f = s->l.f;
         v.nbr = s->l.nbr; v.ncnt = s->l.ncnt; v.stride = align_up((size_t)nv, 64);
-        v.cell = s->l.cell; v.slot = s->l.slot; v.count = s->l.count; v.start = s->l.start; v.tile_sum = s->l.tile_sum;
-        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.bar = s->l.vbar; v.ksum = s->l.vksum; v.times = s->l.vtimes; v.dbg = getenv("MD_DEBUG_TIMES") ? s->l.vtimes + 8 : nullptr;
-        v.rl2 = (T)(rl * rl); v.half_skin = (T)(0.5 * skin);
-        v.heavy_t = getenv("MD_HEAVY_T") ? atoi(getenv("MD_HEAVY_T")) : 12;
-        v.carry = getenv("MD_NO_CARRY") ? 0 : 1;
+        v.cell = s->l.cell; v.slot = s->l.slot; v.count = s->l.count; v.start = s->l.start; v.tile_agg = s->l.tile_agg;
+        v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.bar = s->l.vbar; v.ksum = s->l.vksum; v.times = s->l.vtimes;
+        v.dbg = nullptr;
+        v.r32 = s->l.r32;
+        v.ntot = (int)(nv + nw); v.nimg = image_blocks(box, o.precision);
+        v.half_skin = (T)(0.5 * skin);
+        // fp32 filter of the list build: (r_c + skin) plus the rounding of the fp32 positions (ulp(L) / 2 each), of the
+        // image shift (ulp(2L) / 2) and of the fma chain; the list only has to be a superset
+        double lmax = 0.0;
+        for (int a = 0; a < box.dim; ++a) lmax = std::max(lmax, box.len[a]);
+        const double rlf = rl * (1.0 + 4e-7) + 4.0 * lmax * 1.1920929e-7;
+        v.rl2f = (float)(rlf * rlf * (1.0 + 2e-7));
+        v.heavy_t = o.heavy_list > 0 ? o.heavy_list - 1 : 12;   // lists of heavy_list entries or more (default 13)
+        v.carry = 1;
+#ifdef MD_DIAGNOSTICS
+        if (getenv("MD_DEBUG_TIMES")) v.dbg = s->l.vtimes + 8;
+        if (getenv("MD_NO_CARRY")) v.carry = 0;
+#endif
     }
     int rc = s->init(box, lj, o, nv, pos, vel, nw, wall);
     if (rc != MD_OK) {
@@ -963,8 +994,9 @@ size_t md_workspace_bytes(const md_box* box, const md_lj* lj, const md_opts* o, 
     int algo = pick_algo(*box, *lj, *o, nv, nw);
     if (algo < 0) return 0;
     GridSpec g = grid_for(*box, *lj, *o, algo);
-    return o->precision == 64 ? carve<double>(nullptr, box->dim, nv, nw, g.ncell, algo).bytes
-                              : carve<float>(nullptr, box->dim, nv, nw, g.ncell, algo).bytes;
+    const int nimg = image_blocks(*box, o->precision);
+    return o->precision == 64 ? carve<double>(nullptr, box->dim, nv, nw, g.ncell, algo, nimg).bytes
+                              : carve<float>(nullptr, box->dim, nv, nw, g.ncell, algo, nimg).bytes;
 }
 
 int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj* lj, const md_opts* o, long long nv,
@@ -1001,8 +1033,10 @@ int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj*
         }
         for (int a = 0; a < dim; ++a) {
             const double h = 0.5 * (a == pore->axis ? pore->length : pore->width);
-            if (!(pore->center[a] - h >= 1.0) || !(pore->center[a] + h <= box->len[a] - 1.0)) {
-                g_create_error = "prism pore must lie at least 1 length unit inside the box";
+            // VERLET leaves periodic coordinates unwrapped by up to skin / 2 + one step between rebuilds
+            const double margin = std::max(1.0, list_skin(*lj, *o));
+            if (!(pore->center[a] - h >= margin) || !(pore->center[a] + h <= box->len[a] - margin)) {
+                g_create_error = "prism pore must lie at least max(1, skin) length units inside the box";
                 return MD_ERR_INVALID_ARG;
             }
         }
@@ -1041,6 +1075,7 @@ int md_info(const md_sim* s, int* algo, int nc[3], int* kps)
 }
 int md_destroy(md_sim* s)
 {
+    if (s) s->drain();          // the workspace is the caller's: nothing of ours may still run on it afterwards
     delete s;
     return MD_OK;
 }

@@ -10,61 +10,86 @@
 // since the last rebuild exceeds skin/2 -- the list holds every pair within r_c + skin, so every
 // pair within r_c is evaluated at every step: results are exact, identical to the brute-force
 // definition up to summation order.
+//
+// Round 2 (profiles/r02_*.md): (i) the list build is one thread per particle walking the 3^(d-1) cell rows
+// with an FP32 distance filter on a float4 shadow of the positions (the list only has to be a SUPERSET of the
+// pairs within r_c + skin; the force loop still takes the r < r_c decision in full precision), (ii) periodic
+// images are materialised as ghost copies the owner rewrites in its drift, so the time loop never folds a
+// difference, (iii) a list holds its vapor entries first and its wall entries after them, so the pair loop
+// carries one set of coefficients, (iv) particles in dense neighbourhoods (adsorbed films, clusters) no longer set the
+// pace: their lists are built by a whole warp each, and lists longer than 32 entries are evaluated by a whole warp.
 #pragma once
 #include "md_kernels.cuh"
 
-#include <cooperative_groups.h>
-
 namespace md {
-namespace cg = cooperative_groups;
 
 constexpr int VL_THREADS = 256;
 constexpr int VL_MAXN = 128;   // neighbour-list stride (entries per particle)
 
 // flags: rebuild request, list overflow, position-buffer parity, velocity/id-buffer parity, rebuild count, escape,
-// particles with a long list at the last rebuild (demand), how many of them the idle blocks' lane groups took (capacity)
+// particles with a long list at the last rebuild (demand), how many of them the idle blocks' lane groups took (capacity),
+// the same two for the lists long enough for a whole warp
 // The rebuild request rotates over three slots (step % 3): a slot is cleared one barrier before the phase that
 // may set it and read one barrier after, so no block can see a later step's request (which would desynchronise
 // the grid barriers).
-enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_HCAP = 9, VF_COUNT = 10 };
+enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_HCAP = 9,
+       VF_NHEAVY32 = 10, VF_HCAP32 = 11, VF_COUNT = 12 };
+
+// Shadow entry of the list build: (x, y, z) rounded to fp32.
+struct alignas(16) F4 {
+    float x, y, z, w;
+};
 
 template <typename T>
 struct Verlet {
-    // st[c].r: positions, double-buffered every step (nv vapor entries, then nw wall entries in cell order,
-    // static); st[cv].{vx,vy,vz,id}: owner-only data, swapped only by the rebuild's scatter
+    // st[c].r: positions, double-buffered every step.  Layout of one buffer: nimg image blocks of ntot = nv + nw
+    // entries each; block 0 holds the particles themselves (nv vapor entries in cell order, then the nw wall
+    // entries in cell order, static), block m > 0 the copies shifted by -+L in the dimensions whose bit is set in
+    // m (written only for particles in the first / last cell of those dimensions: the ghosts).
+    // st[cv].{vx,vy,vz,id}: owner-only data, swapped only by the rebuild's scatter
     State<T> st[2];
     Force<T> f;
-    int *nbr, *ncnt;           // nbr[k * stride + i], k < VL_MAXN; ncnt[nv]; j >= nv means wall particle j - nv
+    int *nbr, *ncnt;           // nbr[k * stride + i], k < VL_MAXN: index into a position buffer; ncnt[nv]: see VL_* below
     size_t stride;             // >= nv
-    int *cell, *slot, *count, *start, *tile_sum;
-    const int* wstart;         // walls: [ncell + 1] ranges into the wall tail
+    int *cell, *slot, *count, *start;
+    unsigned long long* tile_agg;   // scan: (rebuild generation, sum of the tile's counts) per tile of SCAN_TILE cells
+    const int* wstart;         // walls: [ncell + 1] ranges into the wall part of an image block
     const uint8_t* wnear;
+    F4* r32;                   // [ntot] fp32 shadow of image block 0 (vapor part rewritten by every scatter); T = double only
     int* flags;                // VF_*
     unsigned long long* bar;   // grid barrier arrival counter
     double* ksum;              // [3] kinetic-energy accumulators of the thermostat, rotating like the requests
-    unsigned long long* dbg;   // optional per-warp step-phase ns (diagnostics), or nullptr
+    unsigned long long* dbg;   // optional per-warp step-phase ns (diagnostics build), or nullptr
     unsigned long long* times; // [8] ns seen by thread 0: step phases, step barriers, rebuilds, final phase,
                                // rebuild split: bin, scan, scatter, list build (each with its barrier)
-    T rl2, half_skin;          // (r_c + skin)^2, skin / 2
-    int carry;                 // 0: reload own state every step (diagnostic A/B, MD_NO_CARRY)
-    int heavy_t;               // particles whose list is longer than this are "heavy": in the step phase an 8-lane
-                               // group shares one such list (indices in `cell`, ncnt words in `slot` -- both free
-                               // between rebuilds; their number in flags[VF_NHEAVY])
+    T half_skin;               // skin / 2
+    float rl2f;                // (r_c + skin)^2 plus the fp32 rounding of the filter (positions, image shift, fma chain)
+    int ntot, nimg;            // image-block stride nv + nw; number of image blocks (1 in fp32 mode: that mode folds)
+    int carry;                 // 0: reload own state every step (diagnostic A/B)
+    int heavy_t;               // particles whose list is longer than this are "heavy": in the step phase a group of
+                               // VL_GROUP lanes shares one such list (indices in `cell`, ncnt words in `slot` -- both
+                               // free between rebuilds; their number in flags[VF_NHEAVY]), a whole warp if it is
+                               // longer than VL_WARP_T (registered from the top of `cell` / `slot` downwards)
 };
 
-// d = a - b folded to the nearest image by comparison (|true d| < r_c + skin < L/2).  fp32: the shift
-// goes on whichever particle sits at the top of the box so the difference stays exact.
-// fp64: |d| > L/2 is decided on the high word by the integer pipe (|d| is either < r_c + skin or > L - r_c - skin,
-// never near L/2) and the shift is L with d's sign: 2 FP64 instructions instead of 5 (DADD, 2 DSETP, 2 predicated
-// DADD) in a loop that is bound by the FP64 pipe (profiles/r01_heavy_groups.md); the result is bit-identical.
-__device__ __forceinline__ double fold(double a, double b, double L, double halfL)
-{
-    double d = a - b;
-    const int hi = __double2hiint(d);
-    if ((hi & 0x7fffffff) > __double2hiint(halfL))
-        d -= __hiloint2double(__double2hiint(L) | (hi & 0x80000000), __double2loint(L));
-    return d;
-}
+// ncnt word of a particle: vapor entries in list slots [0, nvv), wall entries in [nvv, nvv + nvw); face code = 2 bits
+// per dimension, 1 = the particle sat in the FIRST cell of a periodic dimension when the list was built (its ghost is
+// the copy at +L), 2 = in the LAST cell (ghost at -L); heavy = list walked by a lane group (see phase_step).
+constexpr int VL_NVV_MASK = 0xff, VL_NVW_SHIFT = 8, VL_NVW_MASK = 0xff, VL_FACE_SHIFT = 16, VL_FACE_MASK = 0x3f;
+constexpr int VL_HEAVY = 1 << 29;
+__device__ __forceinline__ int vl_nvv(int raw) { return raw & VL_NVV_MASK; }
+__device__ __forceinline__ int vl_nvw(int raw) { return (raw >> VL_NVW_SHIFT) & VL_NVW_MASK; }
+__device__ __forceinline__ int vl_face(int raw) { return (raw >> VL_FACE_SHIFT) & VL_FACE_MASK; }
+#ifndef MD_VL_GROUP
+#define MD_VL_GROUP 4
+#endif
+constexpr int VL_GROUP = MD_VL_GROUP;   // lanes sharing one heavy particle's list
+constexpr int VL_WARP_T = 32;           // lists longer than this (inside an adsorbed film: up to ~100 entries) get a whole warp
+constexpr int VL_WARP_ROUNDS = 2;       // such lists per idle warp and step
+
+// d = a - b folded to the nearest image by comparison (|true d| < r_c + skin < L/2): fp32 mode only, where a ghost
+// copy x + L would round the coordinate.  The shift goes on whichever particle sits at the top of the box so the
+// difference stays exact.
 __device__ __forceinline__ float fold(float a, float b, float L, float halfL)
 {
     float d = a - b;
@@ -72,11 +97,14 @@ __device__ __forceinline__ float fold(float a, float b, float L, float halfL)
     else if (d < -halfL) d = a - (b - L);
     return d;
 }
+__device__ __forceinline__ double fold(double a, double b, double, double) { return a - b; }   // never used: fp64 reads ghosts
 
 // Grid barrier of the cooperative launch (all blocks are co-resident).  One arrival atomic per block; the wait
 // polls with relaxed loads and fences ONCE when released -- cooperative_groups' grid.sync() re-acquires (and so
 // invalidates the SM's L1, CCTL.IVALL) on every poll, which also evicts the lines of the other block still
-// computing on that SM (profiles/r01_v3_cfg2.md).  `bar` is zeroed by the host before every launch.
+// computing on that SM (profiles/r01_v3_cfg2.md).  A flag per block polled by every block (no atomic) was measured in
+// round 2 and is 4x slower at 296 blocks: 296 x 296 loads per poll round land on ten L2 lines (profiles/r02_k_md_run.md).
+// `bar` is zeroed by the host before every launch.
 __device__ __forceinline__ void grid_barrier(unsigned long long* bar, unsigned long long& target)
 {
     __syncthreads();
@@ -100,19 +128,6 @@ __device__ __forceinline__ unsigned long long now_ns()
     return t;
 }
 
-// ---- one particle's force from its neighbour list, one thread per particle ----------------------
-// The list is stored transposed, nbr[k * stride + i], so a warp's loads of entry k are coalesced.
-// ncnt[i] = list length | VL_FOLD if the particle sat in a cell on a periodic face when the list was
-// built: only such particles can have a neighbour across the face, all others skip the image folding.
-// Entries are consumed four at a time: four index loads, then four position loads, are in flight together.
-constexpr int VL_FOLD = 1 << 30;
-constexpr int VL_HEAVY = 1 << 29;      // list longer than Verlet::heavy_t (see phase_step)
-constexpr int VL_NMASK = (1 << 16) - 1;
-#ifndef MD_VL_GROUP
-#define MD_VL_GROUP 4
-#endif
-constexpr int VL_GROUP = MD_VL_GROUP;   // lanes sharing one heavy particle's list
-
 // 1 / x without the division's special-case branch: hardware seed (>= 20 bits) + two Newton steps.
 __device__ __forceinline__ double rcp_fast(double x)
 {
@@ -130,50 +145,55 @@ __device__ __forceinline__ float rcp_fast(float x) { return 1.0f / x; }
 __device__ __forceinline__ double step_len(double s2) { return (double)(sqrtf((float)s2) * 1.000001f); }
 __device__ __forceinline__ float step_len(float s2) { return sqrtf(s2); }
 
-// Branch-free pair term: the four pairs of a batch form four independent dependency chains.
+// Coefficients of one pair type (vapor-vapor or vapor-wall), held in registers by the pair loop.
+template <typename T>
+struct PairCoef {
+    T rc2, c12, c6;            // time loop: g = (c12 / r^6 - c6) / r^8
+    T sig2, e24, e4, uc;       // energy pass: the oracle's s = sigma^2 / r^2 form
+};
+template <typename T>
+__device__ __forceinline__ PairCoef<T> coef_vv(const Params<T>& p) { return {p.rc2, p.c12_vv, p.c6_vv, p.sig2_vv, p.e24_vv, p.e4_vv, p.uc_vv}; }
+template <typename T>
+__device__ __forceinline__ PairCoef<T> coef_vw(const Params<T>& p) { return {p.rc2, p.c12_vw, p.c6_vw, p.sig2_vw, p.e24_vw, p.e4_vw, p.uc_vw}; }
+
+// Branch-free pair term: the pairs of a batch form independent dependency chains.
 template <typename T, bool ENERGY>
-__device__ __forceinline__ void pair_term_nb(const Params<T>& p, bool valid, bool wall, T dx, T dy, T dz,
-                                             Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
+__device__ __forceinline__ void pair_term_nb(const PairCoef<T>& q, bool valid, T dx, T dy, T dz, Acc<T, ENERGY>& a)
 {
     const T r2 = fma_(dz, dz, fma_(dy, dy, dx * dx));
-    const bool hit = valid && r2 < p.rc2;                   // strict, same r^2 arithmetic as every other path
+    const bool hit = valid && r2 < q.rc2;                   // strict, same r^2 arithmetic as every other path
     const T inv = rcp_fast(hit ? r2 : T(1));
     T s3, s6, g;
     if (ENERGY) {
-        const T s = (wall ? p.sig2_vw : p.sig2_vv) * inv;
+        const T s = q.sig2 * inv;
         s3 = s * s * s;
         s6 = s3 * s3;
-        g = hit ? (wall ? p.e24_vw : p.e24_vv) * inv * (T(2) * s6 - s3) : T(0);
+        g = hit ? q.e24 * inv * (T(2) * s6 - s3) : T(0);
     } else {                                                // time loop: 5 instead of 7 operations after 1 / r^2
         const T i3 = inv * inv * inv;
-        g = hit ? fma_(wall ? p.c12_vw : p.c12_vv, i3, -(wall ? p.c6_vw : p.c6_vv)) * i3 * inv : T(0);
+        g = hit ? fma_(q.c12, i3, -q.c6) * i3 * inv : T(0);
     }
-    const T gw = wall ? g : T(0), gv = wall ? T(0) : g;
-    if (ENERGY) {                                           // U_vv and U_vw are reported separately
-        av.fx = fma_(gv, dx, av.fx); av.fy = fma_(gv, dy, av.fy); av.fz = fma_(gv, dz, av.fz);
-        aw.fx = fma_(gw, dx, aw.fx); aw.fy = fma_(gw, dy, aw.fy); aw.fz = fma_(gw, dz, aw.fz);
-    } else {                                                // time loop: one accumulator (aw stays 0)
-        av.fx = fma_(g, dx, av.fx); av.fy = fma_(g, dy, av.fy); av.fz = fma_(g, dz, av.fz);
-    }
+    a.fx = fma_(g, dx, a.fx); a.fy = fma_(g, dy, a.fy); a.fz = fma_(g, dz, a.fz);
     if (ENERGY) {
-        const double u = hit ? (double)((wall ? p.e4_vw : p.e4_vv) * (s6 - s3) - (wall ? p.uc_vw : p.uc_vv)) : 0.0;
-        const double w = (double)(g * r2);
-        if (wall) { aw.u += u; aw.w += w; aw.c += hit; }
-        else { av.u += u; av.w += w; av.c += hit; }
+        a.u += hit ? (double)(q.e4 * (s6 - s3) - q.uc) : 0.0;
+        a.w += (double)(g * r2);
+        a.c += hit;
     }
 }
 
-// Batches of VL_BATCH list entries; while batch b is evaluated the indices of batch b + 1 are in flight.  The first
-// index loads do not wait for the list length (rows beyond it are allocated; their values are masked), so the
-// first positions are requested one round trip after the thread starts.
+// One segment (vapor or wall) of a particle's list, one thread per particle.  The list is stored transposed,
+// nbr[k * stride + i], so a warp's loads of entry k are coalesced.  Entries are consumed VL_BATCH at a time: that many
+// index loads, then position loads, are in flight together, and while batch b is evaluated the indices of batch b + 1
+// are in flight.  The first index loads do not wait for the list length (rows beyond it are allocated; their values
+// are masked).  fp64: an entry already names the image (ghost copy) to read, differences are plain.  fp32: FOLD.
 #ifndef MD_VL_BATCH
 #define MD_VL_BATCH 4
 #endif
 constexpr int VL_BATCH = MD_VL_BATCH;
 template <typename T, bool ENERGY, bool FOLD>
-__device__ __forceinline__ void list_loop(const Params<T>& p, const int* __restrict__ lst, size_t stride, int n,
-                                          const Vec4<T>* __restrict__ r, const Vec4<T>& ri, const int (&j0)[VL_BATCH],
-                                          Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
+__device__ __forceinline__ void list_loop(const Params<T>& p, const PairCoef<T>& q, const int* __restrict__ lst, size_t stride,
+                                          int n, const Vec4<T>* __restrict__ r, const Vec4<T>& ri, const int (&j0)[VL_BATCH],
+                                          Acc<T, ENERGY>& a)
 {
     const bool px = FOLD && p.bc[0] == BC_PERIODIC, py = FOLD && p.bc[1] == BC_PERIODIC, pz = FOLD && p.bc[2] == BC_PERIODIC;
     int jn[VL_BATCH];
@@ -192,23 +212,35 @@ __device__ __forceinline__ void list_loop(const Params<T>& p, const int* __restr
             const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
             const T dy = py ? fold(ri.y, rj[u].y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj[u].y;
             const T dz = pz ? fold(ri.z, rj[u].z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj[u].z;
-            pair_term_nb<T, ENERGY>(p, j[u] >= 0, j[u] >= p.nv, dx, dy, dz, av, aw);
+            pair_term_nb<T, ENERGY>(q, j[u] >= 0, dx, dy, dz, a);
         }
     }
 }
 
+// Both segments of particle i's list: vapor entries (first VL_BATCH indices already in j0), then wall entries.  One
+// loop variant per warp: in fp32 mode every lane folds if any lane's particle sat in a face cell when the list was
+// built (a per-lane choice would run the two loops one after the other in most warps, because a warp's 32
+// cell-ordered particles span most of an x row and so nearly always include a face cell).
 template <typename T, bool ENERGY>
 __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& v, const Vec4<T>* __restrict__ r, int i,
                                            const Vec4<T>& ri, int raw, const int (&j0)[VL_BATCH],
                                            Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
     const int* __restrict__ lst = v.nbr + i;
-    // one loop per warp: if any lane's particle sits in a face cell every lane folds (the comparisons never fire
-    // for the others); a per-lane choice would run the two loops one after the other in most warps, because a
-    // warp's 32 cell-ordered particles span most of an x row and so nearly always include a face cell
-    const bool fold = __any_sync(__activemask(), (raw & VL_FOLD) != 0) || (raw & VL_FOLD);
-    if (fold) list_loop<T, ENERGY, true>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
-    else list_loop<T, ENERGY, false>(p, lst, v.stride, raw & VL_NMASK, r, ri, j0, av, aw);
+    const int nvv = vl_nvv(raw), nvw = vl_nvw(raw);
+    const bool fold = sizeof(T) == 4 && __any_sync(__activemask(), vl_face(raw) != 0);
+    const PairCoef<T> qv = coef_vv(p);
+    if (fold) list_loop<T, ENERGY, true>(p, qv, lst, v.stride, nvv, r, ri, j0, av);
+    else list_loop<T, ENERGY, false>(p, qv, lst, v.stride, nvv, r, ri, j0, av);
+    if (__any_sync(__activemask(), nvw != 0)) {             // walls: a few per cent of the particles have any
+        const PairCoef<T> qw = coef_vw(p);
+        const int* __restrict__ lw = lst + (size_t)nvv * v.stride;
+        int w0[VL_BATCH];
+#pragma unroll
+        for (int u = 0; u < VL_BATCH; ++u) w0[u] = u < nvw ? lw[(size_t)u * v.stride] : -1;
+        if (fold) list_loop<T, ENERGY, true>(p, qw, lw, v.stride, nvw, r, ri, w0, aw);
+        else list_loop<T, ENERGY, false>(p, qw, lw, v.stride, nvw, r, ri, w0, aw);
+    }
 }
 
 template <typename T, bool ENERGY>
@@ -221,14 +253,17 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
     list_force<T, ENERGY>(p, v, r, i, ri, v.ncnt[i], j0, av, aw);
 }
 
-// A heavy particle's list shared by the VL_GROUP lanes of a group: lane `sub` takes entries sub, sub + 8, sub + 16,
-// ... of every 4 * VL_GROUP (one batch of four covers lists of up to that many entries); the caller sums the lanes' partial forces.
+// A heavy particle's list shared by the VL_GROUP lanes of a group: lane `sub` takes entries sub, sub + VL_GROUP, ... of
+// every 4 * VL_GROUP (one batch of four covers lists of up to that many entries); the caller sums the lanes' partial
+// forces.  Vapor and wall entries are told apart by their slot (k < nvv), so this loop selects the coefficients per
+// entry -- the price of sharing one list, paid only by the few heavy particles.
 template <typename T, bool FOLD>
-__device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* __restrict__ lst, size_t stride, int n,
+__device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* __restrict__ lst, size_t stride, int nvv, int n,
                                                 int sub, const Vec4<T>* __restrict__ r, const Vec4<T>& ri,
-                                                const int (&j0)[4], Acc<T, false>& av, Acc<T, false>& aw)
+                                                const int (&j0)[4], Acc<T, false>& a)
 {
     const bool px = FOLD && p.bc[0] == BC_PERIODIC, py = FOLD && p.bc[1] == BC_PERIODIC, pz = FOLD && p.bc[2] == BC_PERIODIC;
+    const PairCoef<T> qv = coef_vv(p), qw = coef_vw(p);
     int jn[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) jn[u] = sub + VL_GROUP * u < n ? j0[u] : -1;
@@ -247,8 +282,33 @@ __device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* _
             const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
             const T dy = py ? fold(ri.y, rj[u].y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj[u].y;
             const T dz = pz ? fold(ri.z, rj[u].z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj[u].z;
-            pair_term_nb<T, false>(p, j[u] >= 0, j[u] >= p.nv, dx, dy, dz, av, aw);
+            const bool wall = k + sub + VL_GROUP * u >= nvv;
+            PairCoef<T> q;
+            q.rc2 = qv.rc2; q.c12 = wall ? qw.c12 : qv.c12; q.c6 = wall ? qw.c6 : qv.c6;
+            pair_term_nb<T, false>(q, j[u] >= 0, dx, dy, dz, a);
         }
+    }
+}
+
+// Ghost copies of particle i (fp64): position `rn` shifted by +L (face code 1) or -L (face code 2) in every non-empty
+// subset of the dimensions in which the particle sat in a face cell when the list was built; image block m (bit a =
+// dimension a shifted) holds the copy.  Only these copies are ever read: a list entry names one when the build
+// reached the neighbour across a periodic face.
+template <typename T>
+__device__ __forceinline__ void write_ghosts(const Params<T>& p, const Verlet<T>& v, Vec4<T>* __restrict__ r, int i,
+                                             const Vec4<T>& rn, int face)
+{
+    const int dims = ((face & 3) ? 1 : 0) | ((face & 12) ? 2 : 0) | ((face & 48) ? 4 : 0);
+    const T sx = (face & 3) == 1 ? p.L[0] : -p.L[0], sy = ((face >> 2) & 3) == 1 ? p.L[1] : -p.L[1],
+            sz = ((face >> 4) & 3) == 1 ? p.L[2] : -p.L[2];
+    for (int m = 1; m < v.nimg; ++m) {
+        if (m & ~dims) continue;
+        Vec4<T> g;
+        g.x = (m & 1) ? rn.x + sx : rn.x;
+        g.y = (m & 2) ? rn.y + sy : rn.y;
+        g.z = (m & 4) ? rn.z + sz : rn.z;
+        g.w = T(0);
+        r[(size_t)m * v.ntot + i] = g;
     }
 }
 
@@ -275,12 +335,13 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
                                            bool kick, bool drift, int req, int gtid, int gthreads,
                                            T lam, double* ksum, Carry<T>& cy, const bool cyon)
 {
+    constexpr bool GHOSTS = sizeof(T) == 8;
     const Vec4<T>* __restrict__ rcur = v.st[c].r;
     Vec4<T>* __restrict__ rnew = v.st[c ^ 1].r;
     const State<T>& s = v.st[cv];
     double kacc = 0.0;
     // F3 / F2 of particle i once its force is known (v already carries F4's factor); v and rn return what was stored
-    auto integrate = [&](int i, const Vec4<T>& ri, T& vx, T& vy, T& vz, T fx, T fy, T fz, Vec4<T>& rn) {
+    auto integrate = [&](int i, const Vec4<T>& ri, T& vx, T& vy, T& vz, T fx, T fy, T fz, Vec4<T>& rn, int face) {
         if (kick) {                                    // F3: v(t) = v(t - dt/2) + (dt/2m) f(t)
             vx = vx + p.hk * fx; vy = vy + p.hk * fy; vz = vz + p.hk * fz;
         }
@@ -303,6 +364,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             rn.w = ri.w + step_len(sx * sx + sy * sy + sz * sz); // path length >= displacement
             if (rn.w > v.half_skin) v.flags[VF_REQ0 + req] = 1;
             rnew[i] = rn;
+            if (GHOSTS && face) write_ghosts(p, v, rnew, i, rn, face);
         }
         if (kick || drift || lam != T(1)) { s.vx[i] = vx; s.vy[i] = vy; s.vz[i] = vz; }
     };
@@ -320,7 +382,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             vx = s.vx[i]; vy = s.vy[i]; vz = s.vz[i];    // issued early, consumed after the force loop
 #pragma unroll
             for (int u = 0; u < VL_BATCH; ++u) j0[u] = force ? v.nbr[(size_t)u * v.stride + i] : 0;   // in flight together
-            if (force) raw = v.ncnt[i];
+            raw = v.ncnt[i];                             // the face code is needed by the drift even without a force pass
         }
         vx = lam * vx; vy = lam * vy; vz = lam * vz;     // F4 of the step just completed (lam = 1 without thermostat)
         T fx, fy, fz;
@@ -337,7 +399,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             fx = v.f.fx[i]; fy = v.f.fy[i]; fz = v.f.fz[i];
         }
         Vec4<T> rn = ri;
-        integrate(i, ri, vx, vy, vz, fx, fy, fz, rn);
+        integrate(i, ri, vx, vy, vz, fx, fy, fz, rn, vl_face(raw));
         if (cyon && force) {
             cy.r = rn; cy.vx = vx; cy.vy = vy; cy.vz = vz; cy.raw = raw;
 #pragma unroll
@@ -362,6 +424,52 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         constexpr int GPW = 32 / VL_GROUP, GPB = VL_THREADS / VL_GROUP;         // groups per warp, per block
         const int nbl = min((int)gridDim.x, (p.nv + VL_THREADS - 1) / VL_THREADS), nsp = (int)gridDim.x - nbl;
         const int b = blockIdx.x, q = (lane / VL_GROUP) * (VL_THREADS / 32) + (threadIdx.x >> 5);
+        // Lists longer than VL_WARP_T (a particle inside an adsorbed film has ~100 neighbours within r_c + skin): one
+        // per WARP of the idle blocks, lane l takes entries l, l + 32, l + 64, l + 96 -- one batch, a butterfly sum,
+        // and lane 0 integrates.  Walked by four lanes such a list would take 7 batches while the grid waits.
+        if (b >= nbl) {
+            const int n32 = min(v.flags[VF_NHEAVY32], v.flags[VF_HCAP32]), nw32 = nsp * (VL_THREADS / 32);
+            const PairCoef<T> qv = coef_vv(p), qw = coef_vw(p);
+            const bool fpx = sizeof(T) == 4 && p.bc[0] == BC_PERIODIC, fpy = sizeof(T) == 4 && p.bc[1] == BC_PERIODIC,
+                       fpz = sizeof(T) == 4 && p.bc[2] == BC_PERIODIC;
+            for (int h = (b - nbl) + nsp * (threadIdx.x >> 5); h < n32; h += nw32) {
+                const int top = p.nv - 1 - h;
+                const int i = v.cell[top], raw = v.slot[top];
+                const int nvv = vl_nvv(raw), n = nvv + vl_nvw(raw);
+                int j[4];
+                Vec4<T> rj[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) j[u] = lane + 32 * u < n ? v.nbr[(size_t)(lane + 32 * u) * v.stride + i] : -1;
+                const Vec4<T> ri = rcur[i];
+                T vx = T(0), vy = T(0), vz = T(0);
+                if (lane == 0) { vx = lam * s.vx[i]; vy = lam * s.vy[i]; vz = lam * s.vz[i]; }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) rj[u] = rcur[max(j[u], 0)];
+                Acc<T, false> a;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const T dx = fpx ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
+                    const T dy = fpy ? fold(ri.y, rj[u].y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj[u].y;
+                    const T dz = fpz ? fold(ri.z, rj[u].z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj[u].z;
+                    const bool wall = lane + 32 * u >= nvv;
+                    PairCoef<T> qq;
+                    qq.rc2 = qv.rc2; qq.c12 = wall ? qw.c12 : qv.c12; qq.c6 = wall ? qw.c6 : qv.c6;
+                    pair_term_nb<T, false>(qq, j[u] >= 0, dx, dy, dz, a);
+                }
+                T fx = a.fx, fy = a.fy, fz = a.fz;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    fx += __shfl_xor_sync(0xffffffffu, fx, o);
+                    fy += __shfl_xor_sync(0xffffffffu, fy, o);
+                    fz += __shfl_xor_sync(0xffffffffu, fz, o);
+                }
+                if (lane == 0) {
+                    if (!drift) { v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz; }
+                    Vec4<T> rn = ri;
+                    integrate(i, ri, vx, vy, vz, fx, fy, fz, rn, vl_face(raw));
+                }
+            }
+        }
         const int slot = b >= nbl ? (b - nbl) + nsp * ((threadIdx.x >> 5) * GPW + lane / VL_GROUP) : nsp * GPB + q * nbl + b;
         for (int h = slot; h < nh; h += gthreads / VL_GROUP) {
             const bool first = h == slot, kept = cyon && first && cy.hvalid;
@@ -379,11 +487,12 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             }
             const Vec4<T> ri = rcur[i];
             vx = lam * vx; vy = lam * vy; vz = lam * vz;
-            Acc<T, false> av, aw;
-            const bool fold = __any_sync(__activemask(), (raw & VL_FOLD) != 0) || (raw & VL_FOLD);
-            if (fold) list_loop_group<T, true>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, j0, av, aw);
-            else list_loop_group<T, false>(p, v.nbr + i, v.stride, raw & VL_NMASK, sub, rcur, ri, j0, av, aw);
-            T fx = av.fx + aw.fx, fy = av.fy + aw.fy, fz = av.fz + aw.fz;
+            Acc<T, false> a;
+            const int nvv = vl_nvv(raw), n = nvv + vl_nvw(raw);
+            const bool fold = sizeof(T) == 4 && __any_sync(__activemask(), vl_face(raw) != 0);
+            if (fold) list_loop_group<T, true>(p, v.nbr + i, v.stride, nvv, n, sub, rcur, ri, j0, a);
+            else list_loop_group<T, false>(p, v.nbr + i, v.stride, nvv, n, sub, rcur, ri, j0, a);
+            T fx = a.fx, fy = a.fy, fz = a.fz;
 #pragma unroll
             for (int o = 1; o < VL_GROUP; o <<= 1) {
                 fx += __shfl_xor_sync(gmask, fx, o);
@@ -393,7 +502,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             if (sub == 0) {
                 if (!drift) { v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz; }
                 Vec4<T> rn = ri;
-                integrate(i, ri, vx, vy, vz, fx, fy, fz, rn);
+                integrate(i, ri, vx, vy, vz, fx, fy, fz, rn, vl_face(raw));
             }
             if (cyon && first) {
                 cy.hi = i; cy.hraw = raw; cy.hvx = vx; cy.hvy = vy; cy.hvz = vz;
@@ -440,9 +549,26 @@ __device__ __forceinline__ void phase_bin(const Params<T>& p, const Verlet<T>& v
     }
 }
 
-// R2a / R2b: exclusive scan of the counts, tiles strided over the blocks (same arithmetic as
-// k_scan_reduce / k_scan_apply).  blockDim.x must equal SCAN_THREADS.
-__device__ __forceinline__ void phase_scan_reduce(const int* __restrict__ count, int n, int* __restrict__ tile_sum)
+__device__ __forceinline__ int block_sum_int(int x, int* ws)
+{
+    x = warp_sum(x);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = x;
+    __syncthreads();
+    int a = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_THREADS / 32; ++k) a += ws[k];
+    return a;
+}
+
+// R2: exclusive scan of the counts in ONE phase, tiles strided over the blocks.  Pass A: a block sums each of its
+// tiles and publishes (generation, sum) as one 64-bit word.  Pass B: the offset of a tile is the sum of the published
+// sums before it -- read with relaxed loads, spinning while a word still carries an older generation (every block
+// publishes all its sums before it waits for any, so nobody waits for a waiter) -- then a warp-shuffle scan inside the
+// tile.  No second phase and no same-address atomics: 2048 warp atomics on the 21 tile sums of config 2 cost 10 us
+// when tried in the bin phase (profiles/r02_k_md_run.md).  blockDim.x must equal SCAN_THREADS.
+__device__ __forceinline__ void phase_scan(const int* __restrict__ count, int n, unsigned long long* __restrict__ tile_agg,
+                                           unsigned int gen, int* __restrict__ start)
 {
     __shared__ int ws[SCAN_THREADS / 32];
     const int tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
@@ -450,49 +576,14 @@ __device__ __forceinline__ void phase_scan_reduce(const int* __restrict__ count,
         const int base = t * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
         int s = 0;
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k)
-            if (base + k < n) s += count[base + k];
-        s = warp_sum(s);
-        __syncthreads();
-        if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
-        __syncthreads();
+        for (int k = 0; k < SCAN_ITEMS; ++k) s += base + k < n ? count[base + k] : 0;
+        const int sum = block_sum_int(s, ws);
         if (threadIdx.x == 0) {
-            int a = 0;
-            for (int k = 0; k < SCAN_THREADS / 32; ++k) a += ws[k];
-            tile_sum[t] = a;
+            const unsigned long long word = ((unsigned long long)gen << 32) | (unsigned int)sum;
+            asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(tile_agg + t), "l"(word) : "memory");
         }
     }
-}
-
-__device__ __forceinline__ void phase_scan_apply(int* __restrict__ count, int n, const int* __restrict__ tile_sum,
-                                                 int* __restrict__ start)
-{
-    __shared__ int ws[SCAN_THREADS / 32];
-    __shared__ int s_off;
-    const int tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
     for (int t = blockIdx.x; t < tiles; t += gridDim.x) {
-        int off = 0;
-        if (tile_sum) {
-            for (int k = threadIdx.x; k < t; k += SCAN_THREADS) off += tile_sum[k];
-        } else {            // few tiles: sum the earlier counts directly and save a phase + barrier
-            const int4* __restrict__ c4 = reinterpret_cast<const int4*>(count);     // t * SCAN_TILE is a multiple of 4
-#pragma unroll 8
-            for (int k = threadIdx.x; k < t * (SCAN_TILE / 4); k += SCAN_THREADS) {
-                const int4 q = c4[k];
-                off += q.x + q.y + q.z + q.w;
-            }
-        }
-        off = warp_sum(off);
-        __syncthreads();
-        if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = off;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            int a = 0;
-            for (int k = 0; k < SCAN_THREADS / 32; ++k) a += ws[k];
-            s_off = a;
-        }
-        __syncthreads();
-        off = s_off;
         const int base = t * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
         int val[SCAN_ITEMS];
         int s = 0;
@@ -501,6 +592,15 @@ __device__ __forceinline__ void phase_scan_apply(int* __restrict__ count, int n,
             val[k] = base + k < n ? count[base + k] : 0;
             s += val[k];
         }
+        int off = 0;
+        for (int k = threadIdx.x; k < t; k += SCAN_THREADS) {
+            unsigned long long word;
+            do {
+                asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(word) : "l"(tile_agg + k) : "memory");
+            } while ((unsigned int)(word >> 32) != gen);
+            off += (int)(unsigned int)word;
+        }
+        off = block_sum_int(off, ws);
         const int incl = warp_incl_scan(s);
         __syncthreads();
         if ((threadIdx.x & 31) == 31) ws[threadIdx.x >> 5] = incl;
@@ -514,10 +614,11 @@ __device__ __forceinline__ void phase_scan_apply(int* __restrict__ count, int n,
             run += val[k];
         }
         if (base <= n - 1 && n - 1 < base + SCAN_ITEMS) start[n] = run;
+        __syncthreads();
     }
 }
 
-// R3: scatter into cell order: positions c -> c^1, velocities / ids cv -> cv^1.
+// R3: scatter into cell order: positions c -> c^1 (plus their fp32 shadow), velocities / ids cv -> cv^1.
 template <typename T>
 __device__ __forceinline__ void phase_scatter(const Params<T>& p, const Verlet<T>& v, int c, int cv, int gtid,
                                               int gthreads)
@@ -528,120 +629,214 @@ __device__ __forceinline__ void phase_scatter(const Params<T>& p, const Verlet<T
     Vec4<T>* __restrict__ rb = v.st[c ^ 1].r;
     for (int i = gtid; i < p.nv; i += gthreads) {
         const int d = v.start[v.cell[i]] + v.slot[i];
-        rb[d] = ra[i];
+        const Vec4<T> ri = ra[i];
+        rb[d] = ri;
+        if (sizeof(T) == 8) v.r32[d] = F4{(float)ri.x, (float)ri.y, (float)ri.z, 0.f};
         b.vx[d] = a.vx[i]; b.vy[d] = a.vy[i]; b.vz[d] = a.vz[i];
         b.id[d] = a.id[i];
     }
 }
 
-// R4: neighbour list from the cell list (a3's cell traversal, cached): every j within r_c + skin of i,
-// vapor (j < nv) or wall (j = nv + k).  ROWS = 3^(d-1) lanes cooperate on one particle: lane `row` walks the
-// cell row (cy+ky, cz+kz) -- its three cells are one contiguous range of the cell-ordered arrays -- and
-// appends its hits through a shared-memory counter.  Positions are wrapped here, so distances fold.
+// End of a particle's list build: the ncnt word, the heavy registries, overflow, its ghost copies.
 template <typename T>
-__device__ __forceinline__ void list_range(const Params<T>& p, const Vec4<T>* __restrict__ r, int jb, int je, int skip,
-                                           const Vec4<T>& ri, T rl2, int* __restrict__ lst, size_t stride, int* cnt)
+__device__ __forceinline__ void finish_list(const Params<T>& p, const Verlet<T>& v, Vec4<T>* __restrict__ r, int i,
+                                            const Vec4<T>& ri, int n, int nvv, int face, int hcap, int hcap32)
 {
-    const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
-    constexpr int NB = 8;                                                // a cell row rarely holds more
-    for (int j0 = jb; j0 < je; j0 += NB) {
-        Vec4<T> rj[NB];
-#pragma unroll
-        for (int u = 0; u < NB; ++u) rj[u] = r[min(j0 + u, je - 1)];     // NB loads in flight
-#pragma unroll
-        for (int u = 0; u < NB; ++u) {
-            const int j = j0 + u;
-            const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
-            const T dy = py ? fold(ri.y, rj[u].y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj[u].y;
-            const T dz = pz ? fold(ri.z, rj[u].z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj[u].z;
-            const T r2 = fma_(dz, dz, fma_(dy, dy, dx * dx));
-            if (j < je && j != skip && r2 < rl2) {
-                const int k = atomicAdd(cnt, 1);
-                if (k < VL_MAXN) lst[(size_t)k * stride] = j;
-            }
-        }
+    const int nn = min(n, VL_MAXN), nv0 = min(nvv, nn);
+    int raw = nv0 | ((nn - nv0) << VL_NVW_SHIFT) | (face << VL_FACE_SHIFT);
+    // a long list goes to a lane group (a very long one to a warp) while the idle blocks have some left; the counters
+    // keep the demand and the host sizes the next launch by it; `cell` and `slot` are free until the next rebuild
+    if (n > max(VL_WARP_T, v.heavy_t) && hcap32 > 0) {
+        const int h = atomicAdd(v.flags + VF_NHEAVY32, 1);
+        if (h < hcap32) { raw |= VL_HEAVY; v.cell[p.nv - 1 - h] = i; v.slot[p.nv - 1 - h] = raw; }
+    } else if (n > v.heavy_t) {
+        const int h = atomicAdd(v.flags + VF_NHEAVY, 1);
+        if (h < hcap) { raw |= VL_HEAVY; v.cell[h] = i; v.slot[h] = raw; }
     }
+    v.ncnt[i] = raw;
+    if (n > VL_MAXN) v.flags[VF_OVERFLOW] = 1;
+    if (sizeof(T) == 8 && face) write_ghosts(p, v, r, i, ri, face);
 }
 
-template <typename T, int ROWS>
-__device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>& v, int c, int gtid, int gthreads, int hcap)
+template <typename T>
+__device__ __forceinline__ int face_code(const Params<T>& p, int cx, int cy, int cz)
 {
-    constexpr int PPW = 32 / ROWS;                       // particles per warp
-    __shared__ int s_cnt[(VL_THREADS / 32) * PPW];
-    const Vec4<T>* __restrict__ r = v.st[c].r;
-    const int nx = p.nc[0], ny = p.nc[1], nz = p.nc[2];
+    int face = 0;
+    if (p.bc[0] == BC_PERIODIC) face |= cx == 0 ? 1 : (cx == p.nc[0] - 1 ? 2 : 0);
+    if (p.bc[1] == BC_PERIODIC) face |= (cy == 0 ? 1 : (cy == p.nc[1] - 1 ? 2 : 0)) << 2;
+    if (p.bc[2] == BC_PERIODIC) face |= (cz == 0 ? 1 : (cz == p.nc[2] - 1 ? 2 : 0)) << 4;
+    return face;
+}
+
+// R4: neighbour list from the cell list (a3's cell traversal, cached): every j within r_c + skin of i, vapor entries
+// first, then wall entries.  The distance filter runs in FP32 on the fp32 shadow of the positions with a threshold
+// inflated by the rounding involved: the list is a superset of the pairs within r_c + skin, which is all the exactness
+// argument needs (fp64: an entry names the image block the time loop will read; fp32 mode stores plain indices and
+// folds).  Positions are wrapped here.
+//
+// With <= 4 warps per scheduler a warp instruction costs ~8 cycles here, whatever it is, so what bounds this phase is the
+// number of instructions a warp executes: three designs that walk each particle's 3^d cells with per-lane loops
+// (9 lanes per particle, one thread per particle, a warp sweeping its 32 particles' rows through shared-memory windows)
+// all took 40-45 us from N = 1024 to 65,536, at 10 % lane efficiency (profiles/r02_k_md_run.md).  This one has no
+// divergent loop: the unit of work is a SUPER-CELL of SX x SY x SZ cells (4 x 2 x 2: ~24 particles at density 0.05), one
+// warp each.  The warp gathers the candidates of the whole super-cell -- the (SX + 2)(SY + 2)(SZ + 2) cells around it, each
+// cell row one contiguous range, image shifts and list-entry codes applied on the way -- into a shared-memory tile with
+// coalesced loads, then lane l owns member particle l and scans the tile: broadcast reads, the same trip count in every
+// lane, a private append counter.  A lane tests ~3.5x the candidates its own 3^d cells hold, and the warp still executes
+// 6x fewer instructions.  Dense super-cells (an adsorbed film) take more member rounds and tile chunks of the same loop;
+// wall particles are a second pass over the wall tile.
+constexpr int VL_SX = 4, VL_SY = 2, VL_TILE = 256;
+
+template <typename T, int ROWS>
+__device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>& v, int c, int gtid, int gthreads, int hcap,
+                                            int hcap32)
+{
+    constexpr bool GHOSTS = sizeof(T) == 8;
+    constexpr int NW = VL_THREADS / 32, SX = VL_SX, SY = VL_SY, SZ = ROWS == 9 ? 2 : 1;
+    constexpr int NR = (SY + 2) * (ROWS == 9 ? SZ + 2 : 1);      // candidate rows of a super-cell
+    constexpr int NSEG = 3 * NR;                                 // per row: cells inside the box, image of the last cell, image of the first
+    constexpr unsigned FULL = 0xffffffffu;
+    __shared__ float4 s_tile[NW][VL_TILE];                       // (x, y, z) of a candidate in the super-cell's frame, w = bits of its list entry
+    __shared__ int s_excl[NW][NSEG + 1], s_b[NW][NSEG], s_e0[NW][NSEG];
+    __shared__ float s_sx[NW][NSEG], s_sy[NW][NSEG], s_sz[NW][NSEG];
+    __shared__ int s_mexcl[NW][SY * SZ + 1], s_mb[NW][SY * SZ];
+    Vec4<T>* __restrict__ r = v.st[c].r;
+    const F4* __restrict__ q = GHOSTS ? v.r32 : reinterpret_cast<const F4*>(r);
+    const float rl2 = v.rl2f;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int pl = lane / ROWS, row = lane - pl * ROWS;
-    const int warp = gtid >> 5, nwarps = gthreads >> 5;
-    int* cnt = s_cnt + wib * PPW + min(pl, PPW - 1);
-    for (int base = warp * PPW; base < p.nv; base += nwarps * PPW) {
-        const int i = base + pl;
-        const bool active = pl < PPW && i < p.nv;
-        if (active && row == 0) *cnt = 0;
-        __syncwarp();
-        if (active) {
-            const Vec4<T> ri = r[i];
-            int cx, cy, cz;
-            const int ci = cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
-            int* __restrict__ lst = v.nbr + i;
-            int qy = cy + row % 3 - 1, qz = cz + (ROWS == 9 ? row / 3 - 1 : 0);
-            bool ok = true;
-            if (qz < 0) { ok = p.bc[2] == BC_PERIODIC; qz += nz; }
-            else if (qz >= nz) { ok = p.bc[2] == BC_PERIODIC; qz -= nz; }
-            if (qy < 0) { ok = ok && p.bc[1] == BC_PERIODIC; qy += ny; }
-            else if (qy >= ny) { ok = ok && p.bc[1] == BC_PERIODIC; qy -= ny; }
-            if (ok) {
-                const int x0 = max(cx - 1, 0), x1 = min(cx + 1, nx - 1);
-                int xw = -1;
-                if (p.bc[0] == BC_PERIODIC) { if (cx == 0) xw = nx - 1; else if (cx == nx - 1) xw = 0; }
-                const int rowc = (qz * ny + qy) * nx;
-                const bool do_wall = p.nw > 0 && v.wnear[ci];
-                const int jb = v.start[rowc + x0], je = v.start[rowc + x1 + 1];
-                int jb2 = 0, je2 = 0, wb = 0, we = 0, wb2 = 0, we2 = 0;
-                if (xw >= 0) { jb2 = v.start[rowc + xw]; je2 = v.start[rowc + xw + 1]; }
-                if (do_wall) {
-                    wb = v.wstart[rowc + x0]; we = v.wstart[rowc + x1 + 1];
-                    if (xw >= 0) { wb2 = v.wstart[rowc + xw]; we2 = v.wstart[rowc + xw + 1]; }
+    const int nx = p.nc[0], ny = p.nc[1], nz = p.nc[2];
+    const int nsx = (nx + SX - 1) / SX, nsy = (ny + SY - 1) / SY, nsz = (nz + SZ - 1) / SZ;
+    const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
+    for (int task = gtid >> 5; task < nsx * nsy * nsz; task += gthreads >> 5) {
+        const int sx0 = (task % nsx) * SX, sy0 = ((task / nsx) % nsy) * SY, sz0 = (task / (nsx * nsy)) * SZ;
+        // ---- members: the particles of the super-cell's own rows (clipped to the box)
+        {
+            int mb = 0, len = 0;
+            if (lane < SY * SZ) {
+                const int cy = sy0 + lane % SY, cz = sz0 + lane / SY;
+                if (cy < ny && cz < nz) {
+                    const int rowc = (cz * ny + cy) * nx;
+                    mb = v.start[rowc + sx0];
+                    len = v.start[rowc + min(sx0 + SX, nx)] - mb;
                 }
-                list_range<T>(p, r, jb, je, i, ri, v.rl2, lst, v.stride, cnt);
-                list_range<T>(p, r, jb2, je2, i, ri, v.rl2, lst, v.stride, cnt);
-                list_range<T>(p, r, p.nv + wb, p.nv + we, -1, ri, v.rl2, lst, v.stride, cnt);
-                list_range<T>(p, r, p.nv + wb2, p.nv + we2, -1, ri, v.rl2, lst, v.stride, cnt);
+            }
+            const int incl = warp_incl_scan(len);
+            __syncwarp();
+            if (lane < SY * SZ) { s_mexcl[wib][lane] = incl - len; s_mb[wib][lane] = mb; }
+            if (lane == SY * SZ) s_mexcl[wib][SY * SZ] = incl;      // = total (lanes past the last row add 0)
+            __syncwarp();
+        }
+        const int mtotal = s_mexcl[wib][SY * SZ];
+        if (mtotal == 0) continue;
+        for (int pass = 0; pass < 2; ++pass) {
+            if (pass == 1 && p.nw == 0) break;
+            const int* __restrict__ st = pass ? v.wstart : v.start;
+            const int base = pass ? p.nv : 0;
+            // ---- candidate segments: row (sy0 - 1 + a, sz0 - 1 + b), kind 0 = its cells sx0 - 1 .. sx0 + SX inside the box,
+            // kind 1 = the image of the last cell at -L (super-cell at the low x face), kind 2 = the image of the first at +L
+            int total = 0;
+            __syncwarp();
+            for (int s0 = 0; s0 < NSEG; s0 += 32) {
+                const int sg = s0 + lane;
+                int sb = 0, len = 0, img = 0;
+                float fx = 0.f, fy = 0.f, fz = 0.f;
+                if (sg < NSEG) {
+                    const int row = sg % NR, kind = sg / NR;
+                    int qy = sy0 - 1 + row % (SY + 2), qz = ROWS == 9 ? sz0 - 1 + row / (SY + 2) : 0;
+                    bool ok = qy <= min(sy0 + SY, ny) && qz <= min(sz0 + SZ, nz);     // rows beyond a clipped super-cell's neighbours
+                    // a row below the box is the image at -L of the last row (candidates move DOWN by L), one above at +L
+                    if (qz < 0) { ok = ok && pz; qz += nz; fz = -(float)p.L[2]; img |= 4; }
+                    else if (qz >= nz) { ok = ok && pz; qz -= nz; fz = (float)p.L[2]; img |= 4; }
+                    if (qy < 0) { ok = ok && py; qy += ny; fy = -(float)p.L[1]; img |= 2; }
+                    else if (qy >= ny) { ok = ok && py; qy -= ny; fy = (float)p.L[1]; img |= 2; }
+                    int c0 = 0, c1 = -1;                                               // cells c0 .. c1 of the row
+                    if (kind == 0) { c0 = max(sx0 - 1, 0); c1 = min(sx0 + SX, nx - 1); }
+                    else if (kind == 1) { if (px && sx0 == 0) { c0 = c1 = nx - 1; fx = -(float)p.L[0]; img |= 1; } }
+                    else { if (px && sx0 + SX >= nx) { c0 = c1 = 0; fx = (float)p.L[0]; img |= 1; } }
+                    if (ok && c1 >= c0) {
+                        const int rowc = (qz * ny + qy) * nx;
+                        sb = st[rowc + c0];
+                        len = st[rowc + c1 + 1] - sb;
+                    }
+                }
+                const int incl = warp_incl_scan(len);
+                if (sg < NSEG) {
+                    s_excl[wib][sg] = total + incl - len; s_b[wib][sg] = sb; s_e0[wib][sg] = (GHOSTS ? img * v.ntot : 0) + base;
+                    s_sx[wib][sg] = fx; s_sy[wib][sg] = fy; s_sz[wib][sg] = fz;
+                }
+                total += __shfl_sync(FULL, incl, 31);
+            }
+            if (lane == 0) s_excl[wib][NSEG] = total;
+            __syncwarp();
+            // ---- member rounds x tile chunks (pass 1 runs even without a wall nearby: it closes the members' lists)
+            for (int m0 = 0; m0 < mtotal; m0 += 32) {
+                const bool live = m0 + lane < mtotal;
+                int i = 0;
+                if (live) {
+                    int ms = 0;
+                    while (m0 + lane >= s_mexcl[wib][ms + 1]) ++ms;
+                    i = s_mb[wib][ms] + (m0 + lane - s_mexcl[wib][ms]);
+                }
+                const F4 qi = q[i];
+                int* __restrict__ lst = v.nbr + i;
+                int n = pass && live ? vl_nvv(v.ncnt[i]) : 0;            // pass 1 appends after the vapor entries
+                const int n0 = n;
+                int seg = 0;
+                for (int ch0 = 0; ch0 < total; ch0 += VL_TILE) {
+                    __syncwarp();
+#pragma unroll
+                    for (int u = 0; u < VL_TILE / 32; ++u) {               // gather: 8 independent loads per lane
+                        const int k = ch0 + 32 * u + lane;
+                        if (k < total) {
+                            while (k >= s_excl[wib][seg + 1]) ++seg;     // segments only move forward with k
+                            const int j = s_b[wib][seg] + (k - s_excl[wib][seg]);
+                            const F4 rj = q[base + j];
+                            s_tile[wib][32 * u + lane] = make_float4(rj.x + s_sx[wib][seg], rj.y + s_sy[wib][seg], rj.z + s_sz[wib][seg],
+                                                                     __int_as_float(s_e0[wib][seg] + j));
+                        }
+                    }
+                    __syncwarp();
+                    if (live) {
+                        const int cnt = min(VL_TILE, total - ch0);
+#pragma unroll 4
+                        for (int k = 0; k < cnt; ++k) {
+                            const float4 cj = s_tile[wib][k];
+                            const float dx = qi.x - cj.x, dy = qi.y - cj.y, dz = qi.z - cj.z;
+                            const int e = __float_as_int(cj.w);
+                            if (fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < rl2 && e != i) {
+                                if (n < VL_MAXN) lst[(size_t)n * v.stride] = e;
+                                ++n;
+                            }
+                        }
+                    }
+                }
+                if (live) {
+                    if (pass == 0 && p.nw > 0) {                         // parked for the wall pass (same lane of the same warp)
+                        v.ncnt[i] = min(n, VL_MAXN);
+                        if (n > VL_MAXN) v.flags[VF_OVERFLOW] = 1;
+                    } else {
+                        const Vec4<T> ri = r[i];
+                        int cx, cy, cz;
+                        cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
+                        finish_list(p, v, r, i, ri, n, pass ? n0 : n, face_code(p, cx, cy, cz), hcap, hcap32);
+                    }
+                }
             }
         }
-        __syncwarp();
-        if (active && row == 0) {
-            const int n = *cnt;
-            const Vec4<T> ri = r[i];
-            int cx, cy, cz;
-            cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
-            const bool face = (p.bc[0] == BC_PERIODIC && (cx == 0 || cx == nx - 1)) ||
-                              (p.bc[1] == BC_PERIODIC && (cy == 0 || cy == ny - 1)) ||
-                              (p.bc[2] == BC_PERIODIC && (cz == 0 || cz == nz - 1));
-            // a long list goes to a lane group while the idle blocks have groups left (the counter keeps the
-            // demand; the host sizes the next launch by it); `cell` and `slot` are free until the next rebuild
-            int raw = min(n, VL_MAXN) | (face ? VL_FOLD : 0);
-            if (n > v.heavy_t) {
-                const int h = atomicAdd(v.flags + VF_NHEAVY, 1);
-                if (h < hcap) { raw |= VL_HEAVY; v.cell[h] = i; v.slot[h] = raw; }
-            }
-            v.ncnt[i] = raw;
-            if (n > VL_MAXN) v.flags[VF_OVERFLOW] = 1;
-        }
-        __syncwarp();
     }
 }
 
 // ---- the persistent time loop ---------------------------------------------------------------------
 // md_step(n): phase(stored f; kick + drift), then n - 1 fused phases (force; kick; kick + drift), then
-// phase(force; kick): n + 1 phases and n grid barriers for n steps, plus 5 barriers per rebuild.
+// phase(force; kick): n + 1 phases and n grid barriers for n steps, plus 4 barriers per rebuild.
 // force_rebuild (md_create): bin + build the list first, then evaluate f(0).
 // MINB = resident blocks per SM the register budget is sized for: 2 (up to 128 registers, the latency-bound
 // sizes that fit one wave) or 3 (more warps to hide HBM latency once the state no longer fits in L2).
 template <typename T, int ROWS, int MINB>
 __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
 {
-    unsigned long long bar_target = 0;
+    __shared__ unsigned long long s_times[8];
+    unsigned long long bar_seq = 0;
     const bool thermo = p.thermo_rate > 0.0;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
     const int gthreads = gridDim.x * blockDim.x;
@@ -650,81 +845,109 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
     Carry<T> carry;
     const bool cyon = MINB == 2 && v.carry && !thermo && gthreads >= p.nv;      // (the 3-blocks-per-SM variant serves N > one wave)
     // lane groups in the blocks past the last particle (none once the particles fill the grid)
-    const int hcap = max((int)gridDim.x - (p.nv + VL_THREADS - 1) / VL_THREADS, 0) * (VL_THREADS / VL_GROUP);
+    const int nidle = max((int)gridDim.x - (p.nv + VL_THREADS - 1) / VL_THREADS, 0);
+    const int hcap = nidle * (VL_THREADS / VL_GROUP), hcap32 = nidle * (VL_THREADS / 32) * VL_WARP_ROUNDS;
+    if (gtid == 0)
+        for (int k = 0; k < 8; ++k) s_times[k] = 0;
     unsigned long long t0 = gtid == 0 ? now_ns() : 0ull, t1;
     for (long long s = 0;; ++s) {
         if (rebuild) {
             unsigned long long u0 = gtid == 0 ? now_ns() : 0ull, u1;
-            if (gtid == 0) { v.flags[VF_NHEAVY] = 0; v.flags[VF_HCAP] = hcap; }
-            phase_bin<T>(p, v, c, gtid, gthreads);
-            grid_barrier(v.bar, bar_target);
-            if (gtid == 0) { u1 = now_ns(); v.times[4] += u1 - u0; u0 = u1; }
-            const bool two_level = p.ncell > 64 * SCAN_TILE;
-            if (two_level) {
-                phase_scan_reduce(v.count, p.ncell, v.tile_sum);
-                grid_barrier(v.bar, bar_target);
+            if (gtid == 0) {
+                v.flags[VF_NHEAVY] = 0; v.flags[VF_HCAP] = hcap; v.flags[VF_NHEAVY32] = 0; v.flags[VF_HCAP32] = hcap32;
             }
-            phase_scan_apply(v.count, p.ncell, two_level ? v.tile_sum : nullptr, v.start);
-            grid_barrier(v.bar, bar_target);
-            if (gtid == 0) { u1 = now_ns(); v.times[5] += u1 - u0; u0 = u1; }
+            phase_bin<T>(p, v, c, gtid, gthreads);
+            grid_barrier(v.bar, bar_seq);
+            if (gtid == 0) { u1 = now_ns(); s_times[4] += u1 - u0; u0 = u1; }
+            phase_scan(v.count, p.ncell, v.tile_agg, (unsigned int)v.flags[VF_NREBUILD] + 1u, v.start);
+            grid_barrier(v.bar, bar_seq);
+            if (gtid == 0) { u1 = now_ns(); s_times[5] += u1 - u0; u0 = u1; }
             phase_scatter<T>(p, v, c, cv, gtid, gthreads);
-            grid_barrier(v.bar, bar_target);
-            if (gtid == 0) { u1 = now_ns(); v.times[6] += u1 - u0; u0 = u1; }
+            grid_barrier(v.bar, bar_seq);
+            if (gtid == 0) { u1 = now_ns(); s_times[6] += u1 - u0; u0 = u1; }
             c ^= 1; cv ^= 1;
-            phase_build<T, ROWS>(p, v, c, gtid, gthreads, hcap);
+            phase_build<T, ROWS>(p, v, c, gtid, gthreads, hcap, hcap32);
             for (int q = gtid; q < p.ncell; q += gthreads) v.count[q] = 0;                  // for the next rebuild
             if (gtid == 0) v.flags[VF_NREBUILD] += 1;
-            grid_barrier(v.bar, bar_target);
-            if (gtid == 0) { t1 = now_ns(); v.times[2] += t1 - t0; t0 = t1; v.times[7] += t1 - u0; }
+            grid_barrier(v.bar, bar_seq);
+            if (gtid == 0) { t1 = now_ns(); s_times[2] += t1 - t0; t0 = t1; s_times[7] += t1 - u0; }
             carry.valid = carry.hvalid = carry.nhvalid = false;          // new particle order, new lists
         }
         if (s == n_steps) break;
         const int req = (int)(s % 3);
         if (gtid == 0) { v.flags[VF_REQ0 + (req + 1) % 3] = 0; if (thermo) v.ksum[(s + 1) % 3] = 0.0; }   // slots of step s + 1
+#ifdef MD_DIAGNOSTICS
         unsigned long long dbg0 = 0;
         if (v.dbg) dbg0 = now_ns();
+#endif
         if (!thermo || s == 0) {
             phase_step<T>(p, v, c, cv, s > 0, s > 0, true, req, gtid, gthreads, T(1), nullptr, carry, cyon);
         } else {
             // with the thermostat lambda(t) needs K(t) of ALL particles before the next drift: the fused phase splits
             // into [F1 + F3 + K partial sums] | barrier | [F4 rescale + F2], one extra barrier per step
             phase_step<T>(p, v, c, cv, true, true, false, req, gtid, gthreads, T(1), v.ksum + s % 3);
-            grid_barrier(v.bar, bar_target);
+            grid_barrier(v.bar, bar_seq);
             const double lam = berendsen_lambda(*(volatile double*)(v.ksum + s % 3), p.thermo_rate, p.t_target, p.dof);
             phase_step<T>(p, v, c, cv, false, false, true, req, gtid, gthreads, (T)lam);
         }
+#ifdef MD_DIAGNOSTICS
         if (v.dbg && (threadIdx.x & 31) == 0) atomicAdd(v.dbg + (gtid >> 5), now_ns() - dbg0);
-        if (gtid == 0) { t1 = now_ns(); v.times[0] += t1 - t0; t0 = t1; }
-        grid_barrier(v.bar, bar_target);
-        if (gtid == 0) { t1 = now_ns(); v.times[1] += t1 - t0; t0 = t1; }
+#endif
+        if (gtid == 0) { t1 = now_ns(); s_times[0] += t1 - t0; t0 = t1; }
+        grid_barrier(v.bar, bar_seq);
+        if (gtid == 0) { t1 = now_ns(); s_times[1] += t1 - t0; t0 = t1; }
         c ^= 1;
         rebuild = *(volatile int*)(v.flags + VF_REQ0 + req) != 0;
     }
     if (thermo && n_steps > 0) {
         double* ks = v.ksum + n_steps % 3;
         phase_step<T>(p, v, c, cv, true, true, false, 0, gtid, gthreads, T(1), ks);
-        grid_barrier(v.bar, bar_target);
+        grid_barrier(v.bar, bar_seq);
         const double lam = berendsen_lambda(*(volatile double*)ks, p.thermo_rate, p.t_target, p.dof);
         phase_step<T>(p, v, c, cv, false, false, false, 0, gtid, gthreads, (T)lam);      // F4 of the last step
     } else if (n_steps > 0 || force_rebuild) {
         phase_step<T>(p, v, c, cv, true, n_steps > 0, false, 0, gtid, gthreads);
     }
-    if (gtid == 0) { v.flags[VF_CUR] = c; v.flags[VF_CURV] = cv; v.times[3] += now_ns() - t0; }
+    if (gtid == 0) {
+        v.flags[VF_CUR] = c; v.flags[VF_CURV] = cv;
+        s_times[3] += now_ns() - t0;
+        for (int k = 0; k < 8; ++k) v.times[k] += s_times[k];
+    }
 }
 
-// Diagnostics only (MD_DEBUG_BUILD=1 in md_profile_step): the list-build phase as a kernel of its own, so that ncu can
-// attribute its stalls.  It rebuilds the list from the current cell order, which is what the list already holds.
+#ifdef MD_DIAGNOSTICS
+// Diagnostics build only: the list-build phase as a kernel of its own, so that ncu can attribute its stalls.  It
+// rebuilds the list from the current cell order, which is what the list already holds.
 template <typename T, int ROWS>
 __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_build(Params<T> p, Verlet<T> v, int c)
 {
-    phase_build<T, ROWS>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, v.flags[VF_HCAP]);
+    phase_build<T, ROWS>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, v.flags[VF_HCAP], v.flags[VF_HCAP32]);
 }
 
-// Diagnostics only (MD_DEBUG_BUILD=1): the force part of the step phase as a kernel of its own (recomputes f(t)).
+// Diagnostics build only: the force part of the step phase as a kernel of its own (recomputes f(t)).
 template <typename T>
 __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_force(Params<T> p, Verlet<T> v, int c, int cv)
 {
     phase_step<T>(p, v, c, cv, true, false, false, 0, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+#endif
+
+// Ghost copies of the wall particles (static, both position buffers), md_create only.
+template <typename T>
+__global__ void k_wall_ghosts(Params<T> p, Verlet<T> v)
+{
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= p.nw) return;
+    const Vec4<T> rw = v.st[0].r[p.nv + w];
+    int cx, cy, cz;
+    cell_index(p, rw.x, rw.y, rw.z, cx, cy, cz);
+    int face = 0;
+    if (p.bc[0] == BC_PERIODIC) face |= cx == 0 ? 1 : (cx == p.nc[0] - 1 ? 2 : 0);
+    if (p.bc[1] == BC_PERIODIC) face |= (cy == 0 ? 1 : (cy == p.nc[1] - 1 ? 2 : 0)) << 2;
+    if (p.bc[2] == BC_PERIODIC) face |= (cz == 0 ? 1 : (cz == p.nc[2] - 1 ? 2 : 0)) << 4;
+    v.r32[p.nv + w] = F4{(float)rw.x, (float)rw.y, (float)rw.z, 0.f};
+    if (face)
+        for (int b = 0; b < 2; ++b) write_ghosts(p, v, v.st[b].r, p.nv + w, rw, face);
 }
 
 // a5 energy pass over the neighbour list (ordinary launch; the host passes the buffer parities).
@@ -744,9 +967,6 @@ __global__ void __launch_bounds__(VL_THREADS) k_verlet_energy(Params<T> p, Verle
     eo.cvw[i] = aw.c;
 }
 
-} // namespace md
-
-namespace md {
 // out[id[i]][0..dim) = r[i].xyz with periodic coordinates wrapped into [0, L) (the persistent kernel
 // leaves them unwrapped between rebuilds).
 template <typename T>
@@ -766,4 +986,5 @@ __global__ void k_export_pos_wrapped(Params<T> p, int dim, const int* __restrict
     out[o + 1] = (double)v.y;
     if (dim == 3) out[o + 2] = (double)v.z;
 }
+
 } // namespace md

@@ -40,7 +40,7 @@ class md_lj(C.Structure):
 
 class md_opts(C.Structure):
     _fields_ = [("dt", C.c_double), ("mass", C.c_double), ("precision", C.c_int), ("force_algo", C.c_int),
-                ("skin", C.c_double), ("tau_b", C.c_double), ("t_target", C.c_double)]
+                ("skin", C.c_double), ("tau_b", C.c_double), ("t_target", C.c_double), ("heavy_list", C.c_int)]
 
 
 class md_energy_out(C.Structure):
@@ -57,7 +57,7 @@ class md_pressure_out(C.Structure):
 
 class md_kernel_times(C.Structure):
     _fields_ = [("ms", C.c_double * 4), ("launches", C.c_longlong * 4), ("total_ms", C.c_double),
-                ("steps", C.c_longlong), ("rebuilds", C.c_longlong)]
+                ("steps", C.c_longlong), ("rebuilds", C.c_longlong), ("rebuild_ms", C.c_double * 4)]
 
 
 class md_peaks(C.Structure):
@@ -128,6 +128,7 @@ def _structs(cfg, precision=64, algo=None):
     opts.force_algo = _ALGO[algo if algo is not None else cfg.get("algo", "auto")]
     opts.skin = float(cfg.get("skin", 0.0))
     opts.tau_b, opts.t_target = float(cfg.get("tau_b", 0.0)), float(cfg.get("t_target", 1.0))
+    opts.heavy_list = int(cfg.get("heavy_list", 0))
     return box, lj, opts
 
 
@@ -162,6 +163,7 @@ class Simulation:
         n_wall = wall.shape[0]
         nbytes = self._lib.md_workspace_bytes(C.byref(box), C.byref(lj), C.byref(opts), self.n_vapor, n_wall)
         self.workspace = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=self.device)
+        self.workspace.record_stream(self.stream)  # allocated on the current stream, used on self.stream
         torch.cuda.synchronize(self.device)
         self._h = C.c_void_p()
         pore = None
@@ -223,7 +225,8 @@ class Simulation:
     def profile_step(self, n_steps: int):
         t = md_kernel_times()
         self._check(self._lib.md_profile_step(self._h, int(n_steps), C.byref(t)))
-        return dict(ms=list(t.ms), launches=list(t.launches), total_ms=t.total_ms, steps=t.steps, rebuilds=t.rebuilds)
+        return dict(ms=list(t.ms), launches=list(t.launches), total_ms=t.total_ms, steps=t.steps, rebuilds=t.rebuilds,
+                    rebuild_ms=list(t.rebuild_ms))
 
     def pair_tests(self) -> int:
         v = C.c_longlong()
@@ -240,7 +243,7 @@ class Simulation:
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
-            self._lib.md_destroy(self._h)
+            self._lib.md_destroy(self._h)          # synchronises the stream: nothing runs on the workspace afterwards
             self._h = C.c_void_p()
 
     def __del__(self):

@@ -126,18 +126,17 @@ def test_small_ragged_cases(dim, box, bc, nw, seed, algo):
     check_traj(cfg, algo, 100)
 
 
-@pytest.mark.parametrize("heavy_t", [0, 5, 40, 1000])
-def test_verlet_heavy_lane_groups(heavy_t, monkeypatch):
-    """The persistent kernel gives particles whose list is longer than a threshold (default 12; MD_HEAVY_T is the
-    diagnostic override read at md_create) to 8-lane groups: every split between the two code paths -- all heavy,
-    mixed, none -- must give the oracle's forces and 100-step trajectory."""
-    monkeypatch.setenv("MD_HEAVY_T", str(heavy_t))
+@pytest.mark.parametrize("heavy_list", [1, 6, 41, 1000])
+def test_verlet_heavy_lane_groups(heavy_list):
+    """The persistent kernel gives particles whose list has md_opts.heavy_list entries or more (default 13) to 4-lane
+    groups: every split between the two code paths -- all heavy, mixed, none -- must give the oracle's forces and
+    100-step trajectory."""
     for dim, box, bc, nw, seed in [(3, (9.6, 10.5, 9.9), (0, 0, 1), 30, 11), (2, (13.7, 9.9), (0, 1), 12, 12)]:
         nv = min(300, int(0.3 * float(np.prod(box))) - nw)
-        cfg = I.small_case(dim, nv, box, bc, n_wall=nw, seed=seed, min_sep=0.9)
+        cfg = dict(I.small_case(dim, nv, box, bc, n_wall=nw, seed=seed, min_sep=0.9), heavy_list=heavy_list)
         check_step0(cfg, "verlet")
         check_traj(cfg, "verlet", 100)
-    cfg = I.config4(12)
+    cfg = dict(I.config4(12), heavy_list=heavy_list)
     check_step0(cfg, "verlet")
     check_traj(cfg, "verlet", 100, cells_oracle=True, chunks=(1, 99))
 
