@@ -25,7 +25,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "pair-interactions/s"
-WORKLOAD = "cfg2_cyl3d_64k: 3D cylindrical pore, 65536 vapor + 1240 wall particles, 110^3 box, fp64, cell list"
+WORKLOAD = ("cfg2_cyl3d_64k: 3D cylindrical pore, 65536 vapor + 1240 wall particles, 110^3 box, fp64, "
+            "cell list cached as a Verlet list (MD_FORCE_AUTO)")
+STATE_BYTES = 96       # compulsory bytes per particle-step of a fully fused step, 3D fp64 (read r, v; write r', v')
 ALGO = "auto"      # resolves to the persistent Verlet-list kernel on this workload (md.h: MD_FORCE_AUTO)
 
 
@@ -165,25 +167,31 @@ def run_ours(args):
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ev = [tuple(torch.cuda.Event(enable_timing=True) for _ in range(3)) for _ in range(args.steps)]
     inter = 0.0
+    e = sim.energy()
+    hits_before = 2 * e["pairs_vv"] + e["pairs_vw"]
     barrier()
-    for a, b in ev:
+    for a, m, b in ev:
         flush.zero_()                                               # L2 flush between timed iterations (untimed)
         sim.stream.wait_stream(torch.cuda.current_stream(dev))
         a.record(sim.stream)
-        sim.step(inner)
+        sim.step(inner)                                             # a1-a4: ONE launch of k_md_run (persistent path)
+        m.record(sim.stream)
         e = sim.energy()                                            # a5; synchronises the stream
         b.record(sim.stream)
-        inter += (2 * e["pairs_vv"] + e["pairs_vw"]) * inner        # ordered within-cut-off evaluations
+        hits = 2 * e["pairs_vv"] + e["pairs_vw"]                    # ordered within-cut-off evaluations per time step,
+        inter += 0.5 * (hits_before + hits) * inner                 # mean of the counts at both ends of the chunk
+        hits_before = hits
     barrier()
-    t_dev = max_over_ranks(sum(a.elapsed_time(b) for a, b in ev) * 1e-3)
+    t_dev = max_over_ranks(sum(a.elapsed_time(b) for a, m, b in ev) * 1e-3)
+    t_run = sum(a.elapsed_time(m) for a, m, b in ev) * 1e-3        # the k_md_run launches alone (this rank)
     clocks = sampler.stop() if rank == 0 else None
     inter_all = sum_over_ranks(inter)
     value = inter_all / t_dev
     steps_per_s = args.steps * inner / t_dev                        # per replica (all replicas advance together)
     persistent = info["algo"] == "verlet"
-    launches = args.steps * ((1 if persistent else inner * info["kernels_per_step"]) + 3)
+    launches = args.steps * ((1 if persistent else inner * info["kernels_per_step"]) + 3)   # + the three energy kernels
 
     # ---------------- end-to-end arm: host arrays in, host arrays out, through the C ABI ----
     host = {k: torch.from_numpy(np.ascontiguousarray(cfg[k])).pin_memory().numpy() for k in ("pos", "vel", "wall")}
@@ -191,7 +199,10 @@ def run_ours(args):
     ecfg.update(host)
     stream = torch.cuda.Stream(device=dev)
     e2e_inter = 0.0
-    md.Simulation(ecfg, algo=ALGO, device=dev, stream=stream).close()
+    s0 = md.Simulation(ecfg, algo=ALGO, device=dev, stream=stream)
+    e = s0.energy()
+    hits0 = 2 * e["pairs_vv"] + e["pairs_vw"]                       # every end-to-end step starts from the same t = 0 state
+    s0.close()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
@@ -199,7 +210,7 @@ def run_ours(args):
         s2.step(inner)
         st = s2.get_state(force=False, pe=False)                              # D2H of pos, vel
         e = s2.energy()
-        e2e_inter += (2 * e["pairs_vv"] + e["pairs_vw"]) * inner
+        e2e_inter += 0.5 * (hits0 + 2 * e["pairs_vv"] + e["pairs_vw"]) * inner
         s2.close()
     barrier()
     t_e2e = max_over_ranks(time.perf_counter() - t0)
@@ -217,21 +228,23 @@ def run_ours(args):
     tests = sim.pair_tests()
     ncell = int(np.prod(info["n_cells"]))
     if persistent:
-        # one launch = prof_steps time steps of k_md_run (force from the list + both half-kicks + drift, and the
-        # in-kernel re-bin / list rebuilds); algorithmic bytes per particle-step, fp64:
-        # r 32 + v 24 read, r' 32 + v' 24 written (f is stored only by the last phase of a launch), list count 4 +
-        # 4 per list entry read
-        prof_steps = 2000
-        sim.profile_step(200)
-        kt = sim.profile_step(prof_steps)
-        per_step = nv * (112 + 4) + 4 * tests
-        top_name, t_top, alg = "k_md_run (persistent: %d time steps per launch)" % prof_steps, kt["ms"][3] * 1e-3, per_step * prof_steps
-        shares = {"k_md_run": 1.0}
-        # DRAM traffic of k_md_run from the committed ncu --set full capture (profiles/r01_v8_cfg2.md):
-        # dram__bytes_read.sum + dram__bytes_write.sum = 11.86 MB for a 200-step launch = 59.3 KB per time step
-        traffic = 59.3e3 * prof_steps
-        extra = {"time_steps_per_launch": prof_steps, "rebuilds_in_launch": kt["rebuilds"],
-                 "us_per_time_step": kt["ms"][3] * 1e3 / prof_steps}
+        # k_md_run is the whole timed step but for the three energy kernels: its launches were timed above with CUDA
+        # events on the stream they run on.  achieved = algorithmic bytes / that time, with SURVEY 8(d)'s compulsory
+        # 96 B per particle-step; the bytes this LAYOUT moves per particle-step (32-byte positions with the path length
+        # in w, read and written; velocities read and written; the list: count word + 4 B per entry) are given beside it
+        top_name = "k_md_run (persistent: %d time steps per launch)" % inner
+        t_top = t_run / args.steps
+        alg = STATE_BYTES * nv * inner
+        layout = (nv * (64 + 48 + 4) + 4 * tests) * inner
+        shares = {"k_md_run": t_run / (sum(a.elapsed_time(b) for a, m, b in ev) * 1e-3)}
+        traffic = None
+        kt = sim.profile_step(inner)                                # in-kernel split of one more launch (after the timed region)
+        extra = {"time_steps_per_launch": inner, "us_per_time_step": t_top * 1e6 / inner, "layout_bytes_per_launch": layout,
+                 "traffic_source": "profiles/r02_k_md_run.md (ncu --set full of one launch: dram__bytes_read.sum + dram__bytes_write.sum)",
+                 "in_kernel_split_of_one_more_launch_us_per_time_step": {
+                     "step_phases": kt["ms"][0] * 1e3 / inner, "grid_barriers": kt["ms"][1] * 1e3 / inner,
+                     "rebuilds": kt["ms"][2] * 1e3 / inner, "rebuilds_in_launch": kt["rebuilds"],
+                     "rebuild_us_each_bin_scan_scatter_build": [x * 1e3 / max(kt["rebuilds"], 1) for x in kt["rebuild_ms"]]}}
     else:
         prof_steps = 200
         sim.profile_step(20)
@@ -295,7 +308,8 @@ def run_ours(args):
                        "l2": "256 MiB buffer written between timed iterations (L2 flush); inside an iteration the "
                              "4.7 MB state stays L2-resident across timesteps, as in any MD time loop",
                        "pair_tests_per_timestep": tests},
-            "pair_tests_per_s": tests * steps_per_s * world, "clocks": clocks,
+            "pair_tests_per_s": tests * steps_per_s * world,
+            "allpairs_equivalent_per_s": float(nv) * (nv - 1.0 + nw) * steps_per_s * world, "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": 1e3 * t_e2e / args.steps},
             "gpu_launches": launches, "roofline": roofline, "cells_every_step_path": cells_path,
@@ -335,6 +349,15 @@ def main():
     ap.add_argument("--allpairs-steps", type=int, default=10)
     ap.add_argument("--cpu-sweep", action="store_true", help="time the brute-force oracle for N_v = 2^10, 2^12, 2^14")
     args = ap.parse_args()
+    if args.gpus > 1 and "RANK" not in os.environ and not args.cpu_sweep and args.impl == "ours":
+        # started plainly: become the N-rank job the contract describes (one process per GPU, NCCL for the barrier)
+        import socket
+
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execvp(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+                                   "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
     if args.cpu_sweep:
         run_cpu_sweep()
     elif args.impl == "reference":

@@ -19,9 +19,15 @@
 namespace md {
 
 constexpr int AD_THREADS = 128;   // threads per block = entries per shared-memory tile
-constexpr int AD_IB = 4;          // particles i per thread for large N; 1 below AD_SMALL_N (more, shorter blocks: the
+#ifndef MD_AD_IB
+#define MD_AD_IB 4
+#endif
+#ifndef MD_AD_UNROLL
+#define MD_AD_UNROLL 16
+#endif
+constexpr int AD_IB = MD_AD_IB;   // particles i per thread for large N; 1 below AD_SMALL_N (more, shorter blocks: the
 constexpr int AD_SMALL_N = 8192;  // kernel is latency-bound there, profiles/r01_final_cfg2.md)
-constexpr int AD_UNROLL = 8;      // tests per i between two candidate checks
+constexpr int AD_UNROLL = MD_AD_UNROLL;   // tests per i between two candidate checks
 
 struct AllPairsDot {
     Vec4<double>* jv;      // [nv + cap_ghost]: real vapor entries in particle order, then this step's ghosts
@@ -160,17 +166,25 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double
     const int nvj = p.nv + *a.ghost_count;
     const int tiles_v = (nvj + AD_THREADS - 1) / AD_THREADS, tiles_w = (a.nwg + AD_THREADS - 1) / AD_THREADS;
     const int thr = a.thr_hi;
+    // the tile after the current one is fetched into a register while the current one is evaluated, so a block never
+    // waits for a global load between two tiles (it did: two barriers and an L2 round trip every 128 entries)
+    auto fetch = [&](int t) {
+        Vec4<double> e = {-1.0e9, -1.0e9, -1.0e9, 3.0e18};              // padding: far from everything
+        if (t < tiles_v + tiles_w) {
+            const bool w = t >= tiles_v;
+            const int j = (w ? t - tiles_v : t) * AD_THREADS + threadIdx.x;
+            if (j < (w ? a.nwg : nvj)) e = (w ? a.jw : a.jv)[j];
+        }
+        return e;
+    };
+    Vec4<double> nxt = fetch(blockIdx.y);
     for (int t = blockIdx.y; t < tiles_v + tiles_w; t += gridDim.y) {
         const bool wall = t >= tiles_v;
         const int j0 = (wall ? t - tiles_v : t) * AD_THREADS;
-        const int nj = wall ? a.nwg : nvj;
         __syncthreads();
-        {
-            Vec4<double> e = {-1.0e9, -1.0e9, -1.0e9, 3.0e18};          // padding: far from everything
-            if (j0 + threadIdx.x < nj) e = (wall ? a.jw : a.jv)[j0 + threadIdx.x];
-            sj[threadIdx.x] = e;
-        }
+        sj[threadIdx.x] = nxt;
         __syncthreads();
+        nxt = fetch(t + gridDim.y);
         for (int k0 = 0; k0 < AD_THREADS; k0 += AD_UNROLL) {
             int cand = 0;
 #pragma unroll

@@ -255,7 +255,7 @@ struct Sim : md_sim {
     int curv = 0, coop_grid = 0, coop_base = 0, coop_max = 0, heavy_seen = 0, heavy32_seen = 0;
     int minb3_threshold = -1;   // particles beyond which the 3-blocks-per-SM build runs; set at the first launch
     long long rebuilds_seen = 0;
-    unsigned long long phase_seen[8] = {}, phase_ns[8] = {};
+    unsigned long long phase_ns[8] = {};
 
     md::AllPairsDot ad;
     md::AllPairsDotF adf;
@@ -489,28 +489,44 @@ struct Sim : md_sim {
             int rc = refresh();
             if (rc) return rc;
             const long long r0 = rebuilds_seen;
+            unsigned long long t[8], tb[8];                 // the kernel's own timers are cumulative: take the difference
+            CK(cudaMemcpy(tb, l.vtimes, sizeof(tb), cudaMemcpyDeviceToHost));
             CK(cudaEventRecord(ev[0], stream));
             if (n > 0 && (rc = launch_run(n, 0))) return rc;
             CK(cudaEventRecord(ev[1], stream));
             if ((rc = refresh())) return rc;
             float ms = 0.f;
             CK(cudaEventElapsedTime(&ms, ev[0], ev[1]));
-            unsigned long long t[8];
             CK(cudaMemcpy(t, l.vtimes, sizeof(t), cudaMemcpyDeviceToHost));
 #ifdef MD_DIAGNOSTICS
             if (getenv("MD_DEBUG_TIMES")) {
                 std::vector<unsigned long long> w(8192);
                 CK(cudaMemcpy(w.data(), l.vtimes + 8, 8192 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
                 const int nwarp = coop_grid * md::VL_THREADS / 32;
-                unsigned long long mx = 0, sm = 0;
-                for (int k = 0; k < nwarp && k < 8192; ++k) { mx = std::max(mx, w[k]); sm += w[k]; }
-                fprintf(stderr, "[md] per-warp cumulative step-phase us: max %.0f mean %.0f\n", mx * 1e-3, sm * 1e-3 / nwarp);
-                int nh = 0;
-                CK(cudaMemcpy(&nh, l.vflags + md::VF_NHEAVY, sizeof(int), cudaMemcpyDeviceToHost));
-                fprintf(stderr, "[md] heavy particles (list > %d entries) after the last rebuild: %d\n", vl.heavy_t, nh);
+                const int nbl = std::min(coop_grid, cdiv(p.nv, md::VL_THREADS)), wpb = md::VL_THREADS / 32;
+                double mx[2] = {0, 0}, sm[2] = {0, 0};
+                int cnt[2] = {0, 0};
+                for (int k = 0; k < nwarp && k < 8192; ++k) {
+                    const int g = k / wpb >= nbl;
+                    mx[g] = std::max(mx[g], (double)w[k]); sm[g] += (double)w[k]; ++cnt[g];
+                }
+                const double per = 1e-3 / std::max<long long>(step_no + n, 1);
+                fprintf(stderr, "[md] step-phase us per step and warp (cumulative / steps): particle blocks (%d) max %.2f mean %.2f | idle blocks (%d) max %.2f mean %.2f\n",
+                        nbl, mx[0] * per, sm[0] * per / std::max(cnt[0], 1), coop_grid - nbl, mx[1] * per, sm[1] * per / std::max(cnt[1], 1));
+                {
+                    double mxp = 0, mxi = 0;
+                    for (int k = 0; k < nwarp && k < 4000; ++k) (k / wpb >= nbl ? mxi : mxp) = std::max(k / wpb >= nbl ? mxi : mxp, (double)w[4096 + k]);
+                    fprintf(stderr, "[md] longest single step phase of any warp: particle blocks %.1f us, idle blocks %.1f us; histogram of warp-phase times (1.024 us bins):", mxp * 1e-3, mxi * 1e-3);
+                    for (int k = 0; k < 16; ++k) fprintf(stderr, " %llu", w[8000 + k]);
+                    fprintf(stderr, "\n");
+                }
+                int hh[md::VF_COUNT];
+                CK(cudaMemcpy(hh, l.vflags, sizeof(hh), cudaMemcpyDeviceToHost));
+                fprintf(stderr, "[md] after the last rebuild: lists > %d entries %d (lane groups hold %d), lists > %d entries %d (warps hold %d)\n",
+                        vl.heavy_t, hh[md::VF_NHEAVY], hh[md::VF_HCAP], md::VL_WARP_T, hh[md::VF_NHEAVY32], hh[md::VF_HCAP32]);
             }
 #endif
-            for (int q = 0; q < 8; ++q) { phase_ns[q] = t[q] - phase_seen[q]; phase_seen[q] = t[q]; }
+            for (int q = 0; q < 8; ++q) phase_ns[q] = t[q] - tb[q];
             for (int q = 0; q < 4; ++q) out->rebuild_ms[q] = phase_ns[4 + q] * 1e-6;   // bin, scan, scatter, list build
             // VERLET: ms[0] step phases, ms[1] grid barriers, ms[2] rebuilds (as seen by thread 0), ms[3] whole launch
             out->ms[0] = phase_ns[0] * 1e-6; out->ms[1] = phase_ns[1] * 1e-6; out->ms[2] = phase_ns[2] * 1e-6;

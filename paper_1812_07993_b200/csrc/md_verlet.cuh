@@ -72,7 +72,8 @@ struct Verlet {
                                // longer than VL_WARP_T (registered from the top of `cell` / `slot` downwards)
 };
 
-// ncnt word of a particle: vapor entries in list slots [0, nvv), wall entries in [nvv, nvv + nvw); face code = 2 bits
+// ncnt word of a particle: vapor entries in list slots [0, nvv), wall entries in the LAST nvw slots [VL_MAXN - nvw,
+// VL_MAXN) (the two are appended by different warps of the build, from the two ends); face code = 2 bits
 // per dimension, 1 = the particle sat in the FIRST cell of a periodic dimension when the list was built (its ghost is
 // the copy at +L), 2 = in the LAST cell (ghost at -L); heavy = list walked by a lane group (see phase_step).
 constexpr int VL_NVV_MASK = 0xff, VL_NVW_SHIFT = 8, VL_NVW_MASK = 0xff, VL_FACE_SHIFT = 16, VL_FACE_MASK = 0x3f;
@@ -84,8 +85,8 @@ __device__ __forceinline__ int vl_face(int raw) { return (raw >> VL_FACE_SHIFT) 
 #define MD_VL_GROUP 4
 #endif
 constexpr int VL_GROUP = MD_VL_GROUP;   // lanes sharing one heavy particle's list
-constexpr int VL_WARP_T = 32;           // lists longer than this (inside an adsorbed film: up to ~100 entries) get a whole warp
-constexpr int VL_WARP_ROUNDS = 2;       // such lists per idle warp and step
+constexpr int VL_WARP_T = 48;           // lists longer than this (inside an adsorbed film: up to ~100 entries) get a whole warp
+constexpr int VL_WARP_ROUNDS = 1;       // such lists per idle warp and step
 
 // d = a - b folded to the nearest image by comparison (|true d| < r_c + skin < L/2): fp32 mode only, where a ghost
 // copy x + L would round the coordinate.  The shift goes on whichever particle sits at the top of the box so the
@@ -234,7 +235,7 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
     else list_loop<T, ENERGY, false>(p, qv, lst, v.stride, nvv, r, ri, j0, av);
     if (__any_sync(__activemask(), nvw != 0)) {             // walls: a few per cent of the particles have any
         const PairCoef<T> qw = coef_vw(p);
-        const int* __restrict__ lw = lst + (size_t)nvv * v.stride;
+        const int* __restrict__ lw = lst + (size_t)(VL_MAXN - nvw) * v.stride;
         int w0[VL_BATCH];
 #pragma unroll
         for (int u = 0; u < VL_BATCH; ++u) w0[u] = u < nvw ? lw[(size_t)u * v.stride] : -1;
@@ -275,7 +276,7 @@ __device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* _
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const int kk = k + 4 * VL_GROUP + sub + VL_GROUP * u;
-            jn[u] = kk < n ? lst[(size_t)kk * stride] : -1;
+            jn[u] = kk < n ? lst[(size_t)(kk < nvv ? kk : kk + VL_MAXN - n) * stride] : -1;   // wall entries sit at the top
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -439,7 +440,10 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
                 int j[4];
                 Vec4<T> rj[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) j[u] = lane + 32 * u < n ? v.nbr[(size_t)(lane + 32 * u) * v.stride + i] : -1;
+                for (int u = 0; u < 4; ++u) {
+                    const int k = lane + 32 * u;
+                    j[u] = k < n ? v.nbr[(size_t)(k < nvv ? k : k + VL_MAXN - n) * v.stride + i] : -1;
+                }
                 const Vec4<T> ri = rcur[i];
                 T vx = T(0), vy = T(0), vz = T(0);
                 if (lane == 0) { vx = lam * s.vx[i]; vy = lam * s.vy[i]; vz = lam * s.vz[i]; }
@@ -482,7 +486,10 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             } else {
                 i = v.cell[h]; raw = v.slot[h];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) j0[u] = v.nbr[(size_t)(sub + VL_GROUP * u) * v.stride + i];
+                for (int u = 0; u < 4; ++u) {
+                    const int k = sub + VL_GROUP * u, nv0 = vl_nvv(raw), n0 = nv0 + vl_nvw(raw);
+                    j0[u] = v.nbr[(size_t)(k < nv0 || k >= n0 ? k : k + VL_MAXN - n0) * v.stride + i];
+                }
                 if (sub == 0) { vx = s.vx[i]; vy = s.vy[i]; vz = s.vz[i]; }
             }
             const Vec4<T> ri = rcur[i];
@@ -637,27 +644,6 @@ __device__ __forceinline__ void phase_scatter(const Params<T>& p, const Verlet<T
     }
 }
 
-// End of a particle's list build: the ncnt word, the heavy registries, overflow, its ghost copies.
-template <typename T>
-__device__ __forceinline__ void finish_list(const Params<T>& p, const Verlet<T>& v, Vec4<T>* __restrict__ r, int i,
-                                            const Vec4<T>& ri, int n, int nvv, int face, int hcap, int hcap32)
-{
-    const int nn = min(n, VL_MAXN), nv0 = min(nvv, nn);
-    int raw = nv0 | ((nn - nv0) << VL_NVW_SHIFT) | (face << VL_FACE_SHIFT);
-    // a long list goes to a lane group (a very long one to a warp) while the idle blocks have some left; the counters
-    // keep the demand and the host sizes the next launch by it; `cell` and `slot` are free until the next rebuild
-    if (n > max(VL_WARP_T, v.heavy_t) && hcap32 > 0) {
-        const int h = atomicAdd(v.flags + VF_NHEAVY32, 1);
-        if (h < hcap32) { raw |= VL_HEAVY; v.cell[p.nv - 1 - h] = i; v.slot[p.nv - 1 - h] = raw; }
-    } else if (n > v.heavy_t) {
-        const int h = atomicAdd(v.flags + VF_NHEAVY, 1);
-        if (h < hcap) { raw |= VL_HEAVY; v.cell[h] = i; v.slot[h] = raw; }
-    }
-    v.ncnt[i] = raw;
-    if (n > VL_MAXN) v.flags[VF_OVERFLOW] = 1;
-    if (sizeof(T) == 8 && face) write_ghosts(p, v, r, i, ri, face);
-}
-
 template <typename T>
 __device__ __forceinline__ int face_code(const Params<T>& p, int cx, int cy, int cz)
 {
@@ -668,161 +654,131 @@ __device__ __forceinline__ int face_code(const Params<T>& p, int cx, int cy, int
     return face;
 }
 
-// R4: neighbour list from the cell list (a3's cell traversal, cached): every j within r_c + skin of i, vapor entries
-// first, then wall entries.  The distance filter runs in FP32 on the fp32 shadow of the positions with a threshold
-// inflated by the rounding involved: the list is a superset of the pairs within r_c + skin, which is all the exactness
-// argument needs (fp64: an entry names the image block the time loop will read; fp32 mode stores plain indices and
-// folds).  Positions are wrapped here.
+// End of a particle's list build: the ncnt word, the heavy registries, overflow, its ghost copies.
+template <typename T>
+__device__ __forceinline__ void finish_list(const Params<T>& p, const Verlet<T>& v, Vec4<T>* __restrict__ r, int i,
+                                            const Vec4<T>& ri, int nvv, int nvw, int face, int hcap, int hcap32)
+{
+    const int n = nvv + nvw;
+    int raw = min(nvv, VL_MAXN) | (min(nvw, VL_MAXN) << VL_NVW_SHIFT) | (face << VL_FACE_SHIFT);
+    if (n > VL_MAXN) { v.flags[VF_OVERFLOW] = 1; raw = face << VL_FACE_SHIFT; }      // reported by the host; the list is not used
+    // a long list goes to a lane group (a very long one to a warp) while the idle blocks have some left; the counters
+    // keep the demand and the host sizes the next launch by it; `cell` and `slot` are free until the next rebuild
+    // (what its own thread would pay is batches, and the two kinds of entries are batched separately: six vapor and six
+    // wall entries cost four batches where twelve vapor entries cost three)
+    else if (n > v.heavy_t || ((nvv + VL_BATCH - 1) / VL_BATCH + (nvw + VL_BATCH - 1) / VL_BATCH) * VL_BATCH > v.heavy_t + VL_BATCH - 1) {
+        bool placed = false;
+        if (n > VL_WARP_T && hcap32 > 0) {
+            const int h = atomicAdd(v.flags + VF_NHEAVY32, 1);
+            placed = h < hcap32;
+            if (placed) { raw |= VL_HEAVY; v.cell[p.nv - 1 - h] = i; v.slot[p.nv - 1 - h] = raw; }
+        }
+        if (!placed) {                                   // no warp left: four lanes are still better than one
+            const int h = atomicAdd(v.flags + VF_NHEAVY, 1);
+            if (h < hcap) { raw |= VL_HEAVY; v.cell[h] = i; v.slot[h] = raw; }
+        }
+    }
+    v.ncnt[i] = raw;
+    if (sizeof(T) == 8 && face) write_ghosts(p, v, r, i, ri, face);
+}
+
+// R4: neighbour list from the cell list (a3's cell traversal, cached): every j within r_c + skin of i, vapor entries from
+// slot 0 up, wall entries from the top slot down.  ROWS = 3^(d-1) lanes cooperate on one particle: lane `row` walks the
+// cell row (cy + ky, cz + kz) -- its three cells are one contiguous range of the cell-ordered arrays, plus the wrapped
+// cell at a periodic x face -- eight candidate loads in flight at a time, and appends its hits through two
+// shared-memory counters.  The periodic image is applied once per row / segment as a shift of r_i, and an entry records
+// the image block of the ghost copy the time loop will read (fp64; fp32 mode stores plain indices and folds).  The
+// distance filter runs in FP32 on the fp32 shadow of the positions with a threshold inflated by the rounding involved: the
+// list is a superset of the pairs within r_c + skin, which is all the exactness argument needs.  Positions are wrapped here.
 //
-// With <= 4 warps per scheduler a warp instruction costs ~8 cycles here, whatever it is, so what bounds this phase is the
-// number of instructions a warp executes: three designs that walk each particle's 3^d cells with per-lane loops
-// (9 lanes per particle, one thread per particle, a warp sweeping its 32 particles' rows through shared-memory windows)
-// all took 40-45 us from N = 1024 to 65,536, at 10 % lane efficiency (profiles/r02_k_md_run.md).  This one has no
-// divergent loop: the unit of work is a SUPER-CELL of SX x SY x SZ cells (4 x 2 x 2: ~24 particles at density 0.05), one
-// warp each.  The warp gathers the candidates of the whole super-cell -- the (SX + 2)(SY + 2)(SZ + 2) cells around it, each
-// cell row one contiguous range, image shifts and list-entry codes applied on the way -- into a shared-memory tile with
-// coalesced loads, then lane l owns member particle l and scans the tile: broadcast reads, the same trip count in every
-// lane, a private append counter.  A lane tests ~3.5x the candidates its own 3^d cells hold, and the warp still executes
-// 6x fewer instructions.  Dense super-cells (an adsorbed film) take more member rounds and tile chunks of the same loop;
-// wall particles are a second pass over the wall tile.
-constexpr int VL_SX = 4, VL_SY = 2, VL_TILE = 256;
+// Why this shape (profiles/r02_k_md_run.md): vapor at density 0.05 and T* = 1 condenses, so a few hundred particles sit in
+// clusters and films with ten times the candidates of the rest, and the phase ends when the slowest warp does.  Units of
+// work whose cost grows with the SQUARE of the local density -- a warp per block of cells, candidates in a tile: measured
+// at 45-60 us -- lose to this one, where a particle's candidates are spread over nine lanes and three particles share a
+// warp: its cost is linear in the density (39 us in round 1, in FP64 with folds).
+template <typename T>
+__device__ __forceinline__ void list_range(const F4* __restrict__ q, int jb, int je, int skip, float xe, float ye, float ze, float rl2,
+                                           int e0, int* __restrict__ lst, size_t stride, int* cnt, bool up)
+{
+    constexpr int NB = 8;                                                // a cell row rarely holds more
+    for (int j0 = jb; j0 < je; j0 += NB) {
+        F4 rj[NB];
+#pragma unroll
+        for (int u = 0; u < NB; ++u) rj[u] = q[min(j0 + u, je - 1)];     // NB loads in flight
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            const int j = j0 + u;
+            const float dx = xe - rj[u].x, dy = ye - rj[u].y, dz = ze - rj[u].z;
+            if (j < je && j != skip && fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < rl2) {
+                const int k = atomicAdd(cnt, 1);
+                if (k < VL_MAXN) lst[(size_t)(up ? k : VL_MAXN - 1 - k) * stride] = e0 + j;
+            }
+        }
+    }
+}
 
 template <typename T, int ROWS>
 __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>& v, int c, int gtid, int gthreads, int hcap,
                                             int hcap32)
 {
     constexpr bool GHOSTS = sizeof(T) == 8;
-    constexpr int NW = VL_THREADS / 32, SX = VL_SX, SY = VL_SY, SZ = ROWS == 9 ? 2 : 1;
-    constexpr int NR = (SY + 2) * (ROWS == 9 ? SZ + 2 : 1);      // candidate rows of a super-cell
-    constexpr int NSEG = 3 * NR;                                 // per row: cells inside the box, image of the last cell, image of the first
-    constexpr unsigned FULL = 0xffffffffu;
-    __shared__ float4 s_tile[NW][VL_TILE];                       // (x, y, z) of a candidate in the super-cell's frame, w = bits of its list entry
-    __shared__ int s_excl[NW][NSEG + 1], s_b[NW][NSEG], s_e0[NW][NSEG];
-    __shared__ float s_sx[NW][NSEG], s_sy[NW][NSEG], s_sz[NW][NSEG];
-    __shared__ int s_mexcl[NW][SY * SZ + 1], s_mb[NW][SY * SZ];
+    constexpr int PPW = 32 / ROWS;                       // particles per warp
+    __shared__ int s_cv[(VL_THREADS / 32) * PPW], s_cw[(VL_THREADS / 32) * PPW];
     Vec4<T>* __restrict__ r = v.st[c].r;
     const F4* __restrict__ q = GHOSTS ? v.r32 : reinterpret_cast<const F4*>(r);
-    const float rl2 = v.rl2f;
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int nx = p.nc[0], ny = p.nc[1], nz = p.nc[2];
-    const int nsx = (nx + SX - 1) / SX, nsy = (ny + SY - 1) / SY, nsz = (nz + SZ - 1) / SZ;
-    const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
-    for (int task = gtid >> 5; task < nsx * nsy * nsz; task += gthreads >> 5) {
-        const int sx0 = (task % nsx) * SX, sy0 = ((task / nsx) % nsy) * SY, sz0 = (task / (nsx * nsy)) * SZ;
-        // ---- members: the particles of the super-cell's own rows (clipped to the box)
-        {
-            int mb = 0, len = 0;
-            if (lane < SY * SZ) {
-                const int cy = sy0 + lane % SY, cz = sz0 + lane / SY;
-                if (cy < ny && cz < nz) {
-                    const int rowc = (cz * ny + cy) * nx;
-                    mb = v.start[rowc + sx0];
-                    len = v.start[rowc + min(sx0 + SX, nx)] - mb;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int pl = lane / ROWS, row = lane - pl * ROWS;
+    const int warp = gtid >> 5, nwarps = gthreads >> 5;
+    int* cv = s_cv + wib * PPW + min(pl, PPW - 1);
+    int* cw = s_cw + wib * PPW + min(pl, PPW - 1);
+    const int istride = GHOSTS ? v.ntot : 0;
+    for (int base = warp * PPW; base < p.nv; base += nwarps * PPW) {
+        const int i = base + pl;
+        const bool active = pl < PPW && i < p.nv;
+        if (active && row == 0) { *cv = 0; *cw = 0; }
+        __syncwarp();
+        Vec4<T> ri = {T(0), T(0), T(0), T(0)};
+        int face = 0;
+        if (active) {
+            ri = r[i];
+            int cx, cy, cz;
+            const int ci = cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
+            face = face_code(p, cx, cy, cz);
+            int qy = cy + row % 3 - 1, qz = cz + (ROWS == 9 ? row / 3 - 1 : 0);
+            bool ok = true;
+            float ye = (float)ri.y, ze = (float)ri.z;
+            int img = 0;
+            // r_i in the first cell looking at the last one: the neighbour's image is at r_j - L, i.e. r_i + L
+            if (qz < 0) { ok = p.bc[2] == BC_PERIODIC; qz += nz; ze += (float)p.L[2]; img |= 4; }
+            else if (qz >= nz) { ok = p.bc[2] == BC_PERIODIC; qz -= nz; ze -= (float)p.L[2]; img |= 4; }
+            if (qy < 0) { ok = ok && p.bc[1] == BC_PERIODIC; qy += ny; ye += (float)p.L[1]; img |= 2; }
+            else if (qy >= ny) { ok = ok && p.bc[1] == BC_PERIODIC; qy -= ny; ye -= (float)p.L[1]; img |= 2; }
+            if (ok) {
+                const int x0 = max(cx - 1, 0), x1 = min(cx + 1, nx - 1);
+                int xw = -1;
+                float xe = (float)ri.x, xe2 = xe;
+                if (p.bc[0] == BC_PERIODIC) { if (cx == 0) { xw = nx - 1; xe2 += (float)p.L[0]; } else if (cx == nx - 1) { xw = 0; xe2 -= (float)p.L[0]; } }
+                const int rowc = (qz * ny + qy) * nx;
+                const bool do_wall = p.nw > 0 && v.wnear[ci];
+                // all cell-start loads first (independent), then the particle loops
+                const int jb = v.start[rowc + x0], je = v.start[rowc + x1 + 1];
+                int jb2 = 0, je2 = 0, wb = 0, we = 0, wb2 = 0, we2 = 0;
+                if (xw >= 0) { jb2 = v.start[rowc + xw]; je2 = v.start[rowc + xw + 1]; }
+                if (do_wall) {
+                    wb = v.wstart[rowc + x0]; we = v.wstart[rowc + x1 + 1];
+                    if (xw >= 0) { wb2 = v.wstart[rowc + xw]; we2 = v.wstart[rowc + xw + 1]; }
                 }
-            }
-            const int incl = warp_incl_scan(len);
-            __syncwarp();
-            if (lane < SY * SZ) { s_mexcl[wib][lane] = incl - len; s_mb[wib][lane] = mb; }
-            if (lane == SY * SZ) s_mexcl[wib][SY * SZ] = incl;      // = total (lanes past the last row add 0)
-            __syncwarp();
-        }
-        const int mtotal = s_mexcl[wib][SY * SZ];
-        if (mtotal == 0) continue;
-        for (int pass = 0; pass < 2; ++pass) {
-            if (pass == 1 && p.nw == 0) break;
-            const int* __restrict__ st = pass ? v.wstart : v.start;
-            const int base = pass ? p.nv : 0;
-            // ---- candidate segments: row (sy0 - 1 + a, sz0 - 1 + b), kind 0 = its cells sx0 - 1 .. sx0 + SX inside the box,
-            // kind 1 = the image of the last cell at -L (super-cell at the low x face), kind 2 = the image of the first at +L
-            int total = 0;
-            __syncwarp();
-            for (int s0 = 0; s0 < NSEG; s0 += 32) {
-                const int sg = s0 + lane;
-                int sb = 0, len = 0, img = 0;
-                float fx = 0.f, fy = 0.f, fz = 0.f;
-                if (sg < NSEG) {
-                    const int row = sg % NR, kind = sg / NR;
-                    int qy = sy0 - 1 + row % (SY + 2), qz = ROWS == 9 ? sz0 - 1 + row / (SY + 2) : 0;
-                    bool ok = qy <= min(sy0 + SY, ny) && qz <= min(sz0 + SZ, nz);     // rows beyond a clipped super-cell's neighbours
-                    // a row below the box is the image at -L of the last row (candidates move DOWN by L), one above at +L
-                    if (qz < 0) { ok = ok && pz; qz += nz; fz = -(float)p.L[2]; img |= 4; }
-                    else if (qz >= nz) { ok = ok && pz; qz -= nz; fz = (float)p.L[2]; img |= 4; }
-                    if (qy < 0) { ok = ok && py; qy += ny; fy = -(float)p.L[1]; img |= 2; }
-                    else if (qy >= ny) { ok = ok && py; qy -= ny; fy = (float)p.L[1]; img |= 2; }
-                    int c0 = 0, c1 = -1;                                               // cells c0 .. c1 of the row
-                    if (kind == 0) { c0 = max(sx0 - 1, 0); c1 = min(sx0 + SX, nx - 1); }
-                    else if (kind == 1) { if (px && sx0 == 0) { c0 = c1 = nx - 1; fx = -(float)p.L[0]; img |= 1; } }
-                    else { if (px && sx0 + SX >= nx) { c0 = c1 = 0; fx = (float)p.L[0]; img |= 1; } }
-                    if (ok && c1 >= c0) {
-                        const int rowc = (qz * ny + qy) * nx;
-                        sb = st[rowc + c0];
-                        len = st[rowc + c1 + 1] - sb;
-                    }
-                }
-                const int incl = warp_incl_scan(len);
-                if (sg < NSEG) {
-                    s_excl[wib][sg] = total + incl - len; s_b[wib][sg] = sb; s_e0[wib][sg] = (GHOSTS ? img * v.ntot : 0) + base;
-                    s_sx[wib][sg] = fx; s_sy[wib][sg] = fy; s_sz[wib][sg] = fz;
-                }
-                total += __shfl_sync(FULL, incl, 31);
-            }
-            if (lane == 0) s_excl[wib][NSEG] = total;
-            __syncwarp();
-            // ---- member rounds x tile chunks (pass 1 runs even without a wall nearby: it closes the members' lists)
-            for (int m0 = 0; m0 < mtotal; m0 += 32) {
-                const bool live = m0 + lane < mtotal;
-                int i = 0;
-                if (live) {
-                    int ms = 0;
-                    while (m0 + lane >= s_mexcl[wib][ms + 1]) ++ms;
-                    i = s_mb[wib][ms] + (m0 + lane - s_mexcl[wib][ms]);
-                }
-                const F4 qi = q[i];
                 int* __restrict__ lst = v.nbr + i;
-                int n = pass && live ? vl_nvv(v.ncnt[i]) : 0;            // pass 1 appends after the vapor entries
-                const int n0 = n;
-                int seg = 0;
-                for (int ch0 = 0; ch0 < total; ch0 += VL_TILE) {
-                    __syncwarp();
-#pragma unroll
-                    for (int u = 0; u < VL_TILE / 32; ++u) {               // gather: 8 independent loads per lane
-                        const int k = ch0 + 32 * u + lane;
-                        if (k < total) {
-                            while (k >= s_excl[wib][seg + 1]) ++seg;     // segments only move forward with k
-                            const int j = s_b[wib][seg] + (k - s_excl[wib][seg]);
-                            const F4 rj = q[base + j];
-                            s_tile[wib][32 * u + lane] = make_float4(rj.x + s_sx[wib][seg], rj.y + s_sy[wib][seg], rj.z + s_sz[wib][seg],
-                                                                     __int_as_float(s_e0[wib][seg] + j));
-                        }
-                    }
-                    __syncwarp();
-                    if (live) {
-                        const int cnt = min(VL_TILE, total - ch0);
-#pragma unroll 4
-                        for (int k = 0; k < cnt; ++k) {
-                            const float4 cj = s_tile[wib][k];
-                            const float dx = qi.x - cj.x, dy = qi.y - cj.y, dz = qi.z - cj.z;
-                            const int e = __float_as_int(cj.w);
-                            if (fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < rl2 && e != i) {
-                                if (n < VL_MAXN) lst[(size_t)n * v.stride] = e;
-                                ++n;
-                            }
-                        }
-                    }
-                }
-                if (live) {
-                    if (pass == 0 && p.nw > 0) {                         // parked for the wall pass (same lane of the same warp)
-                        v.ncnt[i] = min(n, VL_MAXN);
-                        if (n > VL_MAXN) v.flags[VF_OVERFLOW] = 1;
-                    } else {
-                        const Vec4<T> ri = r[i];
-                        int cx, cy, cz;
-                        cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
-                        finish_list(p, v, r, i, ri, n, pass ? n0 : n, face_code(p, cx, cy, cz), hcap, hcap32);
-                    }
-                }
+                list_range<T>(q, jb, je, img ? -1 : i, xe, ye, ze, v.rl2f, img * istride, lst, v.stride, cv, true);
+                list_range<T>(q, jb2, je2, -1, xe2, ye, ze, v.rl2f, (img | 1) * istride, lst, v.stride, cv, true);
+                list_range<T>(q + p.nv, wb, we, -1, xe, ye, ze, v.rl2f, img * istride + p.nv, lst, v.stride, cw, false);
+                list_range<T>(q + p.nv, wb2, we2, -1, xe2, ye, ze, v.rl2f, (img | 1) * istride + p.nv, lst, v.stride, cw, false);
             }
         }
+        __syncwarp();
+        if (active && row == 0) finish_list(p, v, r, i, ri, *cv, *cw, face, hcap, hcap32);
+        __syncwarp();
     }
 }
 
@@ -891,7 +847,12 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
             phase_step<T>(p, v, c, cv, false, false, true, req, gtid, gthreads, (T)lam);
         }
 #ifdef MD_DIAGNOSTICS
-        if (v.dbg && (threadIdx.x & 31) == 0) atomicAdd(v.dbg + (gtid >> 5), now_ns() - dbg0);
+        if (v.dbg && (threadIdx.x & 31) == 0) {
+            const unsigned long long dt = now_ns() - dbg0;
+            atomicAdd(v.dbg + (gtid >> 5), dt);
+            if (s > 0 && !rebuild) atomicMax(v.dbg + 4096 + (gtid >> 5), dt);
+            atomicAdd(v.dbg + 8000 + min((int)(dt >> 10), 15), 1ull);       // histogram of warp-phase times, ~1 us bins
+        }
 #endif
         if (gtid == 0) { t1 = now_ns(); s_times[0] += t1 - t0; t0 = t1; }
         grid_barrier(v.bar, bar_seq);
