@@ -264,24 +264,31 @@ def paper_size(dim, seed=BASE_SEED + 9):
                    "allpairs")
 
 
-def paper_geometry(dim, seed=BASE_SEED + 20):
+def paper_geometry(dim, seed=BASE_SEED + 20, n_pore=None):
     """The paper's own runs in reduced units (NEXT-3; readings A16 of DESIGN.md): a pore with GEOMETRIC reflecting walls
     (no wall particles), open at +x into an outer space with periodic boundaries, pore : outside density 5 : 1.
     2D: square pore 1 um x 1 um with 420 molecules, outer space 1764, 35 C.
     3D: prism 500 x 50 x 50 nm with 1000 molecules, outer space 1800 with 9x the volume, 25 C.
     dt = 0.016 ps = 0.00959 tau.  The gas is so dilute (4e-5 sigma^-2) that a cell grid would hold ~1e7 empty cells:
-    the all-pairs kernel is the one to use, as in the paper."""
+    the all-pairs kernel is the one to use, as in the paper.
+    n_pore: molecules in the pore for the sweeps of Tables 2-3 (N = 100 ... 1500 "in the pore",
+    pore : outside density ratio 5 : 1 kept): same geometry, 4.2 n_pore (2D) / 1.8 n_pore (3D) molecules outside, i.e.
+    N_tot = 5.2 N / 2.8 N (reading A14)."""
     from . import units
 
     rng = SplitMix64(seed + dim)
     if dim == 2:
         l = units.length_reduced(1.0e-6)
         n_in, n_out, t_star = 420, 1764, units.temperature_reduced(35.0)
+        if n_pore is not None:
+            n_in, n_out = int(n_pore), int(round(4.2 * n_pore))
         box = (4.0 * l + 4.0, 7.0 * l)                              # pore + k = 3 pore widths of outer space, 2k + 1 tall
         lo, hi = np.array([2.0, 3.0 * l]), np.array([2.0 + l, 4.0 * l])
     else:
         lx, lw = units.length_reduced(500e-9), units.length_reduced(50e-9)
         n_in, n_out, t_star = 1000, 1800, units.temperature_reduced(25.0)
+        if n_pore is not None:
+            n_in, n_out = int(n_pore), int(round(1.8 * n_pore))
         box = (10.0 * lx + 4.0, lw + 4.0, lw + 4.0)                 # outer space: same cross-section, 9x the length
         lo, hi = np.array([2.0, 2.0, 2.0]), np.array([2.0 + lx, 2.0 + lw, 2.0 + lw])
     L = np.array(box)

@@ -52,7 +52,8 @@ def measure(cfg, algo, precision, n_steps, torch, md, peaks):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--configs", default="0,1,2,3,4,5", help="0-4: BASELINE.json configs; 5: the paper's problem sizes")
+    ap.add_argument("--configs", default="0,1,2,3,4,5", help="0-4: BASELINE.json configs; 5: the paper's problem sizes; "
+                    "6: the paper's N sweeps of Tables 2-3 (N_pore = 100 ... 1500)")
     ap.add_argument("--max-log2n", type=int, default=20)
     ap.add_argument("--min-log2n", type=int, default=10)
     ap.add_argument("--paths", default="allpairs,cells,verlet", help="force paths to run (subset)")
@@ -106,6 +107,10 @@ def main():
             for algo in ("allpairs", "cells", "verlet"):
                 add(cfg, algo, 64, 2000)
             add(I.paper_geometry(dim), "allpairs", 64, 2000)      # the paper's geometry, units and 2000 steps (NEXT-3)
+    if 6 in want:      # Tables 2-3: N molecules in the pore, N_tot = 5.2 N (2D) / 2.8 N (3D), 2000 steps
+        for dim in (2, 3):
+            for n_pore in range(100, 1501, 100):
+                add(I.paper_geometry(dim, n_pore=n_pore), "allpairs", 64, 2000)
     if 4 in want:
         for log2n in range(args.min_log2n, args.max_log2n + 1, 2):
             cfg = I.config4(log2n)

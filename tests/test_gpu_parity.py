@@ -564,15 +564,20 @@ def test_geometric_prism_pore_matches_oracle(algo):
     assert e.value.code == md.MD_ERR_INVALID_ARG
 
 
+@pytest.mark.parametrize("n_pore", [None, 100, 1500])
 @pytest.mark.parametrize("dim", [2, 3])
-def test_paper_geometry_and_units_match_oracle(dim):
-    # NEXT-3: the paper's own runs in reduced units, geometric walls, all-pairs
-    cfg = I.paper_geometry(dim)
-    assert cfg["n_vapor"] == (2184 if dim == 2 else 2800) and abs(cfg["dt"] - 0.00959) < 1e-5
-    ref = O.run(cfg, 200)
+def test_paper_geometry_and_units_match_oracle(dim, n_pore):
+    # NEXT-3: the paper's own runs in reduced units, geometric walls, all-pairs; and the end
+    # points of its N sweeps (Tables 2-3: N = 100 and 1500 molecules in the pore)
+    cfg = I.paper_geometry(dim, n_pore=n_pore)
+    n_tot = {None: 2184 if dim == 2 else 2800, 100: 520 if dim == 2 else 280, 1500: 7800 if dim == 2 else 4200}[n_pore]
+    assert cfg["n_vapor"] == n_tot and abs(cfg["dt"] - 0.00959) < 1e-5
+    # 200 steps; 2000 for the 100-molecule pore, where 200 steps (3.8 sigma of flight in a 3155 sigma pore) see no bounce
+    n_steps = 2000 if n_pore == 100 else 200
+    ref = O.run(cfg, n_steps)
     assert not np.array_equal(np.sign(ref["vel"]), np.sign(cfg["vel"]))          # some molecules did bounce
     sim = md.Simulation(cfg, algo="allpairs")
-    sim.step(200)
+    sim.step(n_steps)
     st = sim.get_state()
     assert traj_error(st["pos"], ref["pos"], cfg["box_len"], cfg["bc"]) <= TRAJ_TOL
     assert np.abs(st["vel"] - ref["vel"]).max() <= 1e-7
