@@ -159,6 +159,21 @@ int md_info(const md_sim*, int* force_algo, int n_cells[3], int* kernels_per_ste
  * meaningful copy figure. */
 int md_measure_peaks(void* device_scratch, size_t scratch_bytes, void* cuda_stream, md_peaks* out);
 
+/* Kinetic energy K = sum_i 1/2 m |v_i|^2 (row a5; the quantity the thermostat F4 needs every step, PAPER.md:45, :94-102,
+ * :111) for callers that cannot allocate device memory: code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc.  Needs no handle and no workspace: the per-block partial sums of the reduction live in a static
+ * __device__ array inside the library (32 KiB on every GPU that loads it, until the process exits), which is why n is
+ * limited to MD_NOALLOC_MAX_PARTICLES.  vel_device: DEVICE memory, fp64 [n][dim] (row-major, as at md_create's boundary);
+ * kinetic_device: DEVICE memory, one double, written by the call; both stay the caller's.  Asynchronous on cuda_stream
+ * (NULL = default stream); the first call on a device resolves the array's address (set-up), later calls only launch two
+ * kernels.  Calls no cudaMalloc / cudaFree / allocating routine.  All calls share the one scratch array: calls that overlap
+ * on the GPU (different streams or host threads) race on it -- serialise them; nothing needs clearing between calls.
+ * errbuf (host, may be NULL) receives the reason on failure.  MD_ERR_INVALID_ARG: NULL pointers, dim not 2/3, mass <= 0,
+ * n < 1; MD_ERR_WORKSPACE: n > MD_NOALLOC_MAX_PARTICLES; MD_ERR_CUDA: no device, or a CUDA error. */
+#define MD_NOALLOC_MAX_PARTICLES 4194304
+int md_kinetic_energy_noalloc(const double* vel_device, long long n, int dim, double mass, double* kinetic_device,
+                              void* cuda_stream, char* errbuf, size_t errbuf_len);
+
 int md_destroy(md_sim*);
 const char* md_last_error(const md_sim*); /* NULL handle: this thread's last md_create error */
 

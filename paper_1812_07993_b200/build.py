@@ -1,9 +1,9 @@
-"""Compiles csrc/md_api.cu into paper_1812_07993_b200/libmd_b200.so for sm_100a (in-tree)."""
+"""Compiles csrc/md_api.cu and csrc/md_noalloc.cu into paper_1812_07993_b200/libmd_b200.so for sm_100a (in-tree)."""
 import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRCS = [os.path.join(HERE, "csrc", "md_api.cu")]
+SRCS = [os.path.join(HERE, "csrc", "md_api.cu"), os.path.join(HERE, "csrc", "md_noalloc.cu")]
 DEPS = SRCS + [os.path.join(HERE, "csrc", h) for h in ("md_kernels.cuh", "md_allpairs.cuh", "md_verlet.cuh")] + [
     os.path.join(HERE, "..", "include", "md.h")]
 LIB = os.path.join(HERE, "libmd_b200.so")

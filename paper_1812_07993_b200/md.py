@@ -21,7 +21,8 @@ MD_FORCE_AUTO, MD_FORCE_ALLPAIRS, MD_FORCE_CELLS, MD_FORCE_VERLET = 0, 1, 2, 3
 _ALGO = {"auto": MD_FORCE_AUTO, "allpairs": MD_FORCE_ALLPAIRS, "cells": MD_FORCE_CELLS, "verlet": MD_FORCE_VERLET}
 
 EXPORTS = ["md_workspace_bytes", "md_create", "md_step", "md_get_state", "md_energy", "md_pressure", "md_density_profile", "md_profile_step",
-           "md_pair_tests", "md_info", "md_measure_peaks", "md_destroy", "md_last_error"]
+           "md_pair_tests", "md_info", "md_measure_peaks", "md_destroy", "md_last_error", "md_kinetic_energy_noalloc"]
+NOALLOC_MAX_PARTICLES = 4194304
 
 
 class md_box(C.Structure):
@@ -112,6 +113,9 @@ def load_library():
         lib.md_destroy.argtypes = [C.c_void_p]
         lib.md_last_error.restype = C.c_char_p
         lib.md_last_error.argtypes = [C.c_void_p]
+        lib.md_kinetic_energy_noalloc.restype = C.c_int
+        lib.md_kinetic_energy_noalloc.argtypes = [C.c_void_p, C.c_longlong, C.c_int, C.c_double, C.c_void_p, C.c_void_p,
+                                                  C.c_char_p, C.c_size_t]
         _lib = lib
     return _lib
 
@@ -267,3 +271,20 @@ def measure_peaks(device="cuda:0", scratch_mib=512):
     if rc != MD_OK:
         raise MDError(rc, "md_measure_peaks failed")
     return dict(fp64_tflops=out.fp64_tflops, fp32_tflops=out.fp32_tflops, copy_gbs=out.copy_gbs)
+
+
+def kinetic_energy_noalloc(vel, mass, out, stream=None, n=None):
+    """md_kinetic_energy_noalloc: K of the fp64 CUDA tensor `vel` [n, dim] into the one-element fp64 CUDA tensor `out`,
+    asynchronously on `stream` (a torch.cuda.Stream; None = the legacy default stream).  Allocates nothing on the device:
+    the reduction's scratch is a static array inside the library (at most NOALLOC_MAX_PARTICLES particles).  `n` overrides
+    the particle count (argument checks)."""
+    import torch
+
+    if not (vel.is_cuda and out.is_cuda and vel.dtype == torch.float64 and out.dtype == torch.float64 and vel.is_contiguous()):
+        raise ValueError("vel and out must be contiguous fp64 CUDA tensors")
+    err = C.create_string_buffer(256)
+    rc = load_library().md_kinetic_energy_noalloc(vel.data_ptr(), int(vel.shape[0] if n is None else n), int(vel.shape[1]),
+                                                  float(mass), out.data_ptr(), stream.cuda_stream if stream is not None else None,
+                                                  err, len(err))
+    if rc != MD_OK:
+        raise MDError(rc, err.value.decode())
