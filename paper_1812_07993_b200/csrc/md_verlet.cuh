@@ -26,12 +26,9 @@ namespace md {
 constexpr int VL_THREADS = 256;
 constexpr int VL_MAXN = 128;   // neighbour-list stride (entries per particle)
 
-// flags: rebuild request, list overflow, position-buffer parity, velocity/id-buffer parity, rebuild count, escape,
+// flags: (slots 0-2 unused: the rebuild request now travels in the grid barrier's word), list overflow, position-buffer parity, velocity/id-buffer parity, rebuild count, escape,
 // particles with a long list at the last rebuild (demand), how many of them the idle blocks' lane groups took (capacity),
 // the same two for the lists long enough for a whole warp
-// The rebuild request rotates over three slots (step % 3): a slot is cleared one barrier before the phase that
-// may set it and read one barrier after, so no block can see a later step's request (which would desynchronise
-// the grid barriers).
 enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_HCAP = 9,
        VF_NHEAVY32 = 10, VF_HCAP32 = 11, VF_COUNT = 12 };
 
@@ -100,26 +97,44 @@ __device__ __forceinline__ float fold(float a, float b, float L, float halfL)
 }
 __device__ __forceinline__ double fold(double a, double b, double, double) { return a - b; }   // never used: fp64 reads ghosts
 
-// Grid barrier of the cooperative launch (all blocks are co-resident).  One arrival atomic per block; the wait
-// polls with relaxed loads and fences ONCE when released -- cooperative_groups' grid.sync() re-acquires (and so
-// invalidates the SM's L1, CCTL.IVALL) on every poll, which also evicts the lines of the other block still
-// computing on that SM (profiles/r01_v3_cfg2.md).  A flag per block polled by every block (no atomic) was measured in
-// round 2 and is 4x slower at 296 blocks: 296 x 296 loads per poll round land on ten L2 lines (profiles/r02_k_md_run.md).
+// Grid barrier of the cooperative launch (all blocks are co-resident), which also carries the step's one global
+// decision.  One arrival per block: a release reduction (MEMBAR.ALL.GPU + REDG; __threadfence() + atomicAdd was a
+// sequentially consistent fence, an L1 invalidation that also evicts the lines of the other block still computing on the
+// SM, and an atomic with a return value), relaxed polling, and ONE acquire load when released (LDG + CCTL.IVALL) --
+// cooperative_groups' grid.sync() re-acquires on every poll (profiles/r01_v3_cfg2.md).  A flag per block polled by every
+// block (no atomic) was measured in round 2 and is 4x slower at 296 blocks (profiles/r02_k_md_run.md).
+// The 64-bit word: arrivals in bits 0..39, and two 12-bit fields that count the blocks asking for a rebuild at even and
+// at odd barriers.  A block reads the field of the barrier's own parity: the other blocks can only have added to it at
+// this barrier (nobody reaches the barrier after the next before everybody has left this one), so every block takes the
+// same decision -- what the three rotating request slots in global memory and a load after every barrier did before.
 // `bar` is zeroed by the host before every launch.
-__device__ __forceinline__ void grid_barrier(unsigned long long* bar, unsigned long long& target)
+struct GridBarrier {
+    unsigned long long target = 0;     // arrivals expected when the current barrier completes (thread 0 only)
+    unsigned int seen_req[2] = {0, 0}; // last value of the two request fields (thread 0 only)
+    unsigned int index = 0;            // barriers passed so far
+};
+
+__device__ __forceinline__ bool grid_barrier(unsigned long long* bar, GridBarrier& g, bool request = false)
 {
-    __syncthreads();
+    __shared__ int s_any;
+    const int par = g.index & 1;
+    ++g.index;
+    const int mine = __syncthreads_or(request);
     if (threadIdx.x == 0) {
-        target += gridDim.x;
-        __threadfence();                                   // release this block's writes
-        atomicAdd(bar, 1ull);
+        g.target += gridDim.x;
+        const unsigned long long add = 1ull + (mine ? 1ull << (40 + 12 * par) : 0ull);
+        asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(bar), "l"(add) : "memory");
         unsigned long long seen;
         do {
             asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(bar) : "memory");
-        } while (seen < target);
-        __threadfence();                                   // acquire: later loads see every block's writes
+        } while ((seen & ((1ull << 40) - 1ull)) < g.target);
+        asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(bar) : "memory");   // later loads see every block's writes
+        const unsigned int field = (unsigned int)(seen >> (40 + 12 * par)) & 0xfffu;
+        s_any = field != g.seen_req[par];
+        g.seen_req[par] = field;
     }
     __syncthreads();
+    return s_any != 0;
 }
 
 __device__ __forceinline__ unsigned long long now_ns()
@@ -333,7 +348,7 @@ struct Carry {
 // drift: start the next step (F2).
 template <typename T>
 __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& v, int c, int cv, bool force,
-                                           bool kick, bool drift, int req, int gtid, int gthreads,
+                                           bool kick, bool drift, bool& want, int gtid, int gthreads,
                                            T lam, double* ksum, Carry<T>& cy, const bool cyon)
 {
     constexpr bool GHOSTS = sizeof(T) == 8;
@@ -363,7 +378,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             if (p.bc[1] == BC_REFLECT) boundary(rn.y, vy, p.L[1], BC_REFLECT, err);
             if (p.bc[2] == BC_REFLECT) boundary(rn.z, vz, p.L[2], BC_REFLECT, err);
             rn.w = ri.w + step_len(sx * sx + sy * sy + sz * sz); // path length >= displacement
-            if (rn.w > v.half_skin) v.flags[VF_REQ0 + req] = 1;
+            if (rn.w > v.half_skin) want = true;
             rnew[i] = rn;
             if (GHOSTS && face) write_ghosts(p, v, rnew, i, rn, face);
         }
@@ -527,11 +542,11 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
 
 template <typename T>
 __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& v, int c, int cv, bool force,
-                                           bool kick, bool drift, int req, int gtid, int gthreads,
+                                           bool kick, bool drift, bool& want, int gtid, int gthreads,
                                            T lam = T(1), double* ksum = nullptr)
 {
     Carry<T> none;
-    phase_step<T>(p, v, c, cv, force, kick, drift, req, gtid, gthreads, lam, ksum, none, false);
+    phase_step<T>(p, v, c, cv, force, kick, drift, want, gtid, gthreads, lam, ksum, none, false);
 }
 
 // ---- rebuild phases (a2 inside the persistent kernel) -------------------------------------------
@@ -792,7 +807,7 @@ template <typename T, int ROWS, int MINB>
 __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
 {
     __shared__ unsigned long long s_times[8];
-    unsigned long long bar_seq = 0;
+    GridBarrier bar_seq;
     const bool thermo = p.thermo_rate > 0.0;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
     const int gthreads = gridDim.x * blockDim.x;
@@ -830,21 +845,21 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
             carry.valid = carry.hvalid = carry.nhvalid = false;          // new particle order, new lists
         }
         if (s == n_steps) break;
-        const int req = (int)(s % 3);
-        if (gtid == 0) { v.flags[VF_REQ0 + (req + 1) % 3] = 0; if (thermo) v.ksum[(s + 1) % 3] = 0.0; }   // slots of step s + 1
+        bool want = false;                                   // this thread asks for a rebuild before the next step
+        if (gtid == 0 && thermo) v.ksum[(s + 1) % 3] = 0.0;                                  // slot of step s + 1
 #ifdef MD_DIAGNOSTICS
         unsigned long long dbg0 = 0;
         if (v.dbg) dbg0 = now_ns();
 #endif
         if (!thermo || s == 0) {
-            phase_step<T>(p, v, c, cv, s > 0, s > 0, true, req, gtid, gthreads, T(1), nullptr, carry, cyon);
+            phase_step<T>(p, v, c, cv, s > 0, s > 0, true, want, gtid, gthreads, T(1), nullptr, carry, cyon);
         } else {
             // with the thermostat lambda(t) needs K(t) of ALL particles before the next drift: the fused phase splits
             // into [F1 + F3 + K partial sums] | barrier | [F4 rescale + F2], one extra barrier per step
-            phase_step<T>(p, v, c, cv, true, true, false, req, gtid, gthreads, T(1), v.ksum + s % 3);
+            phase_step<T>(p, v, c, cv, true, true, false, want, gtid, gthreads, T(1), v.ksum + s % 3);
             grid_barrier(v.bar, bar_seq);
             const double lam = berendsen_lambda(*(volatile double*)(v.ksum + s % 3), p.thermo_rate, p.t_target, p.dof);
-            phase_step<T>(p, v, c, cv, false, false, true, req, gtid, gthreads, (T)lam);
+            phase_step<T>(p, v, c, cv, false, false, true, want, gtid, gthreads, (T)lam);
         }
 #ifdef MD_DIAGNOSTICS
         if (v.dbg && (threadIdx.x & 31) == 0) {
@@ -855,19 +870,20 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
         }
 #endif
         if (gtid == 0) { t1 = now_ns(); s_times[0] += t1 - t0; t0 = t1; }
-        grid_barrier(v.bar, bar_seq);
+        rebuild = grid_barrier(v.bar, bar_seq, want);       // some particle's path since the last rebuild exceeds skin / 2
         if (gtid == 0) { t1 = now_ns(); s_times[1] += t1 - t0; t0 = t1; }
         c ^= 1;
-        rebuild = *(volatile int*)(v.flags + VF_REQ0 + req) != 0;
     }
     if (thermo && n_steps > 0) {
         double* ks = v.ksum + n_steps % 3;
-        phase_step<T>(p, v, c, cv, true, true, false, 0, gtid, gthreads, T(1), ks);
+        bool unused = false;
+        phase_step<T>(p, v, c, cv, true, true, false, unused, gtid, gthreads, T(1), ks);
         grid_barrier(v.bar, bar_seq);
         const double lam = berendsen_lambda(*(volatile double*)ks, p.thermo_rate, p.t_target, p.dof);
-        phase_step<T>(p, v, c, cv, false, false, false, 0, gtid, gthreads, (T)lam);      // F4 of the last step
+        phase_step<T>(p, v, c, cv, false, false, false, unused, gtid, gthreads, (T)lam);      // F4 of the last step
     } else if (n_steps > 0 || force_rebuild) {
-        phase_step<T>(p, v, c, cv, true, n_steps > 0, false, 0, gtid, gthreads);
+        bool unused = false;
+        phase_step<T>(p, v, c, cv, true, n_steps > 0, false, unused, gtid, gthreads);
     }
     if (gtid == 0) {
         v.flags[VF_CUR] = c; v.flags[VF_CURV] = cv;
@@ -889,7 +905,8 @@ __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_build(Params<T> p, Verlet
 template <typename T>
 __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_force(Params<T> p, Verlet<T> v, int c, int cv)
 {
-    phase_step<T>(p, v, c, cv, true, false, false, 0, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+    bool unused = false;
+    phase_step<T>(p, v, c, cv, true, false, false, unused, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 #endif
 
