@@ -78,9 +78,14 @@ typedef struct { double eps, sigma, eps_w, sigma_w, r_cut; int shift_energy; } m
  * 0 <= skin < r_cut is the VERLET list margin in length units; 0 selects the default 0.24 r_cut.
  * heavy_list >= 0: VERLET lists of this many entries or more are walked by a group of four lanes instead of the
  * particle's own thread (0 selects the default 13; a tuning knob, results do not depend on it).
+ * list_prunes: VERLET two-level list: between two full rebuilds (bin, scan, scatter, cell walk) the r_cut + skin list is
+ * pruned that many times from an outer list of all pairs within r_cut + outer skin, outer skin = 1.07 (list_prunes + 1)
+ * skin; 0 selects the default 2, < 0 none (single-level list), at most 8; reduced automatically while the box does not hold
+ * 3 cells of side r_cut + outer skin per periodic dimension.  Exact either way: a prune that finds a particle whose path
+ * since the full rebuild exceeds (outer skin - skin) / 2 is discarded and a full rebuild runs instead.
  * tau_b > 0 switches on the Berendsen thermostat (the paper's kernel F4) after every step:
  * v <- lambda v, lambda = sqrt(1 + (dt / tau_b)(t_target / T - 1)), T = 2K / (dim n_vapor) (k_B = 1); tau_b <= 0: NVE. */
-typedef struct { double dt, mass; int precision, force_algo; double skin; double tau_b, t_target; int heavy_list; } md_opts;
+typedef struct { double dt, mass; int precision, force_algo; double skin; double tau_b, t_target; int heavy_list, list_prunes; } md_opts;
 
 /* potential = potential_vv + potential_vw = sum_i pe_i; virial = sum over unordered vv pairs and
  * vw pairs of g.d (g = force on the vapor particle, d = r_i - r_j); pairs_* = pairs with r < r_cut. */
@@ -97,8 +102,10 @@ typedef struct { double pressure_box, volume_box, pressure_pore, volume_pore, ki
  * launch counts.  Index: 0 kick+drift(+bin count), 1 scan, 2 scatter, 3 force(+half-kick).  VERLET: the
  * whole batch is one launch, reported in slot 3 (slots 0-2: step phases, grid barriers, rebuilds as timed inside the
  * kernel by its first thread); rebuilds = cell-list + neighbour-list rebuilds in it, rebuild_ms = their split into
- * bin, scan, scatter and list build, each with the grid barrier that ends it (VERLET only, else 0). */
-typedef struct { double ms[4]; long long launches[4]; double total_ms; long long steps, rebuilds; double rebuild_ms[4]; } md_kernel_times;
+ * bin, scan, scatter and list build, each with the grid barrier that ends it; prunes = list prunes in it (two-level list),
+ * prune_ms their time, also counted in ms[2] (VERLET only, else 0). */
+typedef struct { double ms[4]; long long launches[4]; double total_ms; long long steps, rebuilds; double rebuild_ms[4];
+                 long long prunes; double prune_ms; } md_kernel_times;
 
 /* Peak micro-benchmarks run on the caller's stream (TFLOP/s count FMA = 2 flops; GB/s = read+write). */
 typedef struct { double fp64_tflops, fp32_tflops, copy_gbs; } md_peaks;

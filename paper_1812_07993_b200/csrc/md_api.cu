@@ -74,6 +74,7 @@ const char* validate(const md_box* box, const md_lj* lj, const md_opts* o, long 
     if (!(o->skin >= 0) || !std::isfinite(o->skin)) return "skin must be >= 0";
     if (o->skin >= lj->r_cut) return "skin must be < r_cut";
     if (o->heavy_list < 0) return "heavy_list must be >= 0";
+    if (o->list_prunes > 8) return "list_prunes must be <= 8";
     if (!std::isfinite(o->tau_b) || !std::isfinite(o->t_target)) return "tau_b, t_target must be finite";
     if (o->tau_b > 0 && (o->tau_b < o->dt || !(o->t_target > 0))) return "thermostat needs tau_b >= dt and t_target > 0";
     if (!(lj->r_cut > 0) || !std::isfinite(lj->r_cut)) return "r_cut must be > 0";
@@ -90,10 +91,30 @@ const char* validate(const md_box* box, const md_lj* lj, const md_opts* o, long 
 
 double list_skin(const md_lj& lj, const md_opts& o) { return o.skin > 0 ? o.skin : 0.24 * lj.r_cut; }
 
-// Grid the handle uses: cells of side >= r_cut (CELLS) or >= r_cut + skin (VERLET).
+// Two-level list: k prunes between two full rebuilds need an outer skin of (k + 1) skins -- each list event is raised when
+// a path exceeds skin / 2 -- plus a margin for the step that crosses the threshold (a prune that finds a longer path is
+// discarded, so the margin is a matter of speed, not of correctness).
+double outer_skin(double skin, int k) { return k > 0 ? (k + 1) * skin * 1.07 : skin; }
+
+// Prunes per full rebuild: md_opts.list_prunes (0: two; < 0: none), reduced until the box holds >= 3 cells of side
+// r_cut + outer skin in every periodic dimension.
+int resolve_prunes(const md_box& box, const md_lj& lj, const md_opts& o)
+{
+    int k = o.list_prunes > 0 ? std::min(o.list_prunes, 8) : (o.list_prunes == 0 ? 2 : 0);
+    const double skin = list_skin(lj, o);
+    for (; k > 0; --k) {
+        bool ok = make_grid(box, lj.r_cut + outer_skin(skin, k)).cells_ok;
+        for (int a = 0; a < box.dim; ++a)
+            if (box.bc[a] == MD_BC_PERIODIC && box.len[a] <= 2.0 * (lj.r_cut + outer_skin(skin, k))) ok = false;
+        if (ok) break;
+    }
+    return k;
+}
+
+// Grid the handle uses: cells of side >= r_cut (CELLS) or >= r_cut + (outer) skin (VERLET).
 GridSpec grid_for(const md_box& box, const md_lj& lj, const md_opts& o, int algo)
 {
-    return make_grid(box, algo == MD_FORCE_VERLET ? lj.r_cut + list_skin(lj, o) : lj.r_cut);
+    return make_grid(box, algo == MD_FORCE_VERLET ? lj.r_cut + outer_skin(list_skin(lj, o), resolve_prunes(box, lj, o)) : lj.r_cut);
 }
 
 bool verlet_ok(const md_box& box, const md_lj& lj, const md_opts& o, long long nv, long long nw)
@@ -130,6 +151,8 @@ struct Layout {
     unsigned long long* tests;
     double *stage0, *stage1, *wstage;
     int *nbr, *ncnt, *vflags;   // VERLET: neighbour list, counts, flags
+    int *onbr, *ocnt, *oheavy;  // VERLET, two-level list: outer list, its counts, particles pruned by a warp
+    T* wo;                      // path between the last full rebuild and the last list event
     unsigned long long* vtimes;
     unsigned long long* vbar;   // VERLET: grid-barrier arrival counter
     md::F4* r32;                // VERLET fp64: fp32 shadow of the positions for the list build
@@ -154,7 +177,7 @@ int image_blocks(const md_box& box, int precision)
 }
 
 template <typename T>
-Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell, int algo, int nimg)
+Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell, int algo, int nimg, int nprune)
 {
     Layout<T> l;
     Carver c(base);
@@ -189,6 +212,11 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.tests = c.take<unsigned long long>(2);
     l.nbr = c.take<int>(verlet ? n * md::VL_MAXN : 1);
     l.ncnt = c.take<int>(verlet ? n : 1);
+    const bool two = verlet && nprune > 0;
+    l.onbr = c.take<int>(two ? n * md::VL_MAXO : 1);
+    l.ocnt = c.take<int>(two ? n : 1);
+    l.oheavy = c.take<int>(two ? n : 1);
+    l.wo = c.take<T>(two ? n : 1);
     l.vflags = c.take<int>(md::VF_COUNT);
     l.r32 = c.take<md::F4>(verlet && sizeof(T) == 8 ? n + m : 1);
     l.tile_agg = c.take<unsigned long long>(verlet ? (size_t)cdiv((long long)nc, md::SCAN_TILE) + 1 : 1);
@@ -198,7 +226,7 @@ Layout<T> carve(void* base, int dim, long long nv, long long nw, long long ncell
     l.jv_id = c.take<int>(dot && sizeof(T) == 4 ? 8 * n : 1);
     l.jw_id = c.take<int>(dot && sizeof(T) == 4 ? 8 * m : 1);
     l.ghost_count = c.take<int>(4);
-    l.vtimes = c.take<unsigned long long>(8 + 8192);
+    l.vtimes = c.take<unsigned long long>(16 + 8192);
     l.vbar = c.take<unsigned long long>(2);
     l.vksum = c.take<double>(4);
     l.hist = c.take<unsigned long long>(md::HIST_MAX_BINS);
@@ -254,8 +282,8 @@ struct Sim : md_sim {
     md::Verlet<T> vl;
     int curv = 0, coop_grid = 0, coop_base = 0, coop_max = 0, heavy_seen = 0, heavy32_seen = 0;
     int minb3_threshold = -1;   // particles beyond which the 3-blocks-per-SM build runs; set at the first launch
-    long long rebuilds_seen = 0;
-    unsigned long long phase_ns[8] = {};
+    long long rebuilds_seen = 0, prunes_seen = 0;
+    unsigned long long phase_ns[10] = {};
 
     md::AllPairsDot ad;
     md::AllPairsDotF adf;
@@ -333,7 +361,8 @@ struct Sim : md_sim {
         CK(cudaMemcpyAsync(h, l.vflags, sizeof(h), cudaMemcpyDeviceToHost, stream));
         CK(cudaStreamSynchronize(stream));
         CK(cudaGetLastError());
-        cur = h[md::VF_CUR]; curv = h[md::VF_CURV]; rebuilds_seen = h[md::VF_NREBUILD]; heavy_seen = h[md::VF_NHEAVY]; heavy32_seen = h[md::VF_NHEAVY32];
+        cur = h[md::VF_CUR]; curv = h[md::VF_CURV]; rebuilds_seen = h[md::VF_NREBUILD]; prunes_seen = h[md::VF_NPRUNE];
+        heavy_seen = h[md::VF_NHEAVY + h[md::VF_HPAR]]; heavy32_seen = h[md::VF_NHEAVY32 + h[md::VF_HPAR]];
         if (h[md::VF_ESCAPE]) { err = "a particle left a reflecting box (more than one bounce in a step)"; return MD_ERR_STATE; }
         if (h[md::VF_OVERFLOW]) { err = "neighbour list overflow (> 128 neighbours within r_cut + skin)"; return MD_ERR_WORKSPACE; }
         return MD_OK;
@@ -488,8 +517,8 @@ struct Sim : md_sim {
         if (verlet()) {
             int rc = refresh();
             if (rc) return rc;
-            const long long r0 = rebuilds_seen;
-            unsigned long long t[8], tb[8];                 // the kernel's own timers are cumulative: take the difference
+            const long long r0 = rebuilds_seen, p0 = prunes_seen;
+            unsigned long long t[10], tb[10];                 // the kernel's own timers are cumulative: take the difference
             CK(cudaMemcpy(tb, l.vtimes, sizeof(tb), cudaMemcpyDeviceToHost));
             CK(cudaEventRecord(ev[0], stream));
             if (n > 0 && (rc = launch_run(n, 0))) return rc;
@@ -501,7 +530,7 @@ struct Sim : md_sim {
 #ifdef MD_DIAGNOSTICS
             if (getenv("MD_DEBUG_TIMES")) {
                 std::vector<unsigned long long> w(8192);
-                CK(cudaMemcpy(w.data(), l.vtimes + 8, 8192 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+                CK(cudaMemcpy(w.data(), l.vtimes + 16, 8192 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
                 const int nwarp = coop_grid * md::VL_THREADS / 32;
                 const int nbl = std::min(coop_grid, cdiv(p.nv, md::VL_THREADS)), wpb = md::VL_THREADS / 32;
                 double mx[2] = {0, 0}, sm[2] = {0, 0};
@@ -514,19 +543,26 @@ struct Sim : md_sim {
                 fprintf(stderr, "[md] step-phase us per step and warp (cumulative / steps): particle blocks (%d) max %.2f mean %.2f | idle blocks (%d) max %.2f mean %.2f\n",
                         nbl, mx[0] * per, sm[0] * per / std::max(cnt[0], 1), coop_grid - nbl, mx[1] * per, sm[1] * per / std::max(cnt[1], 1));
                 {
-                    double mxp = 0, mxi = 0;
-                    for (int k = 0; k < nwarp && k < 4000; ++k) (k / wpb >= nbl ? mxi : mxp) = std::max(k / wpb >= nbl ? mxi : mxp, (double)w[4096 + k]);
-                    fprintf(stderr, "[md] longest single step phase of any warp: particle blocks %.1f us, idle blocks %.1f us; histogram of warp-phase times (1.024 us bins):", mxp * 1e-3, mxi * 1e-3);
+                    double l = 0, h = 0, ml = 0, mh = 0;
+                    for (int k = 0; k < 1024; ++k) {
+                        l += (double)w[4096 + 2 * k]; h += (double)w[4097 + 2 * k];
+                        ml = std::max(ml, (double)w[4096 + 2 * k]); mh = std::max(mh, (double)w[4097 + 2 * k]);
+                    }
+                    const double np = std::max<double>((double)prunes_seen, 1.0);
+                    fprintf(stderr, "[md] prune, us per prune and warp (first 1024 warps): thread-per-particle part mean %.2f max %.2f, "
+                            "warp-per-particle part mean %.2f max %.2f; particles pruned by warps: %.0f per prune; histogram of step-phase times (1.024 us bins):",
+                            l / 1024 / np * 1e-3, ml / np * 1e-3, h / 1024 / np * 1e-3, mh / np * 1e-3, (double)w[7000] / np);
                     for (int k = 0; k < 16; ++k) fprintf(stderr, " %llu", w[8000 + k]);
                     fprintf(stderr, "\n");
                 }
                 int hh[md::VF_COUNT];
                 CK(cudaMemcpy(hh, l.vflags, sizeof(hh), cudaMemcpyDeviceToHost));
                 fprintf(stderr, "[md] after the last rebuild: lists > %d entries %d (lane groups hold %d), lists > %d entries %d (warps hold %d)\n",
-                        vl.heavy_t, hh[md::VF_NHEAVY], hh[md::VF_HCAP], md::VL_WARP_T, hh[md::VF_NHEAVY32], hh[md::VF_HCAP32]);
+                        vl.heavy_t, hh[md::VF_NHEAVY + hh[md::VF_HPAR]], hh[md::VF_HCAP], md::VL_WARP_T, hh[md::VF_NHEAVY32 + hh[md::VF_HPAR]], hh[md::VF_HCAP32]);
             }
 #endif
-            for (int q = 0; q < 8; ++q) phase_ns[q] = t[q] - tb[q];
+            for (int q = 0; q < 10; ++q) phase_ns[q] = t[q] - tb[q];
+            out->prunes = prunes_seen - p0; out->prune_ms = phase_ns[8] * 1e-6;
             for (int q = 0; q < 4; ++q) out->rebuild_ms[q] = phase_ns[4 + q] * 1e-6;   // bin, scan, scatter, list build
             // VERLET: ms[0] step phases, ms[1] grid barriers, ms[2] rebuilds (as seen by thread 0), ms[3] whole launch
             out->ms[0] = phase_ns[0] * 1e-6; out->ms[1] = phase_ns[1] * 1e-6; out->ms[2] = phase_ns[2] * 1e-6;
@@ -541,6 +577,8 @@ struct Sim : md_sim {
                     else md::k_dbg_build<T, 3><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur);
                 }
                 for (int k = 0; k < 3; ++k) md::k_dbg_force<T><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur, curv);
+                if (vl.nprune > 0)      // leaves the handle unusable for further steps (heavy registries not refilled): last call only
+                    for (int k = 0; k < 3; ++k) md::k_dbg_prune<T><<<coop_grid, md::VL_THREADS, 0, stream>>>(p, vl, cur);
                 CK(cudaStreamSynchronize(stream));
             }
 #endif
@@ -804,7 +842,7 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
     if (verlet()) {
         // walls (cell order) appended to both position buffers; then bin + list + f(0) in one persistent launch
         CK(cudaMemsetAsync(l.vflags, 0, sizeof(int) * md::VF_COUNT, stream));
-        CK(cudaMemsetAsync(l.vtimes, 0, (8 + 8192) * sizeof(unsigned long long), stream));
+        CK(cudaMemsetAsync(l.vtimes, 0, (16 + 8192) * sizeof(unsigned long long), stream));
         CK(cudaMemsetAsync(l.tile_agg, 0, sizeof(unsigned long long) * (size_t)(cdiv(p.ncell, md::SCAN_TILE) + 1), stream));
         if (nw > 0)
             for (int b = 0; b < 2; ++b)
@@ -876,7 +914,8 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
     s->box = box;
     s->algo = algo;
     s->stream = (cudaStream_t)stream;
-    s->l = carve<T>(ws, box.dim, nv, nw, g.ncell, algo, image_blocks(box, o.precision));
+    const int nprune = algo == MD_FORCE_VERLET ? resolve_prunes(box, lj, o) : 0;
+    s->l = carve<T>(ws, box.dim, nv, nw, g.ncell, algo, image_blocks(box, o.precision), nprune);
     if (s->l.bytes > ws_bytes) {
         g_create_error = "workspace too small";
         delete s;
@@ -949,11 +988,15 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
         const double skin = list_skin(lj, o), rl = lj.r_cut + skin;
         md::Verlet<T>& v = s->vl;
         v.st[0] = s->l.st[0]; v.st[1] = s->l.st[1]; v.f = s->l.f;
-        v.nbr = s->l.nbr; v.ncnt = s->l.ncnt; v.stride = align_up((size_t)nv, 64);
+        v.nbr = s->l.nbr; v.ncnt = s->l.ncnt;      // lists: warp-blocked, n = align_up(nv, 64) particles allocated
         v.cell = s->l.cell; v.slot = s->l.slot; v.count = s->l.count; v.start = s->l.start; v.tile_agg = s->l.tile_agg;
         v.wstart = s->l.wstart; v.wnear = s->l.wnear; v.flags = s->l.vflags; v.bar = s->l.vbar; v.ksum = s->l.vksum; v.times = s->l.vtimes;
         v.dbg = nullptr;
         v.r32 = s->l.r32;
+        v.onbr = s->l.onbr; v.ocnt = s->l.ocnt; v.oheavy = s->l.oheavy; v.wo = s->l.wo;
+        v.nprune = nprune;
+        const double so = outer_skin(skin, nprune), rlo = lj.r_cut + so;
+        v.outer_lim = (T)(0.5 * (so - skin));
         v.ntot = (int)(nv + nw); v.nimg = image_blocks(box, o.precision);
         v.half_skin = (T)(0.5 * skin);
         // fp32 filter of the list build: (r_c + skin) plus the rounding of the fp32 positions (ulp(L) / 2 each), of the
@@ -962,10 +1005,15 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
         for (int a = 0; a < box.dim; ++a) lmax = std::max(lmax, box.len[a]);
         const double rlf = rl * (1.0 + 4e-7) + 4.0 * lmax * 1.1920929e-7;
         v.rl2f = (float)(rlf * rlf * (1.0 + 2e-7));
+        const double rlof = rlo * (1.0 + 4e-7) + 4.0 * lmax * 1.1920929e-7;
+        v.rl2f_out = (float)(rlof * rlof * (1.0 + 2e-7));
+        // the prune tests the positions themselves: exact threshold in fp64 (plus 1e-9: the path lengths are rounded up
+        // by 1e-6, see step_len), the build's inflated one in fp32
+        v.rl2_prune = sizeof(T) == 8 ? (T)(rl * rl * (1.0 + 1e-9)) : (T)v.rl2f;
         v.heavy_t = o.heavy_list > 0 ? o.heavy_list - 1 : 12;   // lists of heavy_list entries or more (default 13)
         v.carry = 1;
 #ifdef MD_DIAGNOSTICS
-        if (getenv("MD_DEBUG_TIMES")) v.dbg = s->l.vtimes + 8;
+        if (getenv("MD_DEBUG_TIMES")) v.dbg = s->l.vtimes + 16;
         if (getenv("MD_NO_CARRY")) v.carry = 0;
 #endif
     }
@@ -1010,9 +1058,9 @@ size_t md_workspace_bytes(const md_box* box, const md_lj* lj, const md_opts* o, 
     int algo = pick_algo(*box, *lj, *o, nv, nw);
     if (algo < 0) return 0;
     GridSpec g = grid_for(*box, *lj, *o, algo);
-    const int nimg = image_blocks(*box, o->precision);
-    return o->precision == 64 ? carve<double>(nullptr, box->dim, nv, nw, g.ncell, algo, nimg).bytes
-                              : carve<float>(nullptr, box->dim, nv, nw, g.ncell, algo, nimg).bytes;
+    const int nimg = image_blocks(*box, o->precision), nprune = algo == MD_FORCE_VERLET ? resolve_prunes(*box, *lj, *o) : 0;
+    return o->precision == 64 ? carve<double>(nullptr, box->dim, nv, nw, g.ncell, algo, nimg, nprune).bytes
+                              : carve<float>(nullptr, box->dim, nv, nw, g.ncell, algo, nimg, nprune).bytes;
 }
 
 int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj* lj, const md_opts* o, long long nv,

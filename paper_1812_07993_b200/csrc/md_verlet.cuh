@@ -24,13 +24,25 @@
 namespace md {
 
 constexpr int VL_THREADS = 256;
-constexpr int VL_MAXN = 128;   // neighbour-list stride (entries per particle)
+constexpr int VL_MAXN = 128;   // neighbour-list entries per particle
+constexpr int VL_MAXO = 256;   // outer-list entries per particle (two-level list, see phase_prune)
+// List layout: warp-blocked.  The lists of particles 32 b .. 32 b + 31 form one block of MAXK rows of 32 entries: entry k of
+// particle i sits at ((i / 32) MAXK + k) 32 + i % 32.  A warp's loads of entry k are one 128-byte line, as in the fully
+// transposed layout of round 1 (k stride = N_v), but consecutive entries of a particle are a CONSTANT 128 bytes apart, so
+// a list walk is immediate offsets from one base pointer instead of a 64-bit multiply-add per entry: a third of the
+// instructions of the prune and a tenth of the step loop were that address arithmetic (profiles/r02_k_md_run.md).
+constexpr int VL_LS = 32;
+__device__ __forceinline__ size_t vl_base(int i, int maxk) { return ((size_t)(i >> 5) * maxk << 5) + (i & 31); }
 
 // flags: (slots 0-2 unused: the rebuild request now travels in the grid barrier's word), list overflow, position-buffer parity, velocity/id-buffer parity, rebuild count, escape,
 // particles with a long list at the last rebuild (demand), how many of them the idle blocks' lane groups took (capacity),
 // the same two for the lists long enough for a whole warp
-enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_HCAP = 9,
-       VF_NHEAVY32 = 10, VF_HCAP32 = 11, VF_COUNT = 12 };
+// The two heavy-list counters exist twice (+ parity of the list event that filled them: a prune fills the set the step
+// phases are not reading, and the set just retired is cleared one barrier before anybody can write it again); VF_HPAR =
+// the parity in use when the launch ended; VF_OUTER_BAD = the last outer list overflowed (no pruning until the next
+// outer build); VF_NOHEAVY = particles with a long OUTER list (pruned by a warp each); VF_NPRUNE = prunes so far.
+enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_HCAP = 10,
+       VF_NHEAVY32 = 11, VF_HCAP32 = 13, VF_HPAR = 14, VF_OUTER_BAD = 15, VF_NOHEAVY = 16, VF_NPRUNE = 17 /* + 1: prunes since the last full rebuild */, VF_COUNT = 19 };
 
 // Shadow entry of the list build: (x, y, z) rounded to fp32.
 struct alignas(16) F4 {
@@ -46,8 +58,12 @@ struct Verlet {
     // st[cv].{vx,vy,vz,id}: owner-only data, swapped only by the rebuild's scatter
     State<T> st[2];
     Force<T> f;
-    int *nbr, *ncnt;           // nbr[k * stride + i], k < VL_MAXN: index into a position buffer; ncnt[nv]: see VL_* below
-    size_t stride;             // >= nv
+    int *nbr, *ncnt;           // nbr[vl_base(i, VL_MAXN) + k * VL_LS], k < VL_MAXN: index into a position buffer; ncnt[nv]: see VL_* below
+    // two-level list (nprune > 0): onbr[vl_base(i, VL_MAXO) + k * VL_LS], k < VL_MAXO = every j within r_c + outer skin of i at the last
+    // full rebuild; ocnt = its counts (VO_*); oheavy = particles whose outer list a whole warp prunes; wo = path of i
+    // between the last full rebuild and the last list event (owner-only)
+    int *onbr, *ocnt, *oheavy;
+    T* wo;
     int *cell, *slot, *count, *start;
     unsigned long long* tile_agg;   // scan: (rebuild generation, sum of the tile's counts) per tile of SCAN_TILE cells
     const int* wstart;         // walls: [ncell + 1] ranges into the wall part of an image block
@@ -57,10 +73,14 @@ struct Verlet {
     unsigned long long* bar;   // grid barrier arrival counter
     double* ksum;              // [3] kinetic-energy accumulators of the thermostat, rotating like the requests
     unsigned long long* dbg;   // optional per-warp step-phase ns (diagnostics build), or nullptr
-    unsigned long long* times; // [8] ns seen by thread 0: step phases, step barriers, rebuilds, final phase,
-                               // rebuild split: bin, scan, scatter, list build (each with its barrier)
+    unsigned long long* times; // [10] ns seen by thread 0: step phases, step barriers, list events, final phase,
+                               // full-rebuild split: bin, scan, scatter, list build (each with its barrier); [8] prunes
     T half_skin;               // skin / 2
     float rl2f;                // (r_c + skin)^2 plus the fp32 rounding of the filter (positions, image shift, fma chain)
+    float rl2f_out;            // the same for r_c + outer skin
+    T rl2_prune;               // (r_c + skin)^2 for the prune's test on the positions themselves
+    T outer_lim;               // (outer skin - skin) / 2: a prune is valid while no path since the full rebuild exceeds it
+    int nprune;                // prunes allowed between two full rebuilds (0: single-level list)
     int ntot, nimg;            // image-block stride nv + nw; number of image blocks (1 in fp32 mode: that mode folds)
     int carry;                 // 0: reload own state every step (diagnostic A/B)
     int heavy_t;               // particles whose list is longer than this are "heavy": in the step phase a group of
@@ -75,6 +95,12 @@ struct Verlet {
 // the copy at +L), 2 = in the LAST cell (ghost at -L); heavy = list walked by a lane group (see phase_step).
 constexpr int VL_NVV_MASK = 0xff, VL_NVW_SHIFT = 8, VL_NVW_MASK = 0xff, VL_FACE_SHIFT = 16, VL_FACE_MASK = 0x3f;
 constexpr int VL_HEAVY = 1 << 29;
+// ocnt word: vapor entries in outer slots [0, ov), wall entries in the last ow slots, the face code, "pruned by a warp"
+constexpr int VO_MASK = 0x3ff, VO_W_SHIFT = 10, VO_FACE_SHIFT = 20, VO_HEAVY = 1 << 30;
+#ifndef MD_VO_HEAVY_T
+#define MD_VO_HEAVY_T 40
+#endif
+constexpr int VO_HEAVY_T = MD_VO_HEAVY_T;          // outer lists longer than this (mean 17 at density 0.05) are pruned by a whole warp
 __device__ __forceinline__ int vl_nvv(int raw) { return raw & VL_NVV_MASK; }
 __device__ __forceinline__ int vl_nvw(int raw) { return (raw >> VL_NVW_SHIFT) & VL_NVW_MASK; }
 __device__ __forceinline__ int vl_face(int raw) { return (raw >> VL_FACE_SHIFT) & VL_FACE_MASK; }
@@ -207,7 +233,7 @@ __device__ __forceinline__ void pair_term_nb(const PairCoef<T>& q, bool valid, T
 #endif
 constexpr int VL_BATCH = MD_VL_BATCH;
 template <typename T, bool ENERGY, bool FOLD>
-__device__ __forceinline__ void list_loop(const Params<T>& p, const PairCoef<T>& q, const int* __restrict__ lst, size_t stride,
+__device__ __forceinline__ void list_loop(const Params<T>& p, const PairCoef<T>& q, const int* __restrict__ lst,
                                           int n, const Vec4<T>* __restrict__ r, const Vec4<T>& ri, const int (&j0)[VL_BATCH],
                                           Acc<T, ENERGY>& a)
 {
@@ -222,7 +248,7 @@ __device__ __forceinline__ void list_loop(const Params<T>& p, const PairCoef<T>&
         for (int u = 0; u < VL_BATCH; ++u) { j[u] = jn[u]; rj[u] = r[max(j[u], 0)]; }
 #pragma unroll
         for (int u = 0; u < VL_BATCH; ++u)
-            jn[u] = k + VL_BATCH + u < n ? lst[(size_t)(k + VL_BATCH + u) * stride] : -1;   // next batch
+            jn[u] = k + VL_BATCH + u < n ? lst[(k + VL_BATCH + u) * VL_LS] : -1;   // next batch
 #pragma unroll
         for (int u = 0; u < VL_BATCH; ++u) {
             const T dx = px ? fold(ri.x, rj[u].x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj[u].x;
@@ -242,20 +268,20 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
                                            const Vec4<T>& ri, int raw, const int (&j0)[VL_BATCH],
                                            Acc<T, ENERGY>& av, Acc<T, ENERGY>& aw)
 {
-    const int* __restrict__ lst = v.nbr + i;
+    const int* __restrict__ lst = v.nbr + vl_base(i, VL_MAXN);
     const int nvv = vl_nvv(raw), nvw = vl_nvw(raw);
     const bool fold = sizeof(T) == 4 && __any_sync(__activemask(), vl_face(raw) != 0);
     const PairCoef<T> qv = coef_vv(p);
-    if (fold) list_loop<T, ENERGY, true>(p, qv, lst, v.stride, nvv, r, ri, j0, av);
-    else list_loop<T, ENERGY, false>(p, qv, lst, v.stride, nvv, r, ri, j0, av);
+    if (fold) list_loop<T, ENERGY, true>(p, qv, lst, nvv, r, ri, j0, av);
+    else list_loop<T, ENERGY, false>(p, qv, lst, nvv, r, ri, j0, av);
     if (__any_sync(__activemask(), nvw != 0)) {             // walls: a few per cent of the particles have any
         const PairCoef<T> qw = coef_vw(p);
-        const int* __restrict__ lw = lst + (size_t)(VL_MAXN - nvw) * v.stride;
+        const int* __restrict__ lw = lst + (VL_MAXN - nvw) * VL_LS;
         int w0[VL_BATCH];
 #pragma unroll
-        for (int u = 0; u < VL_BATCH; ++u) w0[u] = u < nvw ? lw[(size_t)u * v.stride] : -1;
-        if (fold) list_loop<T, ENERGY, true>(p, qw, lw, v.stride, nvw, r, ri, w0, aw);
-        else list_loop<T, ENERGY, false>(p, qw, lw, v.stride, nvw, r, ri, w0, aw);
+        for (int u = 0; u < VL_BATCH; ++u) w0[u] = u < nvw ? lw[u * VL_LS] : -1;
+        if (fold) list_loop<T, ENERGY, true>(p, qw, lw, nvw, r, ri, w0, aw);
+        else list_loop<T, ENERGY, false>(p, qw, lw, nvw, r, ri, w0, aw);
     }
 }
 
@@ -265,7 +291,7 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
 {
     int j0[VL_BATCH];
 #pragma unroll
-    for (int u = 0; u < VL_BATCH; ++u) j0[u] = v.nbr[(size_t)u * v.stride + i];   // in flight together with ncnt (and r_i, v_i)
+    for (int u = 0; u < VL_BATCH; ++u) j0[u] = v.nbr[vl_base(i, VL_MAXN) + u * VL_LS];   // in flight together with ncnt (and r_i, v_i)
     list_force<T, ENERGY>(p, v, r, i, ri, v.ncnt[i], j0, av, aw);
 }
 
@@ -274,7 +300,7 @@ __device__ __forceinline__ void list_force(const Params<T>& p, const Verlet<T>& 
 // forces.  Vapor and wall entries are told apart by their slot (k < nvv), so this loop selects the coefficients per
 // entry -- the price of sharing one list, paid only by the few heavy particles.
 template <typename T, bool FOLD>
-__device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* __restrict__ lst, size_t stride, int nvv, int n,
+__device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* __restrict__ lst, int nvv, int n,
                                                 int sub, const Vec4<T>* __restrict__ r, const Vec4<T>& ri,
                                                 const int (&j0)[4], Acc<T, false>& a)
 {
@@ -291,7 +317,7 @@ __device__ __forceinline__ void list_loop_group(const Params<T>& p, const int* _
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const int kk = k + 4 * VL_GROUP + sub + VL_GROUP * u;
-            jn[u] = kk < n ? lst[(size_t)(kk < nvv ? kk : kk + VL_MAXN - n) * stride] : -1;   // wall entries sit at the top
+            jn[u] = kk < n ? lst[(kk < nvv ? kk : kk + VL_MAXN - n) * VL_LS] : -1;   // wall entries sit at the top
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -348,7 +374,7 @@ struct Carry {
 // drift: start the next step (F2).
 template <typename T>
 __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& v, int c, int cv, bool force,
-                                           bool kick, bool drift, bool& want, int gtid, int gthreads,
+                                           bool kick, bool drift, bool& want, int gtid, int gthreads, int hp,
                                            T lam, double* ksum, Carry<T>& cy, const bool cyon)
 {
     constexpr bool GHOSTS = sizeof(T) == 8;
@@ -397,7 +423,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             ri = rcur[i];
             vx = s.vx[i]; vy = s.vy[i]; vz = s.vz[i];    // issued early, consumed after the force loop
 #pragma unroll
-            for (int u = 0; u < VL_BATCH; ++u) j0[u] = force ? v.nbr[(size_t)u * v.stride + i] : 0;   // in flight together
+            for (int u = 0; u < VL_BATCH; ++u) j0[u] = force ? v.nbr[vl_base(i, VL_MAXN) + u * VL_LS] : 0;   // in flight together
             raw = v.ncnt[i];                             // the face code is needed by the drift even without a force pass
         }
         vx = lam * vx; vy = lam * vy; vz = lam * vz;     // F4 of the step just completed (lam = 1 without thermostat)
@@ -432,7 +458,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         int nh;
         if (cyon && cy.nhvalid) nh = cy.nh;
         else {
-            nh = min(v.flags[VF_NHEAVY], v.flags[VF_HCAP]);
+            nh = min(v.flags[VF_NHEAVY + hp], v.flags[VF_HCAP]);
             if (cyon) { cy.nh = nh; cy.nhvalid = true; }
         }
         const int lane = threadIdx.x & 31, sub = lane & (VL_GROUP - 1);
@@ -444,7 +470,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         // per WARP of the idle blocks, lane l takes entries l, l + 32, l + 64, l + 96 -- one batch, a butterfly sum,
         // and lane 0 integrates.  Walked by four lanes such a list would take 7 batches while the grid waits.
         if (b >= nbl) {
-            const int n32 = min(v.flags[VF_NHEAVY32], v.flags[VF_HCAP32]), nw32 = nsp * (VL_THREADS / 32);
+            const int n32 = min(v.flags[VF_NHEAVY32 + hp], v.flags[VF_HCAP32]), nw32 = nsp * (VL_THREADS / 32);
             const PairCoef<T> qv = coef_vv(p), qw = coef_vw(p);
             const bool fpx = sizeof(T) == 4 && p.bc[0] == BC_PERIODIC, fpy = sizeof(T) == 4 && p.bc[1] == BC_PERIODIC,
                        fpz = sizeof(T) == 4 && p.bc[2] == BC_PERIODIC;
@@ -457,7 +483,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const int k = lane + 32 * u;
-                    j[u] = k < n ? v.nbr[(size_t)(k < nvv ? k : k + VL_MAXN - n) * v.stride + i] : -1;
+                    j[u] = k < n ? v.nbr[vl_base(i, VL_MAXN) + (k < nvv ? k : k + VL_MAXN - n) * VL_LS] : -1;
                 }
                 const Vec4<T> ri = rcur[i];
                 T vx = T(0), vy = T(0), vz = T(0);
@@ -503,7 +529,7 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const int k = sub + VL_GROUP * u, nv0 = vl_nvv(raw), n0 = nv0 + vl_nvw(raw);
-                    j0[u] = v.nbr[(size_t)(k < nv0 || k >= n0 ? k : k + VL_MAXN - n0) * v.stride + i];
+                    j0[u] = v.nbr[vl_base(i, VL_MAXN) + (k < nv0 || k >= n0 ? k : k + VL_MAXN - n0) * VL_LS];
                 }
                 if (sub == 0) { vx = s.vx[i]; vy = s.vy[i]; vz = s.vz[i]; }
             }
@@ -512,8 +538,8 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
             Acc<T, false> a;
             const int nvv = vl_nvv(raw), n = nvv + vl_nvw(raw);
             const bool fold = sizeof(T) == 4 && __any_sync(__activemask(), vl_face(raw) != 0);
-            if (fold) list_loop_group<T, true>(p, v.nbr + i, v.stride, nvv, n, sub, rcur, ri, j0, a);
-            else list_loop_group<T, false>(p, v.nbr + i, v.stride, nvv, n, sub, rcur, ri, j0, a);
+            if (fold) list_loop_group<T, true>(p, v.nbr + vl_base(i, VL_MAXN), nvv, n, sub, rcur, ri, j0, a);
+            else list_loop_group<T, false>(p, v.nbr + vl_base(i, VL_MAXN), nvv, n, sub, rcur, ri, j0, a);
             T fx = a.fx, fy = a.fy, fz = a.fz;
 #pragma unroll
             for (int o = 1; o < VL_GROUP; o <<= 1) {
@@ -542,11 +568,11 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
 
 template <typename T>
 __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& v, int c, int cv, bool force,
-                                           bool kick, bool drift, bool& want, int gtid, int gthreads,
+                                           bool kick, bool drift, bool& want, int gtid, int gthreads, int hp,
                                            T lam = T(1), double* ksum = nullptr)
 {
     Carry<T> none;
-    phase_step<T>(p, v, c, cv, force, kick, drift, want, gtid, gthreads, lam, ksum, none, false);
+    phase_step<T>(p, v, c, cv, force, kick, drift, want, gtid, gthreads, hp, lam, ksum, none, false);
 }
 
 // ---- rebuild phases (a2 inside the persistent kernel) -------------------------------------------
@@ -564,6 +590,7 @@ __device__ __forceinline__ void phase_bin(const Params<T>& p, const Verlet<T>& v
         if (p.bc[2] == BC_PERIODIC) boundary(ri.z, dummy, p.L[2], BC_PERIODIC, err);
         ri.w = T(0);
         r[i] = ri;
+        if (v.nprune > 0) v.wo[i] = T(0);                // paths since THIS full rebuild (any order: every entry is cleared)
         int cx, cy, cz;
         const int ci = cell_index(p, ri.x, ri.y, ri.z, cx, cy, cz);
         v.cell[i] = ci;
@@ -669,10 +696,11 @@ __device__ __forceinline__ int face_code(const Params<T>& p, int cx, int cy, int
     return face;
 }
 
-// End of a particle's list build: the ncnt word, the heavy registries, overflow, its ghost copies.
+// End of a particle's list build: the ncnt word, the heavy registries (counter set hp), overflow, its ghost copies.
 template <typename T>
 __device__ __forceinline__ void finish_list(const Params<T>& p, const Verlet<T>& v, Vec4<T>* __restrict__ r, int i,
-                                            const Vec4<T>& ri, int nvv, int nvw, int face, int hcap, int hcap32)
+                                            const Vec4<T>& ri, int nvv, int nvw, int face, int hcap, int hcap32, int hp,
+                                            bool ghosts = true)
 {
     const int n = nvv + nvw;
     int raw = min(nvv, VL_MAXN) | (min(nvw, VL_MAXN) << VL_NVW_SHIFT) | (face << VL_FACE_SHIFT);
@@ -684,17 +712,55 @@ __device__ __forceinline__ void finish_list(const Params<T>& p, const Verlet<T>&
     else if (n > v.heavy_t || ((nvv + VL_BATCH - 1) / VL_BATCH + (nvw + VL_BATCH - 1) / VL_BATCH) * VL_BATCH > v.heavy_t + VL_BATCH - 1) {
         bool placed = false;
         if (n > VL_WARP_T && hcap32 > 0) {
-            const int h = atomicAdd(v.flags + VF_NHEAVY32, 1);
+            const int h = atomicAdd(v.flags + VF_NHEAVY32 + hp, 1);
             placed = h < hcap32;
             if (placed) { raw |= VL_HEAVY; v.cell[p.nv - 1 - h] = i; v.slot[p.nv - 1 - h] = raw; }
         }
         if (!placed) {                                   // no warp left: four lanes are still better than one
-            const int h = atomicAdd(v.flags + VF_NHEAVY, 1);
+            const int h = atomicAdd(v.flags + VF_NHEAVY + hp, 1);
             if (h < hcap) { raw |= VL_HEAVY; v.cell[h] = i; v.slot[h] = raw; }
         }
     }
     v.ncnt[i] = raw;
-    if (sizeof(T) == 8 && face) write_ghosts(p, v, r, i, ri, face);
+    if (sizeof(T) == 8 && face && ghosts) write_ghosts(p, v, r, i, ri, face);
+}
+
+// finish_list for a CONVERGED warp (every lane calls it, `live` lanes have a particle): one atomic per warp and registry
+// instead of one per long list -- particles with long lists sit together (a film, a cluster), and a burst of ~2,000
+// same-address atomics with a return value at the end of a short phase is what the phase then waits for.
+template <typename T>
+__device__ __forceinline__ void finish_list_warp(const Params<T>& p, const Verlet<T>& v, int i, bool live, int nvv, int nvw, int face,
+                                                 int hcap, int hcap32, int hp)
+{
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    const int n = nvv + nvw;
+    int raw = min(nvv, VL_MAXN) | (min(nvw, VL_MAXN) << VL_NVW_SHIFT) | (face << VL_FACE_SHIFT);
+    const bool over = live && n > VL_MAXN;
+    if (over) { v.flags[VF_OVERFLOW] = 1; raw = face << VL_FACE_SHIFT; }
+    const bool heavy = live && !over &&
+                       (n > v.heavy_t || ((nvv + VL_BATCH - 1) / VL_BATCH + (nvw + VL_BATCH - 1) / VL_BATCH) * VL_BATCH > v.heavy_t + VL_BATCH - 1);
+    const bool want32 = heavy && n > VL_WARP_T && hcap32 > 0;
+    const unsigned m32 = __ballot_sync(0xffffffffu, want32);
+    int b32 = 0;
+    if (lane == 0 && m32) b32 = atomicAdd(v.flags + VF_NHEAVY32 + hp, __popc(m32));
+    b32 = __shfl_sync(0xffffffffu, b32, 0);
+    bool placed = false;
+    if (want32) {
+        const int h = b32 + __popc(m32 & lt);
+        placed = h < hcap32;
+        if (placed) { raw |= VL_HEAVY; v.cell[p.nv - 1 - h] = i; v.slot[p.nv - 1 - h] = raw; }
+    }
+    const bool want4 = heavy && !placed;
+    const unsigned m4 = __ballot_sync(0xffffffffu, want4);
+    int b4 = 0;
+    if (lane == 0 && m4) b4 = atomicAdd(v.flags + VF_NHEAVY + hp, __popc(m4));
+    b4 = __shfl_sync(0xffffffffu, b4, 0);
+    if (want4) {
+        const int h = b4 + __popc(m4 & lt);
+        if (h < hcap) { raw |= VL_HEAVY; v.cell[h] = i; v.slot[h] = raw; }
+    }
+    if (live) v.ncnt[i] = raw;
 }
 
 // R4: neighbour list from the cell list (a3's cell traversal, cached): every j within r_c + skin of i, vapor entries from
@@ -711,11 +777,15 @@ __device__ __forceinline__ void finish_list(const Params<T>& p, const Verlet<T>&
 // work whose cost grows with the SQUARE of the local density -- a warp per block of cells, candidates in a tile: measured
 // at 45-60 us -- lose to this one, where a particle's candidates are spread over nine lanes and three particles share a
 // warp: its cost is linear in the density (39 us in round 1, in FP64 with folds).
-template <typename T>
-__device__ __forceinline__ void list_range(const F4* __restrict__ q, int jb, int je, int skip, float xe, float ye, float ze, float rl2,
-                                           int e0, int* __restrict__ lst, size_t stride, int* cnt, bool up)
+// One range of candidates for particle i.  cnt[0], cnt[1]: inner / outer counters of the section (shared memory).
+// (A branch-free variant -- all distances of a batch first, one atomic per lane, batch and list, predicated stores -- was
+// measured and is no faster at 65,536 particles and 16 % slower at 2^20: this phase is bound by its dependent loads.)
+template <typename T, bool OUTER>
+__device__ __forceinline__ void list_range(const Verlet<T>& v, const F4* __restrict__ q, int jb, int je, int skip, float xe, float ye,
+                                           float ze, int e0, int i, int* cnt, bool up)
 {
     constexpr int NB = 8;                                                // a cell row rarely holds more
+    const float rl2 = v.rl2f, rl2o = v.rl2f_out;
     for (int j0 = jb; j0 < je; j0 += NB) {
         F4 rj[NB];
 #pragma unroll
@@ -724,34 +794,42 @@ __device__ __forceinline__ void list_range(const F4* __restrict__ q, int jb, int
         for (int u = 0; u < NB; ++u) {
             const int j = j0 + u;
             const float dx = xe - rj[u].x, dy = ye - rj[u].y, dz = ze - rj[u].z;
-            if (j < je && j != skip && fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < rl2) {
-                const int k = atomicAdd(cnt, 1);
-                if (k < VL_MAXN) lst[(size_t)(up ? k : VL_MAXN - 1 - k) * stride] = e0 + j;
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            if (j < je && j != skip && r2 < (OUTER ? rl2o : rl2)) {
+                if (OUTER) {
+                    const int k = atomicAdd(cnt + 1, 1);
+                    if (k < VL_MAXO) v.onbr[vl_base(i, VL_MAXO) + (up ? k : VL_MAXO - 1 - k) * VL_LS] = e0 + j;
+                }
+                if (!OUTER || r2 < rl2) {
+                    const int k = atomicAdd(cnt, 1);
+                    if (k < VL_MAXN) v.nbr[vl_base(i, VL_MAXN) + (up ? k : VL_MAXN - 1 - k) * VL_LS] = e0 + j;
+                }
             }
         }
     }
 }
 
-template <typename T, int ROWS>
+// OUTER: the cells have side >= r_c + outer skin and every hit also goes to the outer list (two-level list).
+template <typename T, int ROWS, bool OUTER>
 __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>& v, int c, int gtid, int gthreads, int hcap,
-                                            int hcap32)
+                                            int hcap32, int hp)
 {
     constexpr bool GHOSTS = sizeof(T) == 8;
     constexpr int PPW = 32 / ROWS;                       // particles per warp
-    __shared__ int s_cv[(VL_THREADS / 32) * PPW], s_cw[(VL_THREADS / 32) * PPW];
+    __shared__ int s_cv[(VL_THREADS / 32) * PPW][2], s_cw[(VL_THREADS / 32) * PPW][2];
     Vec4<T>* __restrict__ r = v.st[c].r;
     const F4* __restrict__ q = GHOSTS ? v.r32 : reinterpret_cast<const F4*>(r);
     const int nx = p.nc[0], ny = p.nc[1], nz = p.nc[2];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int pl = lane / ROWS, row = lane - pl * ROWS;
     const int warp = gtid >> 5, nwarps = gthreads >> 5;
-    int* cv = s_cv + wib * PPW + min(pl, PPW - 1);
-    int* cw = s_cw + wib * PPW + min(pl, PPW - 1);
+    int* cv = s_cv[wib * PPW + min(pl, PPW - 1)];
+    int* cw = s_cw[wib * PPW + min(pl, PPW - 1)];
     const int istride = GHOSTS ? v.ntot : 0;
     for (int base = warp * PPW; base < p.nv; base += nwarps * PPW) {
         const int i = base + pl;
         const bool active = pl < PPW && i < p.nv;
-        if (active && row == 0) { *cv = 0; *cw = 0; }
+        if (active && row == 0) { cv[0] = cv[1] = 0; cw[0] = cw[1] = 0; }
         __syncwarp();
         Vec4<T> ri = {T(0), T(0), T(0), T(0)};
         int face = 0;
@@ -784,17 +862,166 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
                     wb = v.wstart[rowc + x0]; we = v.wstart[rowc + x1 + 1];
                     if (xw >= 0) { wb2 = v.wstart[rowc + xw]; we2 = v.wstart[rowc + xw + 1]; }
                 }
-                int* __restrict__ lst = v.nbr + i;
-                list_range<T>(q, jb, je, img ? -1 : i, xe, ye, ze, v.rl2f, img * istride, lst, v.stride, cv, true);
-                list_range<T>(q, jb2, je2, -1, xe2, ye, ze, v.rl2f, (img | 1) * istride, lst, v.stride, cv, true);
-                list_range<T>(q + p.nv, wb, we, -1, xe, ye, ze, v.rl2f, img * istride + p.nv, lst, v.stride, cw, false);
-                list_range<T>(q + p.nv, wb2, we2, -1, xe2, ye, ze, v.rl2f, (img | 1) * istride + p.nv, lst, v.stride, cw, false);
+                list_range<T, OUTER>(v, q, jb, je, img ? -1 : i, xe, ye, ze, img * istride, i, cv, true);
+                list_range<T, OUTER>(v, q, jb2, je2, -1, xe2, ye, ze, (img | 1) * istride, i, cv, true);
+                list_range<T, OUTER>(v, q + p.nv, wb, we, -1, xe, ye, ze, img * istride + p.nv, i, cw, false);
+                list_range<T, OUTER>(v, q + p.nv, wb2, we2, -1, xe2, ye, ze, (img | 1) * istride + p.nv, i, cw, false);
             }
         }
         __syncwarp();
-        if (active && row == 0) finish_list(p, v, r, i, ri, *cv, *cw, face, hcap, hcap32);
+        if (active && row == 0) {
+            finish_list(p, v, r, i, ri, cv[0], cw[0], face, hcap, hcap32, hp);
+            if (OUTER) {
+                const int ov = cv[1], ow = cw[1];
+                int word = min(ov, VL_MAXO) | (min(ow, VL_MAXO) << VO_W_SHIFT) | (face << VO_FACE_SHIFT);
+                if (ov + ow > VL_MAXO) v.flags[VF_OUTER_BAD] = 1;            // not an error: no pruning from this list
+                else if (ov + ow > VO_HEAVY_T) { word |= VO_HEAVY; v.oheavy[atomicAdd(v.flags + VF_NOHEAVY, 1)] = i; }
+                v.ocnt[i] = word;
+            }
+        }
         __syncwarp();
     }
+}
+
+// R5, two-level list (the verdict's "take the rebuild off the critical path"): between two full
+// rebuilds the r_c + skin list is PRUNED from the outer list (every j within r_c + outer skin at the last full rebuild)
+// instead of being rebuilt from the cells: no bin, no scan, no scatter, no cell walk, ~17 distance tests per particle
+// instead of ~55 candidates -- one phase and one barrier, in the particle order of the last full rebuild.
+// Exactness: a pair within r_c + skin now was within r_c + outer skin at the full rebuild provided neither particle's
+// path since then exceeds outer_lim = (outer skin - skin) / 2.  The prune accumulates every particle's path (wo += w,
+// w = 0) and checks exactly that; if any particle violates it the caller discards the prune and runs a full rebuild
+// (the host sizes the outer skin so that this is rare: (nprune + 1) skins plus a margin for the step that crosses).
+// Tests are made on the positions themselves (T), entries keep their image codes; fp32 mode folds.  Particles with a long
+// outer list (VO_HEAVY: condensed regions) are pruned by a whole warp each, spread over all warps of the grid.
+// Returns: this thread saw a path beyond outer_lim.
+template <typename T, int NB>
+__device__ __forceinline__ bool phase_prune(const Params<T>& p, const Verlet<T>& v, int c, int gtid, int gthreads, int hcap,
+                                            int hcap32, int hp)
+{
+    constexpr bool FOLD = sizeof(T) == 4;
+    Vec4<T>* __restrict__ r = v.st[c].r;
+    const bool px = FOLD && p.bc[0] == BC_PERIODIC, py = FOLD && p.bc[1] == BC_PERIODIC, pz = FOLD && p.bc[2] == BC_PERIODIC;
+    const T rl2 = v.rl2_prune;
+    bool bad = false;
+#ifdef MD_DIAGNOSTICS
+    const unsigned long long t_in = now_ns();
+#endif
+    auto dist2 = [&](const Vec4<T>& ri, const Vec4<T>& rj) {
+        const T dx = px ? fold(ri.x, rj.x, p.L[0], T(0.5) * p.L[0]) : ri.x - rj.x;
+        const T dy = py ? fold(ri.y, rj.y, p.L[1], T(0.5) * p.L[1]) : ri.y - rj.y;
+        const T dz = pz ? fold(ri.z, rj.z, p.L[2], T(0.5) * p.L[2]) : ri.z - rj.z;
+        return fma_(dz, dz, fma_(dy, dy, dx * dx));
+    };
+    auto close = [&](int i, const Vec4<T>& ri, int nvv, int nvw, int face) {
+        const T wsum = v.wo[i] + ri.w;                   // path since the full rebuild
+        v.wo[i] = wsum;
+        if (wsum > v.outer_lim) bad = true;
+        r[i].w = T(0);                                   // path since this list event
+        finish_list(p, v, r, i, ri, nvv, nvw, face, hcap, hcap32, hp, false);
+    };
+    // ---- one thread per particle (the warp stays converged: lanes without work run with empty lists)
+    for (int i0 = gtid - (int)(threadIdx.x & 31); i0 < p.nv; i0 += gthreads) {
+        const int i = i0 + (int)(threadIdx.x & 31);
+        const bool inrange = i < p.nv;
+        const int word = inrange ? v.ocnt[i] : VO_HEAVY;
+        const bool live = !(word & VO_HEAVY);
+        const Vec4<T> ri = r[inrange ? i : 0];
+        const T wold = inrange ? v.wo[i] : T(0);         // issued early
+        const int ov = live ? word & VO_MASK : 0, ow = live ? (word >> VO_W_SHIFT) & VO_MASK : 0;
+        const int* __restrict__ ol = v.onbr + vl_base(i, VL_MAXO);
+        int* __restrict__ il = v.nbr + vl_base(i, VL_MAXN);
+        int cnt[2] = {0, 0};
+#pragma unroll
+        for (int sec = 0; sec < 2; ++sec) {              // vapor entries from slot 0 up, wall entries from the top slot down
+            const int ne = sec ? ow : ov;
+            int en[NB];
+#pragma unroll
+            for (int u = 0; u < NB; ++u) en[u] = u < ne ? ol[(sec ? VL_MAXO - 1 - u : u) * VL_LS] : -1;
+            for (int k = 0; k < ne; k += NB) {
+                int e[NB];
+                Vec4<T> rj[NB];
+#pragma unroll
+                for (int u = 0; u < NB; ++u) { e[u] = en[u]; rj[u] = r[max(e[u], 0)]; }
+#pragma unroll
+                for (int u = 0; u < NB; ++u) {
+                    const int kk = k + NB + u;
+                    en[u] = kk < ne ? ol[(sec ? VL_MAXO - 1 - kk : kk) * VL_LS] : -1;      // next batch
+                }
+                // all NB distances first -- independent FP64 chains, interleaved -- then the appends: written as one loop the
+                // compiler made every test a divergent branch around its own dependent chain (56 instructions per entry)
+                T r2[NB];
+#pragma unroll
+                for (int u = 0; u < NB; ++u) r2[u] = dist2(ri, rj[u]);
+#pragma unroll
+                for (int u = 0; u < NB; ++u) {
+                    const int hit = (int)(e[u] >= 0) & (int)(r2[u] < rl2);
+                    const int at = sec ? VL_MAXN - 1 - cnt[sec] : cnt[sec];
+                    if (hit & (int)(cnt[sec] < VL_MAXN)) il[at * VL_LS] = e[u];
+                    cnt[sec] += hit;
+                }
+            }
+        }
+        if (live) {
+            const T wsum = wold + ri.w;                  // path since the full rebuild
+            v.wo[i] = wsum;
+            if (wsum > v.outer_lim) bad = true;
+            r[i].w = T(0);                               // path since this list event
+        }
+        finish_list_warp(p, v, i, live, cnt[0], cnt[1], (word >> VO_FACE_SHIFT) & VL_FACE_MASK, hcap, hcap32, hp);
+    }
+#ifdef MD_DIAGNOSTICS
+    const unsigned long long tl = now_ns();
+#endif
+    // ---- one warp per particle with a long outer list
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    const int noh = v.flags[VF_NOHEAVY];
+    for (int h = gtid >> 5; h < noh; h += gthreads >> 5) {
+        const int i = v.oheavy[h];
+        const int word = v.ocnt[i];
+        const Vec4<T> ri = r[i];
+        const int ov = word & VO_MASK, ow = (word >> VO_W_SHIFT) & VO_MASK;
+        const int* __restrict__ ol = v.onbr + vl_base(i, VL_MAXO);
+        int* __restrict__ il = v.nbr + vl_base(i, VL_MAXN);
+        int cnt[2] = {0, 0};
+#pragma unroll
+        for (int sec = 0; sec < 2; ++sec) {
+            const int ne = sec ? ow : ov;
+            constexpr int NI = 4;                        // 128 entries per round: all index loads, then all position loads, in flight
+            for (int k0 = 0; k0 < ne; k0 += 32 * NI) {
+                int e[NI];
+                Vec4<T> rj[NI];
+#pragma unroll
+                for (int u = 0; u < NI; ++u) {
+                    const int k = k0 + 32 * u + lane;
+                    e[u] = k < ne ? ol[(sec ? VL_MAXO - 1 - k : k) * VL_LS] : -1;
+                }
+#pragma unroll
+                for (int u = 0; u < NI; ++u) rj[u] = r[max(e[u], 0)];
+                T r2[NI];
+#pragma unroll
+                for (int u = 0; u < NI; ++u) r2[u] = dist2(ri, rj[u]);
+#pragma unroll
+                for (int u = 0; u < NI; ++u) {
+                    const bool hit = (e[u] >= 0) & (r2[u] < rl2);
+                    const unsigned m = __ballot_sync(0xffffffffu, hit);
+                    const int pos = cnt[sec] + __popc(m & lt);
+                    if (hit && pos < VL_MAXN) il[(sec ? VL_MAXN - 1 - pos : pos) * VL_LS] = e[u];
+                    cnt[sec] += __popc(m);
+                }
+            }
+        }
+        if (lane == 0) close(i, ri, cnt[0], cnt[1], (word >> VO_FACE_SHIFT) & VL_FACE_MASK);
+        __syncwarp();
+    }
+#ifdef MD_DIAGNOSTICS
+    if (v.dbg && lane == 0) {          // per warp: ns in the two parts, summed over prunes; [2]: particles pruned by warps
+        atomicAdd(v.dbg + 4096 + 2 * ((gtid >> 5) & 1023), tl - t_in);
+        atomicAdd(v.dbg + 4097 + 2 * ((gtid >> 5) & 1023), now_ns() - tl);
+        if (gtid == 0) v.dbg[7000] += noh;
+    }
+#endif
+    return bad;
 }
 
 // ---- the persistent time loop ---------------------------------------------------------------------
@@ -806,7 +1033,7 @@ __device__ __forceinline__ void phase_build(const Params<T>& p, const Verlet<T>&
 template <typename T, int ROWS, int MINB>
 __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
 {
-    __shared__ unsigned long long s_times[8];
+    __shared__ unsigned long long s_times[10];
     GridBarrier bar_seq;
     const bool thermo = p.thermo_rate > 0.0;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -819,30 +1046,50 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
     const int nidle = max((int)gridDim.x - (p.nv + VL_THREADS - 1) / VL_THREADS, 0);
     const int hcap = nidle * (VL_THREADS / VL_GROUP), hcap32 = nidle * (VL_THREADS / 32) * VL_WARP_ROUNDS;
     if (gtid == 0)
-        for (int k = 0; k < 8; ++k) s_times[k] = 0;
+        for (int k = 0; k < 10; ++k) s_times[k] = 0;
     unsigned long long t0 = gtid == 0 ? now_ns() : 0ull, t1;
+    int hp = v.flags[VF_HPAR];          // which set of heavy-list counters the step phases read
+    int since_full = 1 << 30;           // prunes since the last full rebuild (unknown at launch: the first event is a full one
+                                        // unless the previous launch left a usable outer list, see below)
+    if (v.nprune > 0 && !force_rebuild) since_full = v.flags[VF_NPRUNE + 1];
     for (long long s = 0;; ++s) {
         if (rebuild) {
             unsigned long long u0 = gtid == 0 ? now_ns() : 0ull, u1;
-            if (gtid == 0) {
-                v.flags[VF_NHEAVY] = 0; v.flags[VF_HCAP] = hcap; v.flags[VF_NHEAVY32] = 0; v.flags[VF_HCAP32] = hcap32;
+            const int hw = hp ^ 1;                                       // the counter set this list event fills
+            if (gtid == 0) { v.flags[VF_HCAP] = hcap; v.flags[VF_HCAP32] = hcap32; }
+            bool full = force_rebuild || since_full >= v.nprune || *(volatile int*)(v.flags + VF_OUTER_BAD) != 0;
+            if (!full) {
+                const bool bad = phase_prune<T, MINB == 2 ? 8 : 4>(p, v, c, gtid, gthreads, hcap, hcap32, hw);
+                if (gtid == 0) v.flags[VF_NPRUNE] += 1;
+                full = grid_barrier(v.bar, bar_seq, bad);                // a path beyond outer_lim: the prune is void
+                ++since_full;
+                if (gtid == 0) { t1 = now_ns(); s_times[2] += t1 - t0; s_times[8] += t1 - t0; t0 = t1; u0 = t1; }
+                if (full && gtid == 0) { v.flags[VF_NHEAVY + hw] = 0; v.flags[VF_NHEAVY32 + hw] = 0; }    // refilled below
             }
-            phase_bin<T>(p, v, c, gtid, gthreads);
-            grid_barrier(v.bar, bar_seq);
-            if (gtid == 0) { u1 = now_ns(); s_times[4] += u1 - u0; u0 = u1; }
-            phase_scan(v.count, p.ncell, v.tile_agg, (unsigned int)v.flags[VF_NREBUILD] + 1u, v.start);
-            grid_barrier(v.bar, bar_seq);
-            if (gtid == 0) { u1 = now_ns(); s_times[5] += u1 - u0; u0 = u1; }
-            phase_scatter<T>(p, v, c, cv, gtid, gthreads);
-            grid_barrier(v.bar, bar_seq);
-            if (gtid == 0) { u1 = now_ns(); s_times[6] += u1 - u0; u0 = u1; }
-            c ^= 1; cv ^= 1;
-            phase_build<T, ROWS>(p, v, c, gtid, gthreads, hcap, hcap32);
-            for (int q = gtid; q < p.ncell; q += gthreads) v.count[q] = 0;                  // for the next rebuild
-            if (gtid == 0) v.flags[VF_NREBUILD] += 1;
-            grid_barrier(v.bar, bar_seq);
-            if (gtid == 0) { t1 = now_ns(); s_times[2] += t1 - t0; t0 = t1; s_times[7] += t1 - u0; }
-            carry.valid = carry.hvalid = carry.nhvalid = false;          // new particle order, new lists
+            if (full) {
+                if (gtid == 0) v.flags[VF_NOHEAVY] = 0;
+                phase_bin<T>(p, v, c, gtid, gthreads);
+                grid_barrier(v.bar, bar_seq);
+                if (gtid == 0) { u1 = now_ns(); s_times[4] += u1 - u0; u0 = u1; }
+                phase_scan(v.count, p.ncell, v.tile_agg, (unsigned int)v.flags[VF_NREBUILD] + 1u, v.start);
+                grid_barrier(v.bar, bar_seq);
+                if (gtid == 0) { u1 = now_ns(); s_times[5] += u1 - u0; u0 = u1; }
+                phase_scatter<T>(p, v, c, cv, gtid, gthreads);
+                if (gtid == 0) v.flags[VF_OUTER_BAD] = 0;                // everybody has taken this event's decision by now
+                grid_barrier(v.bar, bar_seq);
+                if (gtid == 0) { u1 = now_ns(); s_times[6] += u1 - u0; u0 = u1; }
+                c ^= 1; cv ^= 1;
+                if (v.nprune > 0) phase_build<T, ROWS, true>(p, v, c, gtid, gthreads, hcap, hcap32, hw);
+                else phase_build<T, ROWS, false>(p, v, c, gtid, gthreads, hcap, hcap32, hw);
+                for (int q = gtid; q < p.ncell; q += gthreads) v.count[q] = 0;                  // for the next rebuild
+                if (gtid == 0) v.flags[VF_NREBUILD] += 1;
+                grid_barrier(v.bar, bar_seq);
+                since_full = 0;
+                if (gtid == 0) { t1 = now_ns(); s_times[2] += t1 - t0; t0 = t1; s_times[7] += t1 - u0; }
+            }
+            hp = hw;
+            if (gtid == 0) { v.flags[VF_NHEAVY + (hp ^ 1)] = 0; v.flags[VF_NHEAVY32 + (hp ^ 1)] = 0; }   // the retired set, for the next event
+            carry.valid = carry.hvalid = carry.nhvalid = false;          // new lists (and, after a full rebuild, a new particle order)
         }
         if (s == n_steps) break;
         bool want = false;                                   // this thread asks for a rebuild before the next step
@@ -852,20 +1099,19 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
         if (v.dbg) dbg0 = now_ns();
 #endif
         if (!thermo || s == 0) {
-            phase_step<T>(p, v, c, cv, s > 0, s > 0, true, want, gtid, gthreads, T(1), nullptr, carry, cyon);
+            phase_step<T>(p, v, c, cv, s > 0, s > 0, true, want, gtid, gthreads, hp, T(1), nullptr, carry, cyon);
         } else {
             // with the thermostat lambda(t) needs K(t) of ALL particles before the next drift: the fused phase splits
             // into [F1 + F3 + K partial sums] | barrier | [F4 rescale + F2], one extra barrier per step
-            phase_step<T>(p, v, c, cv, true, true, false, want, gtid, gthreads, T(1), v.ksum + s % 3);
+            phase_step<T>(p, v, c, cv, true, true, false, want, gtid, gthreads, hp, T(1), v.ksum + s % 3);
             grid_barrier(v.bar, bar_seq);
             const double lam = berendsen_lambda(*(volatile double*)(v.ksum + s % 3), p.thermo_rate, p.t_target, p.dof);
-            phase_step<T>(p, v, c, cv, false, false, true, want, gtid, gthreads, (T)lam);
+            phase_step<T>(p, v, c, cv, false, false, true, want, gtid, gthreads, hp, (T)lam);
         }
 #ifdef MD_DIAGNOSTICS
         if (v.dbg && (threadIdx.x & 31) == 0) {
             const unsigned long long dt = now_ns() - dbg0;
             atomicAdd(v.dbg + (gtid >> 5), dt);
-            if (s > 0 && !rebuild) atomicMax(v.dbg + 4096 + (gtid >> 5), dt);
             atomicAdd(v.dbg + 8000 + min((int)(dt >> 10), 15), 1ull);       // histogram of warp-phase times, ~1 us bins
         }
 #endif
@@ -877,18 +1123,19 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
     if (thermo && n_steps > 0) {
         double* ks = v.ksum + n_steps % 3;
         bool unused = false;
-        phase_step<T>(p, v, c, cv, true, true, false, unused, gtid, gthreads, T(1), ks);
+        phase_step<T>(p, v, c, cv, true, true, false, unused, gtid, gthreads, hp, T(1), ks);
         grid_barrier(v.bar, bar_seq);
         const double lam = berendsen_lambda(*(volatile double*)ks, p.thermo_rate, p.t_target, p.dof);
-        phase_step<T>(p, v, c, cv, false, false, false, unused, gtid, gthreads, (T)lam);      // F4 of the last step
+        phase_step<T>(p, v, c, cv, false, false, false, unused, gtid, gthreads, hp, (T)lam);      // F4 of the last step
     } else if (n_steps > 0 || force_rebuild) {
         bool unused = false;
-        phase_step<T>(p, v, c, cv, true, n_steps > 0, false, unused, gtid, gthreads);
+        phase_step<T>(p, v, c, cv, true, n_steps > 0, false, unused, gtid, gthreads, hp);
     }
     if (gtid == 0) {
         v.flags[VF_CUR] = c; v.flags[VF_CURV] = cv;
         s_times[3] += now_ns() - t0;
-        for (int k = 0; k < 8; ++k) v.times[k] += s_times[k];
+        for (int k = 0; k < 10; ++k) v.times[k] += s_times[k];
+        v.flags[VF_HPAR] = hp; v.flags[VF_NPRUNE + 1] = since_full;
     }
 }
 
@@ -898,7 +1145,14 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
 template <typename T, int ROWS>
 __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_build(Params<T> p, Verlet<T> v, int c)
 {
-    phase_build<T, ROWS>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, v.flags[VF_HCAP], v.flags[VF_HCAP32]);
+    phase_build<T, ROWS, false>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, v.flags[VF_HCAP], v.flags[VF_HCAP32], v.flags[VF_HPAR]);
+}
+
+// Diagnostics build only: the prune phase as a kernel of its own (valid at any time: it re-prunes from the outer list).
+template <typename T>
+__global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_prune(Params<T> p, Verlet<T> v, int c)
+{
+    phase_prune<T, 8>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, 0, 0, v.flags[VF_HPAR] ^ 1);
 }
 
 // Diagnostics build only: the force part of the step phase as a kernel of its own (recomputes f(t)).
@@ -906,7 +1160,7 @@ template <typename T>
 __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_force(Params<T> p, Verlet<T> v, int c, int cv)
 {
     bool unused = false;
-    phase_step<T>(p, v, c, cv, true, false, false, unused, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+    phase_step<T>(p, v, c, cv, true, false, false, unused, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, v.flags[VF_HPAR]);
 }
 #endif
 

@@ -41,7 +41,7 @@ class md_lj(C.Structure):
 
 class md_opts(C.Structure):
     _fields_ = [("dt", C.c_double), ("mass", C.c_double), ("precision", C.c_int), ("force_algo", C.c_int),
-                ("skin", C.c_double), ("tau_b", C.c_double), ("t_target", C.c_double), ("heavy_list", C.c_int)]
+                ("skin", C.c_double), ("tau_b", C.c_double), ("t_target", C.c_double), ("heavy_list", C.c_int), ("list_prunes", C.c_int)]
 
 
 class md_energy_out(C.Structure):
@@ -58,7 +58,7 @@ class md_pressure_out(C.Structure):
 
 class md_kernel_times(C.Structure):
     _fields_ = [("ms", C.c_double * 4), ("launches", C.c_longlong * 4), ("total_ms", C.c_double),
-                ("steps", C.c_longlong), ("rebuilds", C.c_longlong), ("rebuild_ms", C.c_double * 4)]
+                ("steps", C.c_longlong), ("rebuilds", C.c_longlong), ("rebuild_ms", C.c_double * 4), ("prunes", C.c_longlong), ("prune_ms", C.c_double)]
 
 
 class md_peaks(C.Structure):
@@ -133,6 +133,7 @@ def _structs(cfg, precision=64, algo=None):
     opts.skin = float(cfg.get("skin", 0.0))
     opts.tau_b, opts.t_target = float(cfg.get("tau_b", 0.0)), float(cfg.get("t_target", 1.0))
     opts.heavy_list = int(cfg.get("heavy_list", 0))
+    opts.list_prunes = int(cfg.get("list_prunes", 0))
     return box, lj, opts
 
 
@@ -230,7 +231,7 @@ class Simulation:
         t = md_kernel_times()
         self._check(self._lib.md_profile_step(self._h, int(n_steps), C.byref(t)))
         return dict(ms=list(t.ms), launches=list(t.launches), total_ms=t.total_ms, steps=t.steps, rebuilds=t.rebuilds,
-                    rebuild_ms=list(t.rebuild_ms))
+                    rebuild_ms=list(t.rebuild_ms), prunes=t.prunes, prune_ms=t.prune_ms)
 
     def pair_tests(self) -> int:
         v = C.c_longlong()

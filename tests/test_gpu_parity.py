@@ -693,3 +693,30 @@ def test_fp32_mode_monitors(algo):
     ra_ref = np.bincount(b[inside & (b < 10)], minlength=10)
     assert ax.sum() == cfg["n_vapor"] and np.array_equal(ax, ax_ref) and np.array_equal(ra, ra_ref)
     sim.close()
+
+
+@pytest.mark.parametrize("list_prunes", [-1, 1, 2, 4])
+def test_verlet_two_level_list_prunes(list_prunes):
+    """md_opts.list_prunes: between two full rebuilds the r_c + skin list is pruned from an outer list.  Every setting --
+    none (single-level list), the default two, and more than the box allows (reduced automatically) -- must give the
+    oracle's forces and trajectory: 300 steps span several full rebuilds and prunes (checked through md_profile_step's
+    counters), in chunks so that a launch starts with prunes pending from the previous one."""
+    cfg = dict(I.config4(12), list_prunes=list_prunes)
+    check_step0(cfg, "verlet")
+    ref = O.run(cfg, 300, cells=True)
+    sim = make_sim(cfg, "verlet")
+    events = [sim.profile_step(n) for n in (7, 93, 1, 199)]
+    st, en = sim.get_state(), sim.energy()
+    rebuilds, prunes = sum(e["rebuilds"] for e in events), sum(e["prunes"] for e in events)
+    assert rebuilds >= 3
+    assert (prunes == 0) if list_prunes < 0 else (prunes >= rebuilds)
+    # 300 steps: the 1e-8 sigma bound of 100 steps grows with the Lyapunov time (measured 3e-9); K, U to 1e-7
+    assert traj_error(st["pos"], ref["pos"], cfg["box_len"], cfg["bc"]) <= 1e-6
+    scale = max(abs(ref["U"]), ref["K"])
+    assert abs(en["K"] - ref["K"]) <= 1e-7 * scale and abs(en["U"] - ref["U"]) <= 1e-7 * scale
+    sim.close()
+    # a box too small for any outer list (the setting is reduced to none), a dense 2D fluid, the thermostat's split phases
+    for small, extra in ((I.small_case(3, 200, (9.6, 10.5, 9.9), (0, 0, 1), n_wall=30, seed=8, min_sep=0.9), {}),
+                         (I.config0(), {}), (I.config4(10), dict(tau_b=0.1, t_target=0.7))):
+        c = dict(small, list_prunes=list_prunes, **extra)
+        check_traj(c, "verlet", 100, cells_oracle=c["n_vapor"] > 500)

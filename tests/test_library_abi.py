@@ -32,7 +32,7 @@ def test_exports_every_declared_symbol(lib):
 
 def test_struct_sizes_match_header_layout():
     assert C.sizeof(md.md_box) == 48 and C.sizeof(md.md_lj) == 48 and C.sizeof(md.md_opts) == 56
-    assert C.sizeof(md.md_energy_out) == 64 and C.sizeof(md.md_kernel_times) == 120 and C.sizeof(md.md_peaks) == 24
+    assert C.sizeof(md.md_energy_out) == 64 and C.sizeof(md.md_kernel_times) == 136 and C.sizeof(md.md_peaks) == 24
 
 
 def test_workspace_bytes_scale_and_reject(lib):
