@@ -28,6 +28,10 @@ constexpr int AD_THREADS = 128;   // threads per block = entries per shared-memo
 constexpr int AD_IB = MD_AD_IB;   // particles i per thread for large N; 1 below AD_SMALL_N (more, shorter blocks: the
 constexpr int AD_SMALL_N = 8192;  // kernel is latency-bound there, profiles/r01_final_cfg2.md)
 constexpr int AD_UNROLL = MD_AD_UNROLL;   // tests per i between two candidate checks
+#ifndef MD_AD_JB
+#define MD_AD_JB 4
+#endif
+constexpr int AD_JB = MD_AD_JB;           // list entries whose tests are advanced together, stage by stage
 
 struct AllPairsDot {
     Vec4<double>* jv;      // [nv + cap_ghost]: real vapor entries in particle order, then this step's ghosts
@@ -186,17 +190,38 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double
         __syncthreads();
         nxt = fetch(t + gridDim.y);
         for (int k0 = 0; k0 < AD_THREADS; k0 += AD_UNROLL) {
-            int cand = 0;
+            // one integer instruction per test beside the four FP64 ones: the running minimum of the high words (for
+            // r^2 >= 0 the high word orders like the value; a slightly negative r^2 -- cancellation -- is smaller still)
+            int lowest = 0x7fffffff;
 #pragma unroll
-            for (int u = 0; u < AD_UNROLL; ++u) {
-                const Vec4<double> q = sj[k0 + u];
+            for (int u = 0; u < AD_UNROLL; u += AD_JB) {
+                // AD_JB entries x IB particles independent chains, advanced one stage at a time
+                Vec4<double> q[AD_JB];
+                double r2[AD_JB][IB];
 #pragma unroll
-                for (int b = 0; b < IB; ++b) {
-                    const double r2 = fma(ax[b], q.x, fma(ay[b], q.y, fma(az[b], q.z, si[b] + q.w)));
-                    cand |= (__double2hiint(r2) < thr);
-                }
+                for (int w = 0; w < AD_JB; ++w) q[w] = sj[k0 + u + w];
+#pragma unroll
+                for (int w = 0; w < AD_JB; ++w)
+#pragma unroll
+                    for (int b = 0; b < IB; ++b) r2[w][b] = si[b] + q[w].w;
+#pragma unroll
+                for (int w = 0; w < AD_JB; ++w)
+#pragma unroll
+                    for (int b = 0; b < IB; ++b) r2[w][b] = fma(az[b], q[w].z, r2[w][b]);
+#pragma unroll
+                for (int w = 0; w < AD_JB; ++w)
+#pragma unroll
+                    for (int b = 0; b < IB; ++b) r2[w][b] = fma(ay[b], q[w].y, r2[w][b]);
+#pragma unroll
+                for (int w = 0; w < AD_JB; ++w)
+#pragma unroll
+                    for (int b = 0; b < IB; ++b) r2[w][b] = fma(ax[b], q[w].x, r2[w][b]);
+#pragma unroll
+                for (int w = 0; w < AD_JB; ++w)
+#pragma unroll
+                    for (int b = 0; b < IB; ++b) lowest = min(lowest, __double2hiint(r2[w][b]));
             }
-            if (cand) {      // some lane of the warp has a candidate: each lane redoes ITS flagged pairs exactly
+            if (lowest < thr) {      // this lane has a candidate in the group: it redoes ITS flagged pairs exactly
                 for (int u = 0; u < AD_UNROLL; ++u) {
                     const Vec4<double> q = sj[k0 + u];
 #pragma unroll
