@@ -11,13 +11,14 @@
 // pair within r_c is evaluated at every step: results are exact, identical to the brute-force
 // definition up to summation order.
 //
-// Round 2 (profiles/r02_*.md): (i) the list build is one thread per particle walking the 3^(d-1) cell rows
-// with an FP32 distance filter on a float4 shadow of the positions (the list only has to be a SUPERSET of the
-// pairs within r_c + skin; the force loop still takes the r < r_c decision in full precision), (ii) periodic
-// images are materialised as ghost copies the owner rewrites in its drift, so the time loop never folds a
-// difference, (iii) a list holds its vapor entries first and its wall entries after them, so the pair loop
-// carries one set of coefficients, (iv) particles in dense neighbourhoods (adsorbed films, clusters) no longer set the
-// pace: their lists are built by a whole warp each, and lists longer than 32 entries are evaluated by a whole warp.
+// Round 2 (profiles/r02_*.md): (i) the list build runs its distance filter in FP32 on a float4 shadow of the positions
+// (the list only has to be a SUPERSET of the pairs within r_c + skin; the force loop still takes the r < r_c decision in
+// full precision); (ii) periodic images are materialised as ghost copies the owner rewrites in its drift, so the time loop
+// never folds a difference; (iii) a list holds its vapor entries from the first slot up and its wall entries from the last
+// slot down, so the pair loop carries one set of coefficients at a time; (iv) lists are stored warp-blocked with a constant
+// stride between a particle's entries; (v) the grid barrier is a release reduction plus one acquire load and carries the
+// rebuild request; (vi) TWO-LEVEL LIST: between two full rebuilds (bin, scan, scatter, cell walk) the r_c + skin list is
+// pruned from an outer list of the pairs within r_c + outer skin (phase_prune), exactly.
 #pragma once
 #include "md_kernels.cuh"
 
