@@ -58,7 +58,7 @@ typedef struct { int dim; double len[3]; int bc[3]; } md_box;
  * |r[1-axis] - center[1-axis]| < length/2.  MD_PORE_PRISM switches on GEOMETRIC walls (the paper's own pore,
  * PAPER.md:115-121, :186): the axis-aligned box of size `length` along `axis` and `width` across, centred at `center`,
  * reflects particles specularly from both sides of every face except the open one at +axis; it must lie at least
- * max(1, skin) length units inside the simulation box.  Other kinds are stored but neither monitored nor active. */
+ * max(1, outer skin) length units inside the simulation box (outer skin: see md_opts.list_prunes; 1.93 by default).  Other kinds are stored but neither monitored nor active. */
 typedef struct { int kind, axis; double center[3], length, r0, r1, neck_len, width; } md_pore;
 
 /* 12-6 Lennard-Jones: u(r) = 4 eps [(sigma/r)^12 - (sigma/r)^6] for r < r_cut, else 0 (strict <);

@@ -1097,10 +1097,11 @@ int md_create(md_sim** out, const md_box* box, const md_pore* pore, const md_lj*
         }
         for (int a = 0; a < dim; ++a) {
             const double h = 0.5 * (a == pore->axis ? pore->length : pore->width);
-            // VERLET leaves periodic coordinates unwrapped by up to skin / 2 + one step between rebuilds
-            const double margin = std::max(1.0, list_skin(*lj, *o));
+            // VERLET leaves periodic coordinates unwrapped between FULL rebuilds: by up to (outer skin - skin) / 2 + skin / 2
+            // + one step with the two-level list
+            const double margin = std::max(1.0, outer_skin(list_skin(*lj, *o), resolve_prunes(*box, *lj, *o)));
             if (!(pore->center[a] - h >= margin) || !(pore->center[a] + h <= box->len[a] - margin)) {
-                g_create_error = "prism pore must lie at least max(1, skin) length units inside the box";
+                g_create_error = "prism pore must lie at least max(1, outer skin) length units inside the box";
                 return MD_ERR_INVALID_ARG;
             }
         }

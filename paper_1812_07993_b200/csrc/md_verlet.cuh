@@ -779,33 +779,49 @@ __device__ __forceinline__ void finish_list_warp(const Params<T>& p, const Verle
 // at 45-60 us -- lose to this one, where a particle's candidates are spread over nine lanes and three particles share a
 // warp: its cost is linear in the density (39 us in round 1, in FP64 with folds).
 // One range of candidates for particle i.  cnt[0], cnt[1]: inner / outer counters of the section (shared memory).
-// (A branch-free variant -- all distances of a batch first, one atomic per lane, batch and list, predicated stores -- was
-// measured and is no faster at 65,536 particles and 16 % slower at 2^20: this phase is bound by its dependent loads.)
+// Per batch of NB candidates a lane turns its hits into two bit masks, reserves their slots with ONE shared-memory atomic
+// per list, and stores them in a loop that runs as long as the lane with the most hits needs (3-4 trips for 8 candidates).
+// The obvious form -- test, atomic and store inside one `if` per candidate -- executes that hit path once per candidate
+// slot, because among the 27 active lanes some lane nearly always hits: it was half of the build's 10,300 instructions per
+// warp (ncu, profiles/r02_k_md_run.md).  (Eight predicated store sequences per batch instead of the loop were no faster.)
 template <typename T, bool OUTER>
 __device__ __forceinline__ void list_range(const Verlet<T>& v, const F4* __restrict__ q, int jb, int je, int skip, float xe, float ye,
                                            float ze, int e0, int i, int* cnt, bool up)
 {
     constexpr int NB = 8;                                                // a cell row rarely holds more
     const float rl2 = v.rl2f, rl2o = v.rl2f_out;
+    int* __restrict__ il = v.nbr + vl_base(i, VL_MAXN);
+    int* __restrict__ ol = OUTER ? v.onbr + vl_base(i, VL_MAXO) : nullptr;
     for (int j0 = jb; j0 < je; j0 += NB) {
         F4 rj[NB];
 #pragma unroll
         for (int u = 0; u < NB; ++u) rj[u] = q[min(j0 + u, je - 1)];     // NB loads in flight
+        unsigned mi = 0u, mo = 0u;
 #pragma unroll
         for (int u = 0; u < NB; ++u) {
-            const int j = j0 + u;
             const float dx = xe - rj[u].x, dy = ye - rj[u].y, dz = ze - rj[u].z;
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            if (j < je && j != skip && r2 < (OUTER ? rl2o : rl2)) {
-                if (OUTER) {
-                    const int k = atomicAdd(cnt + 1, 1);
-                    if (k < VL_MAXO) v.onbr[vl_base(i, VL_MAXO) + (up ? k : VL_MAXO - 1 - k) * VL_LS] = e0 + j;
-                }
-                if (!OUTER || r2 < rl2) {
-                    const int k = atomicAdd(cnt, 1);
-                    if (k < VL_MAXN) v.nbr[vl_base(i, VL_MAXN) + (up ? k : VL_MAXN - 1 - k) * VL_LS] = e0 + j;
-                }
-            }
+            const unsigned ok = (unsigned)(j0 + u < je) & (unsigned)(j0 + u != skip);
+            mi |= (ok & (unsigned)(r2 < rl2)) << u;
+            if (OUTER) mo |= (ok & (unsigned)(r2 < rl2o)) << u;
+        }
+        if (OUTER && mo) {
+            int k = atomicAdd(cnt + 1, __popc(mo));
+            do {
+                const int u = __ffs(mo) - 1;
+                mo &= mo - 1u;
+                if (k < VL_MAXO) ol[(up ? k : VL_MAXO - 1 - k) * VL_LS] = e0 + j0 + u;
+                ++k;
+            } while (mo);
+        }
+        if (mi) {
+            int k = atomicAdd(cnt, __popc(mi));
+            do {
+                const int u = __ffs(mi) - 1;
+                mi &= mi - 1u;
+                if (k < VL_MAXN) il[(up ? k : VL_MAXN - 1 - k) * VL_LS] = e0 + j0 + u;
+                ++k;
+            } while (mi);
         }
     }
 }
@@ -1146,7 +1162,9 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
 template <typename T, int ROWS>
 __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_build(Params<T> p, Verlet<T> v, int c)
 {
-    phase_build<T, ROWS, false>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, v.flags[VF_HCAP], v.flags[VF_HCAP32], v.flags[VF_HPAR]);
+    const int gtid = blockIdx.x * blockDim.x + threadIdx.x, gthreads = gridDim.x * blockDim.x;
+    if (v.nprune > 0) phase_build<T, ROWS, true>(p, v, c, gtid, gthreads, v.flags[VF_HCAP], v.flags[VF_HCAP32], v.flags[VF_HPAR]);
+    else phase_build<T, ROWS, false>(p, v, c, gtid, gthreads, v.flags[VF_HCAP], v.flags[VF_HCAP32], v.flags[VF_HPAR]);
 }
 
 // Diagnostics build only: the prune phase as a kernel of its own (valid at any time: it re-prunes from the outer list).

@@ -42,3 +42,35 @@ def test_reference_arm_line():
     d = _line("bench_r02_final_reference_arm.json.txt")
     assert d["impl"] == "reference" and d["metric"] == "pair-interactions/s" and d["cpu_baseline"]["kind"] == "oracle"
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"]
+
+
+def test_plain_start_with_gpus_n_spawns_n_ranks(monkeypatch):
+    """`python bench.py --gpus 8` started without torchrun must become the 8-rank job itself (one process per GPU)."""
+    import importlib.util
+    import sys
+
+    spec = importlib.util.spec_from_file_location("bench_under_test", os.path.join(ROOT, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    seen = {}
+
+    def fake_exec(prog, argv):
+        seen["argv"] = argv
+        raise SystemExit(0)
+
+    monkeypatch.setattr(bench.os, "execvp", fake_exec)
+    monkeypatch.delenv("RANK", raising=False)
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "8", "--steps", "2", "--warmup", "3"])
+    try:
+        bench.main()
+    except SystemExit:
+        pass
+    argv = seen["argv"]
+    assert "torch.distributed.run" in argv and argv[argv.index("--nproc-per-node") + 1] == "8"
+    assert argv[argv.index("--master-addr") + 1] == "127.0.0.1" and argv[-6:] == ["--gpus", "8", "--steps", "2", "--warmup", "3"]
+    # under torchrun (RANK set) it must not spawn again
+    seen.clear()
+    monkeypatch.setenv("RANK", "0")
+    monkeypatch.setattr(bench, "run_ours", lambda args: seen.setdefault("ran", args.gpus))
+    bench.main()
+    assert seen == {"ran": 8}
