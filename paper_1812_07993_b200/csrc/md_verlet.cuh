@@ -940,6 +940,12 @@ __device__ __forceinline__ bool phase_prune(const Params<T>& p, const Verlet<T>&
     for (int i0 = gtid - (int)(threadIdx.x & 31); i0 < p.nv; i0 += gthreads) {
         const int i = i0 + (int)(threadIdx.x & 31);
         const bool inrange = i < p.nv;
+        int olv[NB];                                     // issued together with the count word
+        {
+            const int* __restrict__ o0 = v.onbr + vl_base(i, VL_MAXO);
+#pragma unroll
+            for (int u = 0; u < NB; ++u) olv[u] = o0[u * VL_LS];
+        }
         const int word = inrange ? v.ocnt[i] : VO_HEAVY;
         const bool live = !(word & VO_HEAVY);
         const Vec4<T> ri = r[inrange ? i : 0];
@@ -952,8 +958,15 @@ __device__ __forceinline__ bool phase_prune(const Params<T>& p, const Verlet<T>&
         for (int sec = 0; sec < 2; ++sec) {              // vapor entries from slot 0 up, wall entries from the top slot down
             const int ne = sec ? ow : ov;
             int en[NB];
+            if (sec == 0) {                              // the first vapor entries do not wait for the count (the rows exist)
 #pragma unroll
-            for (int u = 0; u < NB; ++u) en[u] = u < ne ? ol[(sec ? VL_MAXO - 1 - u : u) * VL_LS] : -1;
+                for (int u = 0; u < NB; ++u) en[u] = olv[u];
+#pragma unroll
+                for (int u = 0; u < NB; ++u) en[u] = u < ne ? en[u] : -1;
+            } else {
+#pragma unroll
+                for (int u = 0; u < NB; ++u) en[u] = u < ne ? ol[(VL_MAXO - 1 - u) * VL_LS] : -1;
+            }
             for (int k = 0; k < ne; k += NB) {
                 int e[NB];
                 Vec4<T> rj[NB];
@@ -993,7 +1006,11 @@ __device__ __forceinline__ bool phase_prune(const Params<T>& p, const Verlet<T>&
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
     const int noh = v.flags[VF_NOHEAVY];
-    for (int h = gtid >> 5; h < noh; h += gthreads >> 5) {
+    // the warps of the blocks past the last particle have no list of their own to prune: they take these first, so that the
+    // long lists run beside the short ones instead of after them
+    const int nbl = min((int)gridDim.x, (p.nv + VL_THREADS - 1) / VL_THREADS), nidlew = ((int)gridDim.x - nbl) * (VL_THREADS / 32);
+    const int widx = (int)blockIdx.x >= nbl ? (gtid >> 5) - nbl * (VL_THREADS / 32) : nidlew + (gtid >> 5);
+    for (int h = widx; h < noh; h += gthreads >> 5) {
         const int i = v.oheavy[h];
         const int word = v.ocnt[i];
         const Vec4<T> ri = r[i];
