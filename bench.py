@@ -345,7 +345,7 @@ def main():
     ap.add_argument("--inner", type=int, default=2000, help="MD timesteps per bench step")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-inner", type=int, default=20, help="oracle timesteps per bench step (--impl reference)")
-    ap.add_argument("--cpu-steps", type=int, default=300, help="oracle timesteps of the cpu_baseline sample")
+    ap.add_argument("--cpu-steps", type=int, default=3000, help="oracle timesteps of the cpu_baseline sample (~15 s on 16 cores)")
     ap.add_argument("--allpairs-steps", type=int, default=10)
     ap.add_argument("--cpu-sweep", action="store_true", help="time the brute-force oracle for N_v = 2^10, 2^12, 2^14")
     args = ap.parse_args()
