@@ -345,7 +345,6 @@ struct Sim : md_sim {
             const int idle32 = cdiv(heavy32_seen * 5 / 4, md::VL_WARP_ROUNDS * (md::VL_THREADS / 32));
             coop_grid = std::min(coop_max, std::max(coop_base, light + std::max(light / 8, std::max(idle4, idle32)) + 1));
         }
-        CK(cudaMemsetAsync(l.vflags + md::VF_REQ0, 0, 3 * sizeof(int), stream));   // rebuild-request slots
         CK(cudaMemsetAsync(l.vbar, 0, 2 * sizeof(unsigned long long), stream));        // grid barrier counter
         CK(cudaMemsetAsync(l.vksum, 0, 4 * sizeof(double), stream));
         void* args[] = {(void*)&p, (void*)&vl, (void*)&n, (void*)&force_rebuild};

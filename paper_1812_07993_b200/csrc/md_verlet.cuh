@@ -42,7 +42,7 @@ __device__ __forceinline__ size_t vl_base(int i, int maxk) { return ((size_t)(i 
 // phases are not reading, and the set just retired is cleared one barrier before anybody can write it again); VF_HPAR =
 // the parity in use when the launch ended; VF_OUTER_BAD = the last outer list overflowed (no pruning until the next
 // outer build); VF_NOHEAVY = particles with a long OUTER list (pruned by a warp each); VF_NPRUNE = prunes so far.
-enum { VF_REQ0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_HCAP = 10,
+enum { VF_UNUSED0 = 0, VF_OVERFLOW = 3, VF_CUR = 4, VF_CURV = 5, VF_NREBUILD = 6, VF_ESCAPE = 7, VF_NHEAVY = 8, VF_HCAP = 10,
        VF_NHEAVY32 = 11, VF_HCAP32 = 13, VF_HPAR = 14, VF_OUTER_BAD = 15, VF_NOHEAVY = 16, VF_NPRUNE = 17 /* + 1: prunes since the last full rebuild */, VF_COUNT = 19 };
 
 // Shadow entry of the list build: (x, y, z) rounded to fp32.
@@ -72,7 +72,8 @@ struct Verlet {
     F4* r32;                   // [ntot] fp32 shadow of image block 0 (vapor part rewritten by every scatter); T = double only
     int* flags;                // VF_*
     unsigned long long* bar;   // grid barrier arrival counter
-    double* ksum;              // [3] kinetic-energy accumulators of the thermostat, rotating like the requests
+    double* ksum;              // [3] kinetic-energy accumulators of the thermostat, rotating over the steps (a slot is
+                               // cleared one barrier before the phase that adds to it and read one barrier after)
     unsigned long long* dbg;   // optional per-warp step-phase ns (diagnostics build), or nullptr
     unsigned long long* times; // [10] ns seen by thread 0: step phases, step barriers, list events, final phase,
                                // full-rebuild split: bin, scan, scatter, list build (each with its barrier); [8] prunes
