@@ -285,7 +285,7 @@ def run_ours(args):
     t_ap = ap["ms"][3] * 1e-3 / ap["launches"][3]
     ap_tests = sim_ap.pair_tests()
     sim_ap.close()
-    flops_per_test = 7.0            # executed per test: 1 DADD + 3 DFMA (md_allpairs.cuh)
+    flops_per_test = 6.0            # executed per test: 3 DFMA (md_allpairs.cuh)
     ap_tflops = ap_tests * flops_per_test / t_ap * 1e-12
     allpairs = {"kernel": "force_allpairs", "bound": "alu", "pair_tests_per_s": ap_tests / t_ap,
                 "achieved": ap_tflops, "peak": peaks["fp64_tflops"], "unit": "TFLOP/s",

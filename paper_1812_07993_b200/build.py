@@ -23,5 +23,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_operand_bench() -> str:
+    """Compiles the stand-alone FP64 operand-pattern diagnostic (csrc/fp64_operand_bench.cu; profiles/r02_counters.md
+    section 3) into build/fp64_operand_bench at the repository root.  Not part of the library."""
+    out_dir = os.path.join(HERE, "..", "build")
+    os.makedirs(out_dir, exist_ok=True)
+    exe = os.path.join(out_dir, "fp64_operand_bench")
+    subprocess.run([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+                    os.path.join(HERE, "csrc", "fp64_operand_bench.cu"), "-o", exe], check=True)
+    return os.path.abspath(exe)
+
+
 if __name__ == "__main__":
-    print(build(force=True, verbose=True))
+    import sys
+    if "--operand-bench" in sys.argv[1:]:
+        print(build_operand_bench())
+    else:
+        print(build(force=True, verbose=True))

@@ -2,16 +2,21 @@
 //
 // The paper's F1 tests every pair (Fig. 1 at :69-73).  With r_c = 2.5 sigma only ~5e-5 of
 // the tests at N = 65,536 are hits, so the kernel is the distance TEST, and the test is written to cost
-// four FP64 instructions:
-//     r^2 = (|r_i|^2 + |r_j|^2) - 2 x_i x_j - 2 y_i y_j - 2 z_i z_j      1 DADD + 3 DFMA  (7 flops)
-// with (x_j, y_j, z_j, |r_j|^2) staged through shared memory as one 32-byte entry, four particles i per
-// thread in registers, and the comparison done on the high word of r^2 by the integer pipe.  That form
-// loses ~1e-12 absolute in r^2, so it is only a conservative FILTER (threshold r_c^2 + margin): a group
-// of tests with any candidate re-evaluates its pairs exactly -- d = r_i - r_j, r^2 = fma(dz,dz,fma(dy,dy,
-// dx*dx)), strict r^2 < r_c^2 -- and only that exact path produces forces and energies.
+// three FP64 instructions:
+//     t = |r_i|^2 - r^2 = 2 x_i x_j + 2 y_i y_j + 2 z_i z_j - |r_j|^2      3 DFMA  (6 flops)
+//     r^2 < r_c^2  <=>  t > |r_i|^2 - r_c^2                                  (a threshold per particle i)
+// with (x_j, y_j, z_j, -|r_j|^2) staged through shared memory as one 32-byte entry (its last word starts the chain),
+// four particles i per thread in registers, and the comparison done by the integer pipe: the origin of the
+// coordinates is placed so that |r_i|^2 > r_c^2 + margin for every particle i (x is measured from r_c + 1 sigma
+// outside the box), hence every threshold is a positive double, positive doubles order like their high words, and a
+// negative t (a pair further apart than |r_i|) is a negative integer.  One running integer maximum per particle i
+// replaces the compare.  The form loses ~1e-11 absolute, and the high word of a value near |r_i|^2 has a grain of up
+// to 2^-20 |r_i|^2, so it is only a conservative FILTER: a group of tests with any candidate re-evaluates its pairs
+// exactly -- d = r_i - r_j, r^2 = fma(dz,dz,fma(dy,dy,dx*dx)), strict r^2 < r_c^2 -- and only that exact path
+// produces forces and energies.  (Until the last hours of round 2 the filter value was r^2 itself: 1 DADD + 3 DFMA.)
 // Periodic images are materialised once per step as ghost entries (particles within r_c of a periodic
-// face), so the inner loop has no minimum-image arithmetic.  Coordinates are centred on the box middle
-// to halve |r|^2.  The fp32 variant is at the end of this file; boxes with a periodic length below 2.2 r_c
+// face), so the inner loop has no minimum-image arithmetic.  y and z are centred on the box middle to keep |r|^2
+// small.  The fp32 variant is at the end of this file; boxes with a periodic length below 2.2 r_c
 // (more than one image per dimension) keep the per-pair minimum-image kernel of md_kernels.cuh.
 #pragma once
 #include "md_kernels.cuh"
@@ -38,8 +43,8 @@ struct AllPairsDot {
     Vec4<double>* jw;      // [nwg]: wall particles and their ghosts (static)
     int* ghost_count;      // number of vapor ghosts appended this step
     int nwg;
-    int thr_hi;            // candidate iff hi32(r^2 filter value) < thr_hi
-    double half[3];        // box centre
+    double thr;            // r_c^2 + rounding bound: candidate iff hi32(t) >= hi32(|r_i|^2 - thr)
+    double org[3];         // origin of the stored coordinates (entry = r - org): x: -(r_c + 1), y and z: box centre
     double edge;           // r_c + margin: distance from a periodic face that spawns a ghost
 };
 
@@ -50,16 +55,17 @@ __device__ __forceinline__ void push_images(const Params<double>& p, const AllPa
     // shift options per dimension: 0, and +-L when within `edge` of the opposite face
     double sx[2] = {0.0, 0.0}, sy[2] = {0.0, 0.0}, sz[2] = {0.0, 0.0};
     int nx = 1, ny = 1, nz = 1;
-    if (p.bc[0] == BC_PERIODIC) { if (x < a.edge - a.half[0]) sx[nx++] = p.L[0]; else if (x > a.half[0] - a.edge) sx[nx++] = -p.L[0]; }
-    if (p.bc[1] == BC_PERIODIC) { if (y < a.edge - a.half[1]) sy[ny++] = p.L[1]; else if (y > a.half[1] - a.edge) sy[ny++] = -p.L[1]; }
-    if (p.bc[2] == BC_PERIODIC) { if (z < a.edge - a.half[2]) sz[nz++] = p.L[2]; else if (z > a.half[2] - a.edge) sz[nz++] = -p.L[2]; }
+    // the box is [-org, L - org) in the stored coordinates
+    if (p.bc[0] == BC_PERIODIC) { if (x < a.edge - a.org[0]) sx[nx++] = p.L[0]; else if (x > p.L[0] - a.org[0] - a.edge) sx[nx++] = -p.L[0]; }
+    if (p.bc[1] == BC_PERIODIC) { if (y < a.edge - a.org[1]) sy[ny++] = p.L[1]; else if (y > p.L[1] - a.org[1] - a.edge) sy[ny++] = -p.L[1]; }
+    if (p.bc[2] == BC_PERIODIC) { if (z < a.edge - a.org[2]) sz[nz++] = p.L[2]; else if (z > p.L[2] - a.org[2] - a.edge) sz[nz++] = -p.L[2]; }
     for (int c = 0; c < nz; ++c)
         for (int b = 0; b < ny; ++b)
             for (int q = 0; q < nx; ++q) {
                 if (q + b + c == 0) continue;
                 Vec4<double> e;
                 e.x = x + sx[q]; e.y = y + sy[b]; e.z = z + sz[c];
-                e.w = fma(e.z, e.z, fma(e.y, e.y, e.x * e.x));
+                e.w = -fma(e.z, e.z, fma(e.y, e.y, e.x * e.x));
                 out[base + atomicAdd(counter, 1)] = e;
             }
 }
@@ -91,8 +97,8 @@ __global__ void __launch_bounds__(256) k_ap_kick_drift_list(Params<double> p, St
     }
     f.fx[i] = 0.0; f.fy[i] = 0.0; f.fz[i] = 0.0;
     Vec4<double> e;
-    e.x = ri.x - a.half[0]; e.y = ri.y - a.half[1]; e.z = ri.z - a.half[2];
-    e.w = fma(e.z, e.z, fma(e.y, e.y, e.x * e.x));
+    e.x = ri.x - a.org[0]; e.y = ri.y - a.org[1]; e.z = ri.z - a.org[2];
+    e.w = -fma(e.z, e.z, fma(e.y, e.y, e.x * e.x));
     a.jv[i] = e;
     push_images(p, a, e.x, e.y, e.z, a.jv, p.nv, a.ghost_count);
 }
@@ -103,8 +109,8 @@ __global__ void k_ap_wall_list(Params<double> p, const Vec4<double>* __restrict_
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= p.nw) return;
     Vec4<double> e;
-    e.x = wr[i].x - a.half[0]; e.y = wr[i].y - a.half[1]; e.z = wr[i].z - a.half[2];
-    e.w = fma(e.z, e.z, fma(e.y, e.y, e.x * e.x));
+    e.x = wr[i].x - a.org[0]; e.y = wr[i].y - a.org[1]; e.z = wr[i].z - a.org[2];
+    e.w = -fma(e.z, e.z, fma(e.y, e.y, e.x * e.x));
     a.jw[i] = e;
     push_images(p, a, e.x, e.y, e.z, a.jw, p.nw, counter);
 }
@@ -152,28 +158,28 @@ template <bool ENERGY, int IB>
 __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double> p, AllPairsDot a, Force<double> f,
                                                                    EnergyOut eo)
 {
-    __shared__ Vec4<double> sj[AD_THREADS];
+    __shared__ Vec4<double> sjb[2][AD_THREADS];            // two tiles: one barrier per tile (see the loop)
     const int base = blockIdx.x * (AD_THREADS * IB) + threadIdx.x;
-    double ax[IB], ay[IB], az[IB], si[IB];      // -2 x_i, -2 y_i, -2 z_i, |r_i|^2
-    int idx[IB];
+    double ax[IB], ay[IB], az[IB];              // 2 x_i, 2 y_i, 2 z_i
+    int idx[IB], thr[IB];                       // thr: high word of |r_i|^2 - (r_c^2 + rounding bound) > 0
 #pragma unroll
     for (int b = 0; b < IB; ++b) {
         idx[b] = base + b * AD_THREADS;
         // particles beyond nv: parked far away so that they never pass the filter
-        Vec4<double> e = {1.0e9, 1.0e9, 1.0e9, 3.0e18};
+        Vec4<double> e = {1.0e9, 1.0e9, 1.0e9, -3.0e18};
         if (idx[b] < p.nv) e = a.jv[idx[b]];
-        ax[b] = -2.0 * e.x; ay[b] = -2.0 * e.y; az[b] = -2.0 * e.z; si[b] = e.w;
+        ax[b] = 2.0 * e.x; ay[b] = 2.0 * e.y; az[b] = 2.0 * e.z;
+        thr[b] = __double2hiint(-e.w - a.thr);
     }
     double fx[IB] = {}, fy[IB] = {}, fz[IB] = {}, uv[IB] = {}, uw[IB] = {}, wv[IB] = {}, ww[IB] = {};
     int cv[IB] = {}, cw[IB] = {};
     bool any = false;
     const int nvj = p.nv + *a.ghost_count;
     const int tiles_v = (nvj + AD_THREADS - 1) / AD_THREADS, tiles_w = (a.nwg + AD_THREADS - 1) / AD_THREADS;
-    const int thr = a.thr_hi;
     // the tile after the current one is fetched into a register while the current one is evaluated, so a block never
     // waits for a global load between two tiles (it did: two barriers and an L2 round trip every 128 entries)
     auto fetch = [&](int t) {
-        Vec4<double> e = {-1.0e9, -1.0e9, -1.0e9, 3.0e18};              // padding: far from everything
+        Vec4<double> e = {-1.0e9, -1.0e9, -1.0e9, -3.0e18};             // padding: far from everything
         if (t < tiles_v + tiles_w) {
             const bool w = t >= tiles_v;
             const int j = (w ? t - tiles_v : t) * AD_THREADS + threadIdx.x;
@@ -181,56 +187,61 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double
         }
         return e;
     };
-    Vec4<double> nxt = fetch(blockIdx.y);
-    for (int t = blockIdx.y; t < tiles_v + tiles_w; t += gridDim.y) {
+    // Tile t is evaluated from buffer `cur` while tile t + gridDim.y is written into the other one, whose previous
+    // contents (the tile before t) every warp finished before it passed the barrier that published tile t.
+    int cur = 0;
+    sjb[0][threadIdx.x] = fetch(blockIdx.y);
+    Vec4<double> nxt = fetch(blockIdx.y + gridDim.y);
+    for (int t = blockIdx.y; t < tiles_v + tiles_w; t += gridDim.y, cur ^= 1) {
         const bool wall = t >= tiles_v;
         const int j0 = (wall ? t - tiles_v : t) * AD_THREADS;
         __syncthreads();
-        sj[threadIdx.x] = nxt;
-        __syncthreads();
-        nxt = fetch(t + gridDim.y);
+        sjb[cur ^ 1][threadIdx.x] = nxt;
+        nxt = fetch(t + 2 * gridDim.y);
+        const Vec4<double>* __restrict__ sj = sjb[cur];
         for (int k0 = 0; k0 < AD_THREADS; k0 += AD_UNROLL) {
-            // one integer instruction per test beside the four FP64 ones: the running minimum of the high words (for
-            // r^2 >= 0 the high word orders like the value; a slightly negative r^2 -- cancellation -- is smaller still)
-            int lowest = 0x7fffffff;
+            // one integer instruction per test beside the three FP64 ones: the running maximum, per particle i, of the
+            // high words of t (t > 0 orders like its high word; t < 0 is a negative integer and never the maximum)
+            int top[IB];
+#pragma unroll
+            for (int b = 0; b < IB; ++b) top[b] = (int)0x80000000;
 #pragma unroll
             for (int u = 0; u < AD_UNROLL; u += AD_JB) {
                 // AD_JB entries x IB particles independent chains, advanced one stage at a time
                 Vec4<double> q[AD_JB];
-                double r2[AD_JB][IB];
+                double t[AD_JB][IB];
 #pragma unroll
                 for (int w = 0; w < AD_JB; ++w) q[w] = sj[k0 + u + w];
 #pragma unroll
                 for (int w = 0; w < AD_JB; ++w)
 #pragma unroll
-                    for (int b = 0; b < IB; ++b) r2[w][b] = si[b] + q[w].w;
+                    for (int b = 0; b < IB; ++b) t[w][b] = fma(q[w].z, az[b], q[w].w);
 #pragma unroll
                 for (int w = 0; w < AD_JB; ++w)
 #pragma unroll
-                    for (int b = 0; b < IB; ++b) r2[w][b] = fma(az[b], q[w].z, r2[w][b]);
+                    for (int b = 0; b < IB; ++b) t[w][b] = fma(q[w].y, ay[b], t[w][b]);
 #pragma unroll
                 for (int w = 0; w < AD_JB; ++w)
 #pragma unroll
-                    for (int b = 0; b < IB; ++b) r2[w][b] = fma(ay[b], q[w].y, r2[w][b]);
+                    for (int b = 0; b < IB; ++b) t[w][b] = fma(q[w].x, ax[b], t[w][b]);
 #pragma unroll
                 for (int w = 0; w < AD_JB; ++w)
 #pragma unroll
-                    for (int b = 0; b < IB; ++b) r2[w][b] = fma(ax[b], q[w].x, r2[w][b]);
-#pragma unroll
-                for (int w = 0; w < AD_JB; ++w)
-#pragma unroll
-                    for (int b = 0; b < IB; ++b) lowest = min(lowest, __double2hiint(r2[w][b]));
+                    for (int b = 0; b < IB; ++b) top[b] = max(top[b], __double2hiint(t[w][b]));
             }
-            if (lowest < thr) {      // this lane has a candidate in the group: it redoes ITS flagged pairs exactly
+            bool cand = false;
+#pragma unroll
+            for (int b = 0; b < IB; ++b) cand |= top[b] >= thr[b];
+            if (cand) {              // this lane has a candidate in the group: it redoes ITS flagged pairs exactly
                 for (int u = 0; u < AD_UNROLL; ++u) {
                     const Vec4<double> q = sj[k0 + u];
 #pragma unroll
                     for (int b = 0; b < IB; ++b) {
-                        const double r2 = fma(ax[b], q.x, fma(ay[b], q.y, fma(az[b], q.z, si[b] + q.w)));
-                        if (__double2hiint(r2) >= thr) continue;               // same filter value as above
+                        const double t = fma(ax[b], q.x, fma(ay[b], q.y, fma(az[b], q.z, q.w)));
+                        if (__double2hiint(t) < thr[b]) continue;              // same filter value as above
                         if (!wall && j0 + k0 + u == idx[b]) continue;          // j == i skipped by index
-                        if (wall) ap_exact<ENERGY>(p, true, -0.5 * ax[b], -0.5 * ay[b], -0.5 * az[b], q, fx[b], fy[b], fz[b], uw[b], ww[b], cw[b]);
-                        else ap_exact<ENERGY>(p, false, -0.5 * ax[b], -0.5 * ay[b], -0.5 * az[b], q, fx[b], fy[b], fz[b], uv[b], wv[b], cv[b]);
+                        if (wall) ap_exact<ENERGY>(p, true, 0.5 * ax[b], 0.5 * ay[b], 0.5 * az[b], q, fx[b], fy[b], fz[b], uw[b], ww[b], cw[b]);
+                        else ap_exact<ENERGY>(p, false, 0.5 * ax[b], 0.5 * ay[b], 0.5 * az[b], q, fx[b], fy[b], fz[b], uv[b], wv[b], cv[b]);
                     }
                 }
                 any = true;

@@ -957,7 +957,8 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
         double smax = 0.0;
         for (int a = 0; a < box.dim; ++a) {
             if (box.bc[a] == MD_BC_PERIODIC && box.len[a] < 2.2 * lj.r_cut) ok = false;
-            const double h = 0.5 * box.len[a] + 1.1 * lj.r_cut;
+            // largest |coordinate| of an entry, ghosts included: x runs from r_c + 1 (see org below), y and z are centred
+            const double h = (a == 0 ? box.len[a] + lj.r_cut + 1.0 : 0.5 * box.len[a]) + 1.1 * lj.r_cut;
             smax += 2.0 * h * h;
         }
         if (ok) {
@@ -965,18 +966,18 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
             s->dot = true;
             if constexpr (std::is_same<T, double>::value) { a.jv = s->l.jv; a.jw = s->l.jw; }
             a.ghost_count = s->l.ghost_count; a.nwg = 0;
-            for (int k = 0; k < 3; ++k) a.half[k] = k < box.dim ? 0.5 * box.len[k] : 0.0;
+            // origin: x' = x + r_c + 1 >= r_c + 1 makes |r_i|^2 - r_c^2 - bound > 0 for every particle in the box (the
+            // filter compares positive doubles through their high words, md_allpairs.cuh); y, z: box centre
+            for (int k = 0; k < 3; ++k) a.org[k] = k < box.dim ? 0.5 * box.len[k] : 0.0;
+            a.org[0] = -(lj.r_cut + 1.0);
             a.edge = lj.r_cut * (1.0 + 1e-9) + 1e-9;
-            // filter threshold: r_c^2 plus a bound on the rounding of the 4-term dot-product form
-            const double thr = lj.r_cut * lj.r_cut + 64.0 * 2.3e-16 * smax + 1e-12;
-            long long bits;
-            memcpy(&bits, &thr, sizeof(bits));
-            a.thr_hi = (int)(bits >> 32) + 1;
+            // filter threshold: r_c^2 plus a bound on the rounding of the dot-product form and of |r_i|^2 - thr
+            a.thr = lj.r_cut * lj.r_cut + 64.0 * 2.3e-16 * smax + 1e-12;
             if constexpr (std::is_same<T, float>::value) {
                 md::AllPairsDotF& g = s->adf;
                 g.jv = s->l.jv; g.jw = s->l.jw; g.jv_id = s->l.jv_id; g.jw_id = s->l.jw_id; g.wr = s->l.wtr;
                 g.ghost_count = s->l.ghost_count; g.nwg = 0;
-                for (int k = 0; k < 3; ++k) g.half[k] = (float)a.half[k];
+                for (int k = 0; k < 3; ++k) g.half[k] = (float)(k < box.dim ? 0.5 * box.len[k] : 0.0);
                 g.edge = (float)(lj.r_cut * (1.0 + 1e-5) + 1e-4);
                 // fp32 filter: rounding of the 4-term form (~6 eps32 |r|^2 terms) plus the centring error
                 g.thr = (float)(lj.r_cut * lj.r_cut + 1e-6 * smax + 1e-3);

@@ -24,7 +24,11 @@
 
 namespace md {
 
-constexpr int VL_THREADS = 256;
+#ifndef MD_VL_THREADS
+#define MD_VL_THREADS 256
+#endif
+constexpr int VL_THREADS = MD_VL_THREADS;   // threads per block of the persistent kernel
+constexpr int VS_ITEMS = 8, VS_TILE = VL_THREADS * VS_ITEMS;   // in-kernel scan: counts per thread, per tile
 constexpr int VL_MAXN = 128;   // neighbour-list entries per particle
 constexpr int VL_MAXO = 256;   // outer-list entries per particle (two-level list, see phase_prune)
 // List layout: warp-blocked.  The lists of particles 32 b .. 32 b + 31 form one block of MAXK rows of 32 entries: entry k of
@@ -66,7 +70,7 @@ struct Verlet {
     int *onbr, *ocnt, *oheavy;
     T* wo;
     int *cell, *slot, *count, *start;
-    unsigned long long* tile_agg;   // scan: (rebuild generation, sum of the tile's counts) per tile of SCAN_TILE cells
+    unsigned long long* tile_agg;   // scan: (rebuild generation, sum of the tile's counts) per tile of VS_TILE cells
     const int* wstart;         // walls: [ncell + 1] ranges into the wall part of an image block
     const uint8_t* wnear;
     F4* r32;                   // [ntot] fp32 shadow of image block 0 (vapor part rewritten by every scatter); T = double only
@@ -608,7 +612,7 @@ __device__ __forceinline__ int block_sum_int(int x, int* ws)
     __syncthreads();
     int a = 0;
 #pragma unroll
-    for (int k = 0; k < SCAN_THREADS / 32; ++k) a += ws[k];
+    for (int k = 0; k < VL_THREADS / 32; ++k) a += ws[k];
     return a;
 }
 
@@ -617,17 +621,17 @@ __device__ __forceinline__ int block_sum_int(int x, int* ws)
 // sums before it -- read with relaxed loads, spinning while a word still carries an older generation (every block
 // publishes all its sums before it waits for any, so nobody waits for a waiter) -- then a warp-shuffle scan inside the
 // tile.  No second phase and no same-address atomics: 2048 warp atomics on the 21 tile sums of config 2 cost 10 us
-// when tried in the bin phase (profiles/r02_k_md_run.md).  blockDim.x must equal SCAN_THREADS.
+// when tried in the bin phase (profiles/r02_k_md_run.md).  blockDim.x must equal VL_THREADS.
 __device__ __forceinline__ void phase_scan(const int* __restrict__ count, int n, unsigned long long* __restrict__ tile_agg,
                                            unsigned int gen, int* __restrict__ start)
 {
-    __shared__ int ws[SCAN_THREADS / 32];
-    const int tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+    __shared__ int ws[VL_THREADS / 32];
+    const int tiles = (n + VS_TILE - 1) / VS_TILE;
     for (int t = blockIdx.x; t < tiles; t += gridDim.x) {
-        const int base = t * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+        const int base = t * VS_TILE + threadIdx.x * VS_ITEMS;
         int s = 0;
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) s += base + k < n ? count[base + k] : 0;
+        for (int k = 0; k < VS_ITEMS; ++k) s += base + k < n ? count[base + k] : 0;
         const int sum = block_sum_int(s, ws);
         if (threadIdx.x == 0) {
             const unsigned long long word = ((unsigned long long)gen << 32) | (unsigned int)sum;
@@ -635,16 +639,16 @@ __device__ __forceinline__ void phase_scan(const int* __restrict__ count, int n,
         }
     }
     for (int t = blockIdx.x; t < tiles; t += gridDim.x) {
-        const int base = t * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
-        int val[SCAN_ITEMS];
+        const int base = t * VS_TILE + threadIdx.x * VS_ITEMS;
+        int val[VS_ITEMS];
         int s = 0;
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
+        for (int k = 0; k < VS_ITEMS; ++k) {
             val[k] = base + k < n ? count[base + k] : 0;
             s += val[k];
         }
         int off = 0;
-        for (int k = threadIdx.x; k < t; k += SCAN_THREADS) {
+        for (int k = threadIdx.x; k < t; k += VL_THREADS) {
             unsigned long long word;
             do {
                 asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(word) : "l"(tile_agg + k) : "memory");
@@ -660,11 +664,11 @@ __device__ __forceinline__ void phase_scan(const int* __restrict__ count, int n,
         for (int k = 0; k < (int)(threadIdx.x >> 5); ++k) wofs += ws[k];
         int run = off + wofs + incl - s;
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
+        for (int k = 0; k < VS_ITEMS; ++k) {
             if (base + k < n) start[base + k] = run;     // counts are cleared in the list-build phase
             run += val[k];
         }
-        if (base <= n - 1 && n - 1 < base + SCAN_ITEMS) start[n] = run;
+        if (base <= n - 1 && n - 1 < base + VS_ITEMS) start[n] = run;
         __syncthreads();
     }
 }
@@ -1066,7 +1070,7 @@ __device__ __forceinline__ bool phase_prune(const Params<T>& p, const Verlet<T>&
 // MINB = resident blocks per SM the register budget is sized for: 2 (up to 128 registers, the latency-bound
 // sizes that fit one wave) or 3 (more warps to hide HBM latency once the state no longer fits in L2).
 template <typename T, int ROWS, int MINB>
-__global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
+__global__ void __launch_bounds__(VL_THREADS, (MINB * 256) / VL_THREADS) k_md_run(Params<T> p, Verlet<T> v, long long n_steps, int force_rebuild)
 {
     __shared__ unsigned long long s_times[10];
     GridBarrier bar_seq;
@@ -1178,7 +1182,7 @@ __global__ void __launch_bounds__(VL_THREADS, MINB) k_md_run(Params<T> p, Verlet
 // Diagnostics build only: the list-build phase as a kernel of its own, so that ncu can attribute its stalls.  It
 // rebuilds the list from the current cell order, which is what the list already holds.
 template <typename T, int ROWS>
-__global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_build(Params<T> p, Verlet<T> v, int c)
+__global__ void __launch_bounds__(VL_THREADS, 512 / VL_THREADS) k_dbg_build(Params<T> p, Verlet<T> v, int c)
 {
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x, gthreads = gridDim.x * blockDim.x;
     if (v.nprune > 0) phase_build<T, ROWS, true>(p, v, c, gtid, gthreads, v.flags[VF_HCAP], v.flags[VF_HCAP32], v.flags[VF_HPAR]);
@@ -1187,14 +1191,14 @@ __global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_build(Params<T> p, Verlet
 
 // Diagnostics build only: the prune phase as a kernel of its own (valid at any time: it re-prunes from the outer list).
 template <typename T>
-__global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_prune(Params<T> p, Verlet<T> v, int c)
+__global__ void __launch_bounds__(VL_THREADS, 512 / VL_THREADS) k_dbg_prune(Params<T> p, Verlet<T> v, int c)
 {
     phase_prune<T, 8>(p, v, c, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, 0, 0, v.flags[VF_HPAR] ^ 1);
 }
 
 // Diagnostics build only: the force part of the step phase as a kernel of its own (recomputes f(t)).
 template <typename T>
-__global__ void __launch_bounds__(VL_THREADS, 2) k_dbg_force(Params<T> p, Verlet<T> v, int c, int cv)
+__global__ void __launch_bounds__(VL_THREADS, 512 / VL_THREADS) k_dbg_force(Params<T> p, Verlet<T> v, int c, int cv)
 {
     bool unused = false;
     phase_step<T>(p, v, c, cv, true, false, false, unused, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, v.flags[VF_HPAR]);

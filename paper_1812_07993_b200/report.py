@@ -42,7 +42,7 @@ def measure(cfg, algo, precision, n_steps, torch, md, peaks):
                pair_tests_per_s=tests / sec, allpairs_equivalent_per_s=nv * (nv - 1.0 + nw) / sec, us_per_step=sec * 1e6,
                state_gbs=state_bytes / sec * 1e-9, state_frac_of_copy_peak=state_bytes / sec * 1e-9 / peaks["copy_gbs"])
     if algo == "allpairs":
-        flops = 7.0                                   # executed per test (1 add + 3 fma): DESIGN.md section 5
+        flops = 6.0                                   # executed per test (3 fma): DESIGN.md section 5
         peak = peaks["fp64_tflops"] if precision == 64 else peaks["fp32_tflops"]
         row["alu_tflops"] = tests * flops / sec * 1e-12
         row["alu_frac_of_measured_peak"] = row["alu_tflops"] / peak
