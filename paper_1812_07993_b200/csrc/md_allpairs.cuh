@@ -268,11 +268,11 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dot(Params<double
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// fp32 mode of the same kernel.  The filter is the same 4-instruction form in FP32 (1 FADD + 3 FFMA); its
-// rounding (~1e-6 |r|^2) is covered by a wider margin.  Candidates are NOT re-evaluated from the centred
-// ghost entries -- a ghost coordinate x +- L rounded to fp32 would cost 4e-6 sigma -- but from the original
-// positions with the two-sided minimum image of md_kernels.cuh (exact differences for near pairs), found
-// through the original index every entry carries.
+// fp32 mode of the same kernel.  The filter is the same three-instruction form in FP32 (3 FFMA, running integer
+// maximum of the float's bits per particle i); its rounding (~1e-6 |r|^2) is covered by a wider margin.  Candidates
+// are NOT re-evaluated from the shifted ghost entries -- a ghost coordinate x +- L rounded to fp32 would cost 4e-6
+// sigma -- but from the original positions with the two-sided minimum image of md_kernels.cuh (exact differences
+// for near pairs), found through the original index every entry carries.
 // ---------------------------------------------------------------------------------------------------------
 struct AllPairsDotF {
     Vec4<float>* jv;  int* jv_id;      // vapor entries + ghosts; id = particle index
@@ -280,8 +280,8 @@ struct AllPairsDotF {
     const Vec4<float>* wr;             // wall positions, caller order
     int* ghost_count;
     int nwg;
-    float thr;                         // candidate iff filter r^2 < thr
-    float half[3];
+    float thr;                         // r_c^2 + rounding bound: candidate iff bits(t) >= bits(|r_i|^2 - thr)
+    float org[3];                      // origin of the stored coordinates, as AllPairsDot::org
     float edge;
 };
 
@@ -291,16 +291,16 @@ __device__ __forceinline__ void push_images_f(const Params<float>& p, const AllP
 {
     float sx[2] = {0.f, 0.f}, sy[2] = {0.f, 0.f}, sz[2] = {0.f, 0.f};
     int nx = 1, ny = 1, nz = 1;
-    if (p.bc[0] == BC_PERIODIC) { if (x < a.edge - a.half[0]) sx[nx++] = p.L[0]; else if (x > a.half[0] - a.edge) sx[nx++] = -p.L[0]; }
-    if (p.bc[1] == BC_PERIODIC) { if (y < a.edge - a.half[1]) sy[ny++] = p.L[1]; else if (y > a.half[1] - a.edge) sy[ny++] = -p.L[1]; }
-    if (p.bc[2] == BC_PERIODIC) { if (z < a.edge - a.half[2]) sz[nz++] = p.L[2]; else if (z > a.half[2] - a.edge) sz[nz++] = -p.L[2]; }
+    if (p.bc[0] == BC_PERIODIC) { if (x < a.edge - a.org[0]) sx[nx++] = p.L[0]; else if (x > p.L[0] - a.org[0] - a.edge) sx[nx++] = -p.L[0]; }
+    if (p.bc[1] == BC_PERIODIC) { if (y < a.edge - a.org[1]) sy[ny++] = p.L[1]; else if (y > p.L[1] - a.org[1] - a.edge) sy[ny++] = -p.L[1]; }
+    if (p.bc[2] == BC_PERIODIC) { if (z < a.edge - a.org[2]) sz[nz++] = p.L[2]; else if (z > p.L[2] - a.org[2] - a.edge) sz[nz++] = -p.L[2]; }
     for (int c = 0; c < nz; ++c)
         for (int b = 0; b < ny; ++b)
             for (int q = 0; q < nx; ++q) {
                 if (q + b + c == 0) continue;
                 Vec4<float> e;
                 e.x = x + sx[q]; e.y = y + sy[b]; e.z = z + sz[c];
-                e.w = fmaf(e.z, e.z, fmaf(e.y, e.y, e.x * e.x));
+                e.w = -fmaf(e.z, e.z, fmaf(e.y, e.y, e.x * e.x));
                 const int k = base + atomicAdd(counter, 1);
                 out[k] = e;
                 out_id[k] = id;
@@ -332,8 +332,8 @@ __global__ void __launch_bounds__(256) k_apf_kick_drift_list(Params<float> p, St
     }
     f.fx[i] = 0.f; f.fy[i] = 0.f; f.fz[i] = 0.f;
     Vec4<float> e;
-    e.x = ri.x - a.half[0]; e.y = ri.y - a.half[1]; e.z = ri.z - a.half[2];
-    e.w = fmaf(e.z, e.z, fmaf(e.y, e.y, e.x * e.x));
+    e.x = ri.x - a.org[0]; e.y = ri.y - a.org[1]; e.z = ri.z - a.org[2];
+    e.w = -fmaf(e.z, e.z, fmaf(e.y, e.y, e.x * e.x));
     a.jv[i] = e;
     a.jv_id[i] = i;
     push_images_f(p, a, e.x, e.y, e.z, i, a.jv, a.jv_id, p.nv, a.ghost_count);
@@ -344,8 +344,8 @@ __global__ void k_apf_wall_list(Params<float> p, AllPairsDotF a, int* __restrict
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= p.nw) return;
     Vec4<float> e;
-    e.x = a.wr[i].x - a.half[0]; e.y = a.wr[i].y - a.half[1]; e.z = a.wr[i].z - a.half[2];
-    e.w = fmaf(e.z, e.z, fmaf(e.y, e.y, e.x * e.x));
+    e.x = a.wr[i].x - a.org[0]; e.y = a.wr[i].y - a.org[1]; e.z = a.wr[i].z - a.org[2];
+    e.w = -fmaf(e.z, e.z, fmaf(e.y, e.y, e.x * e.x));
     a.jw[i] = e;
     a.jw_id[i] = i;
     push_images_f(p, a, e.x, e.y, e.z, i, a.jw, a.jw_id, p.nw, counter);
@@ -355,33 +355,33 @@ template <bool ENERGY, int IB>
 __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dotf(Params<float> p, State<float> s, AllPairsDotF a,
                                                                     Force<float> f, EnergyOut eo)
 {
-    __shared__ Vec4<float> sj[AD_THREADS];
-    __shared__ int sid[AD_THREADS];
+    __shared__ Vec4<float> sj[AD_THREADS];               // one tile, two barriers per tile: the fp64 kernel's register
+    __shared__ int sid[AD_THREADS];                      // prefetch + second buffer measured 4-6 % slower here
     const int base = blockIdx.x * (AD_THREADS * IB) + threadIdx.x;
-    float ax[IB], ay[IB], az[IB], si[IB];
+    float ax[IB], ay[IB], az[IB];                          // 2 x_i, 2 y_i, 2 z_i
     Vec4<float> ro[IB];                                    // original positions, for the exact path
-    int idx[IB];
+    int idx[IB], thr[IB];                                  // thr: bits of |r_i|^2 - (r_c^2 + rounding bound) > 0
 #pragma unroll
     for (int b = 0; b < IB; ++b) {
         idx[b] = base + b * AD_THREADS;
-        Vec4<float> e = {1.0e9f, 1.0e9f, 1.0e9f, 3.0e18f};
+        Vec4<float> e = {1.0e9f, 1.0e9f, 1.0e9f, -3.0e18f};
         ro[b] = e;
         if (idx[b] < p.nv) { e = a.jv[idx[b]]; ro[b] = s.r[idx[b]]; }
-        ax[b] = -2.f * e.x; ay[b] = -2.f * e.y; az[b] = -2.f * e.z; si[b] = e.w;
+        ax[b] = 2.f * e.x; ay[b] = 2.f * e.y; az[b] = 2.f * e.z;
+        thr[b] = __float_as_int(-e.w - a.thr);
     }
     Acc<float, ENERGY> av[IB], aw[IB];
     bool any = false;
     const bool px = p.bc[0] == BC_PERIODIC, py = p.bc[1] == BC_PERIODIC, pz = p.bc[2] == BC_PERIODIC;
     const int nvj = p.nv + *a.ghost_count;
     const int tiles_v = (nvj + AD_THREADS - 1) / AD_THREADS, tiles_w = (a.nwg + AD_THREADS - 1) / AD_THREADS;
-    const float thr = a.thr;
     for (int t = blockIdx.y; t < tiles_v + tiles_w; t += gridDim.y) {
         const bool wall = t >= tiles_v;
         const int j0 = (wall ? t - tiles_v : t) * AD_THREADS;
         const int nj = wall ? a.nwg : nvj;
         __syncthreads();
         {
-            Vec4<float> e = {-1.0e9f, -1.0e9f, -1.0e9f, 3.0e18f};
+            Vec4<float> e = {-1.0e9f, -1.0e9f, -1.0e9f, -3.0e18f};
             int id = -1;
             if (j0 + threadIdx.x < nj) { e = (wall ? a.jw : a.jv)[j0 + threadIdx.x]; id = (wall ? a.jw_id : a.jv_id)[j0 + threadIdx.x]; }
             sj[threadIdx.x] = e;
@@ -389,21 +389,27 @@ __global__ void __launch_bounds__(AD_THREADS) k_force_allpairs_dotf(Params<float
         }
         __syncthreads();
         for (int k0 = 0; k0 < AD_THREADS; k0 += AD_UNROLL) {
-            bool cand = false;
+            // positive floats order like their bits, a negative t is a negative integer (see the fp64 kernel)
+            int top[IB];
+#pragma unroll
+            for (int b = 0; b < IB; ++b) top[b] = (int)0x80000000;
 #pragma unroll
             for (int u = 0; u < AD_UNROLL; ++u) {
                 const Vec4<float> q = sj[k0 + u];
 #pragma unroll
                 for (int b = 0; b < IB; ++b)
-                    cand |= fmaf(ax[b], q.x, fmaf(ay[b], q.y, fmaf(az[b], q.z, si[b] + q.w))) < thr;
+                    top[b] = max(top[b], __float_as_int(fmaf(ax[b], q.x, fmaf(ay[b], q.y, fmaf(az[b], q.z, q.w)))));
             }
+            bool cand = false;
+#pragma unroll
+            for (int b = 0; b < IB; ++b) cand |= top[b] >= thr[b];
             if (cand) {
                 for (int u = 0; u < AD_UNROLL; ++u) {
                     const Vec4<float> q = sj[k0 + u];
                     const int jo = sid[k0 + u];
 #pragma unroll
                     for (int b = 0; b < IB; ++b) {
-                        if (!(fmaf(ax[b], q.x, fmaf(ay[b], q.y, fmaf(az[b], q.z, si[b] + q.w))) < thr)) continue;
+                        if (__float_as_int(fmaf(ax[b], q.x, fmaf(ay[b], q.y, fmaf(az[b], q.z, q.w)))) < thr[b]) continue;
                         if (jo < 0 || idx[b] >= p.nv || (!wall && jo == idx[b])) continue;
                         const Vec4<float> rj = wall ? a.wr[jo] : s.r[jo];
                         float dx = ro[b].x - rj.x, dy = ro[b].y - rj.y, dz = ro[b].z - rj.z;

@@ -977,9 +977,9 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
                 md::AllPairsDotF& g = s->adf;
                 g.jv = s->l.jv; g.jw = s->l.jw; g.jv_id = s->l.jv_id; g.jw_id = s->l.jw_id; g.wr = s->l.wtr;
                 g.ghost_count = s->l.ghost_count; g.nwg = 0;
-                for (int k = 0; k < 3; ++k) g.half[k] = (float)(k < box.dim ? 0.5 * box.len[k] : 0.0);
+                for (int k = 0; k < 3; ++k) g.org[k] = (float)a.org[k];
                 g.edge = (float)(lj.r_cut * (1.0 + 1e-5) + 1e-4);
-                // fp32 filter: rounding of the 4-term form (~6 eps32 |r|^2 terms) plus the centring error
+                // fp32 filter: rounding of the dot-product form (~6 eps32 |r|^2 terms), of |r_i|^2 - thr and of the shift
                 g.thr = (float)(lj.r_cut * lj.r_cut + 1e-6 * smax + 1e-3);
             }
         }
