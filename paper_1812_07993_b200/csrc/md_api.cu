@@ -874,7 +874,8 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
             CK(cudaStreamSynchronize(stream));
             ad.nwg = adf.nwg = (int)nw + wg;
             const int tiles = cdiv(nv, md::AD_THREADS) + cdiv(ad.nwg, md::AD_THREADS) + 1;
-            // j slices: enough blocks to fill the GPU, and a block count that wastes little of the last wave
+            // j slices: enough blocks to fill the GPU, a block count that wastes little of the last wave, and among equals
+            // the finer split (measured at N = 65,536: 52 slices 0.625 of the FP64 peak, 128-220 slices 0.631-0.633)
             int dev = 0, sms = 148, nb = 4;
             cudaGetDevice(&dev);
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -885,9 +886,9 @@ int Sim<T>::init(const md_box& box, const md_lj& lj, const md_opts& o, long long
                 cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, md::k_force_allpairs_dotf<false, md::AD_IB>, md::AD_THREADS, 0);
             const int slots = std::max(1, nb * sms), ib = cdiv(nv, md::AD_THREADS * ad_ib);
             double best = -1.0;
-            for (int sl = 1; sl <= std::min(tiles, 96); ++sl) {
+            for (int sl = 1; sl <= std::min(std::max(tiles / 3, 1), 192); ++sl) {
                 const double waves = (double)ib * sl / slots;
-                const double eff = waves / std::ceil(waves) - (sl * 1e-4) + (waves >= 1.0 ? 0.0 : waves - 1.0);
+                const double eff = waves / std::ceil(waves) + (sl * 2e-4) + (waves >= 1.0 ? 0.0 : waves - 1.0);
                 if (eff > best) { best = eff; ad_slices = sl; }
             }
             if constexpr (std::is_same<T, double>::value)
