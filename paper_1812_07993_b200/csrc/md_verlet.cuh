@@ -115,7 +115,10 @@ __device__ __forceinline__ int vl_face(int raw) { return (raw >> VL_FACE_SHIFT) 
 #endif
 constexpr int VL_GROUP = MD_VL_GROUP;   // lanes sharing one heavy particle's list
 constexpr int VL_WARP_T = 48;           // lists longer than this (inside an adsorbed film: up to ~100 entries) get a whole warp
-constexpr int VL_WARP_ROUNDS = 1;       // such lists per idle warp and step
+#ifndef MD_VL_WARP_ROUNDS
+#define MD_VL_WARP_ROUNDS 1
+#endif
+constexpr int VL_WARP_ROUNDS = MD_VL_WARP_ROUNDS;       // such lists per idle warp and step
 
 // d = a - b folded to the nearest image by comparison (|true d| < r_c + skin < L/2): fp32 mode only, where a ghost
 // copy x + L would round the coordinate.  The shift goes on whichever particle sits at the top of the box so the
@@ -370,7 +373,7 @@ struct Carry {
     T vx, vy, vz;
     int raw, j0[VL_BATCH];
     bool valid = false;
-    int nh, hi, hraw, hj[4];
+    int nh, n32, hi, hraw, hj[4];
     T hvx, hvy, hvz;
     bool nhvalid = false, hvalid = false;
 };
@@ -461,11 +464,12 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         // barrier.  Group slots are numbered so that the blocks past the last particle (idle when the particles
         // fill less than one wave) take this work first and the rest is dealt round-robin over the other blocks,
         // one group per block and warp at a time.
-        int nh;
-        if (cyon && cy.nhvalid) nh = cy.nh;
+        int nh, n32;
+        if (cyon && cy.nhvalid) { nh = cy.nh; n32 = cy.n32; }
         else {
             nh = min(v.flags[VF_NHEAVY + hp], v.flags[VF_HCAP]);
-            if (cyon) { cy.nh = nh; cy.nhvalid = true; }
+            n32 = min(v.flags[VF_NHEAVY32 + hp], v.flags[VF_HCAP32]);
+            if (cyon) { cy.nh = nh; cy.n32 = n32; cy.nhvalid = true; }
         }
         const int lane = threadIdx.x & 31, sub = lane & (VL_GROUP - 1);
         const unsigned gmask = ((1u << VL_GROUP) - 1u) << (lane & ~(VL_GROUP - 1));
@@ -473,27 +477,45 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         const int nbl = min((int)gridDim.x, (p.nv + VL_THREADS - 1) / VL_THREADS), nsp = (int)gridDim.x - nbl;
         const int b = blockIdx.x, q = (lane / VL_GROUP) * (VL_THREADS / 32) + (threadIdx.x >> 5);
         // Lists longer than VL_WARP_T (a particle inside an adsorbed film has ~100 neighbours within r_c + skin): one
-        // per WARP of the idle blocks, lane l takes entries l, l + 32, l + 64, l + 96 -- one batch, a butterfly sum,
-        // and lane 0 integrates.  Walked by four lanes such a list would take 7 batches while the grid waits.
-        if (b >= nbl) {
-            const int n32 = min(v.flags[VF_NHEAVY32 + hp], v.flags[VF_HCAP32]), nw32 = nsp * (VL_THREADS / 32);
+        // per WARP, lane l takes entries l, l + 32, l + 64, l + 96 -- one batch, a butterfly sum, and lane 0 integrates.
+        // Walked by four lanes such a list would take 7 batches while the grid waits.  The warps of the idle blocks take
+        // VL_WARP_ROUNDS each first; the rest goes to the warps of the particle blocks, one each after their own
+        // particles (a film that covers the wall has ~1,500 such lists at N = 65,536, the idle blocks 320 warps).
+        if (n32 > 0) {
+            const int icap = nsp * (VL_THREADS / 32) * VL_WARP_ROUNDS;
+            const bool idle = b >= nbl;
+            // particle blocks: one block after the other, last warp first (spilled lane groups start at warp 0)
+            const int h0 = idle ? (b - nbl) + nsp * (threadIdx.x >> 5) : icap + (VL_THREADS / 32 - 1 - (threadIdx.x >> 5)) * nbl + b;
+            const int hlim = idle ? min(n32, icap) : n32, nw32 = (idle ? nsp : nbl) * (VL_THREADS / 32);
             const PairCoef<T> qv = coef_vv(p), qw = coef_vw(p);
             const bool fpx = sizeof(T) == 4 && p.bc[0] == BC_PERIODIC, fpy = sizeof(T) == 4 && p.bc[1] == BC_PERIODIC,
                        fpz = sizeof(T) == 4 && p.bc[2] == BC_PERIODIC;
-            for (int h = (b - nbl) + nsp * (threadIdx.x >> 5); h < n32; h += nw32) {
-                const int top = p.nv - 1 - h;
-                const int i = v.cell[top], raw = v.slot[top];
-                const int nvv = vl_nvv(raw), n = nvv + vl_nvw(raw);
-                int j[4];
-                Vec4<T> rj[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int k = lane + 32 * u;
-                    j[u] = k < n ? v.nbr[vl_base(i, VL_MAXN) + (k < nvv ? k : k + VL_MAXN - n) * VL_LS] : -1;
-                }
-                const Vec4<T> ri = rcur[i];
+            // a warp of a particle block that holds no lane group keeps its list's head in the group's carry registers
+            // (the warp's first lane group has its lowest slot number: warp-uniform)
+            const bool wcarry = cyon && !idle && !(nsp * GPB + (int)(threadIdx.x >> 5) * nbl + b < nh);
+            for (int h = h0; h < hlim; h += nw32) {
+                const bool first = h == h0, kept = wcarry && first && cy.hvalid;
+                int i, raw, j[4];
                 T vx = T(0), vy = T(0), vz = T(0);
-                if (lane == 0) { vx = lam * s.vx[i]; vy = lam * s.vy[i]; vz = lam * s.vz[i]; }
+                if (kept) {
+                    i = cy.hi; raw = cy.hraw; vx = cy.hvx; vy = cy.hvy; vz = cy.hvz;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) j[u] = cy.hj[u];
+                } else {
+                    const int top = p.nv - 1 - h;
+                    i = v.cell[top]; raw = v.slot[top];
+                    const int nv0 = vl_nvv(raw), n0 = nv0 + vl_nvw(raw);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int k = lane + 32 * u;
+                        j[u] = k < n0 ? v.nbr[vl_base(i, VL_MAXN) + (k < nv0 ? k : k + VL_MAXN - n0) * VL_LS] : -1;
+                    }
+                    if (lane == 0) { vx = s.vx[i]; vy = s.vy[i]; vz = s.vz[i]; }
+                }
+                const int nvv = vl_nvv(raw);
+                Vec4<T> rj[4];
+                const Vec4<T> ri = rcur[i];
+                vx = lam * vx; vy = lam * vy; vz = lam * vz;
 #pragma unroll
                 for (int u = 0; u < 4; ++u) rj[u] = rcur[max(j[u], 0)];
                 Acc<T, false> a;
@@ -518,6 +540,12 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
                     if (!drift) { v.f.fx[i] = fx; v.f.fy[i] = fy; v.f.fz[i] = fz; }
                     Vec4<T> rn = ri;
                     integrate(i, ri, vx, vy, vz, fx, fy, fz, rn, vl_face(raw));
+                }
+                if (wcarry && first) {
+                    cy.hi = i; cy.hraw = raw; cy.hvx = vx; cy.hvy = vy; cy.hvz = vz;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) cy.hj[u] = j[u];
+                    cy.hvalid = drift;
                 }
             }
         }
@@ -1083,7 +1111,9 @@ __global__ void __launch_bounds__(VL_THREADS, (MINB * 256) / VL_THREADS) k_md_ru
     const bool cyon = MINB == 2 && v.carry && !thermo && gthreads >= p.nv;      // (the 3-blocks-per-SM variant serves N > one wave)
     // lane groups in the blocks past the last particle (none once the particles fill the grid)
     const int nidle = max((int)gridDim.x - (p.nv + VL_THREADS - 1) / VL_THREADS, 0);
-    const int hcap = nidle * (VL_THREADS / VL_GROUP), hcap32 = nidle * (VL_THREADS / 32) * VL_WARP_ROUNDS;
+    // whole-warp lists: VL_WARP_ROUNDS per warp of the idle blocks, one per warp of the particle blocks
+    const int hcap = nidle * (VL_THREADS / VL_GROUP),
+              hcap32 = (nidle * VL_WARP_ROUNDS + ((int)gridDim.x - nidle)) * (VL_THREADS / 32);
     if (gtid == 0)
         for (int k = 0; k < 10; ++k) s_times[k] = 0;
     unsigned long long t0 = gtid == 0 ? now_ns() : 0ull, t1;

@@ -229,6 +229,29 @@ def config2(seed=BASE_SEED + 2):
     return cylinder_config(65536, seed, "cfg2_cyl3d_64k", steps=10000, box=110.0, length=40)
 
 
+def config2_condensed(seed=BASE_SEED + 2, side=12.0, density=0.6, corner=(14.0, 14.0, 14.0)):
+    """config 2 with part of the vapor condensed: the vapor particles inside a cube of `side` at `corner` (far from the pore)
+    are replaced, one for one, by a jittered simple-cubic lattice at liquid `density` filling the cube (the rest of the
+    replaced particles come from the end of the array).  About 1,000 particles then have 60-90 neighbours within
+    r_c + skin -- the state a long run of config 2 reaches on the pore wall -- while N_v stays 65,536.  Velocities unchanged."""
+    cfg = config2(seed)
+    rng = SplitMix64(seed + 77)
+    a = density ** (-1.0 / 3.0)
+    m = int(math.floor(side / a))
+    grid = np.array([(i, j, k) for i in range(m) for j in range(m) for k in range(m)], dtype=np.float64)
+    drop = np.array(corner) + 0.5 * a + a * grid + 0.1 * a * (rng.uniform(3 * len(grid)).reshape(-1, 3) * 2.0 - 1.0)
+    pos = cfg["pos"].copy()
+    lo, hi = np.array(corner) - 1.0, np.array(corner) + m * a + 1.0         # 1 sigma clear of the remaining vapor
+    inside = np.nonzero(np.all((pos > lo) & (pos < hi), axis=1))[0]
+    n = len(drop)
+    assert len(inside) <= n < len(pos)
+    outside_tail = [i for i in range(len(pos) - 1, -1, -1) if i not in set(inside.tolist())][: n - len(inside)]
+    idx = np.concatenate([inside, np.array(outside_tail, dtype=np.int64)])
+    pos[idx] = drop
+    cfg.update(name="cfg2_condensed", pos=np.ascontiguousarray(pos), n_droplet=n)
+    return cfg
+
+
 def config3(shape, seed=None, n_vapor=262144):
     """3D pore-shape variants: shape in {'cone', 'inkbottle', 'slit'}."""
     k = ("cone", "inkbottle", "slit").index(shape)

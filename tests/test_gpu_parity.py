@@ -141,6 +141,24 @@ def test_verlet_heavy_lane_groups(heavy_list):
     check_traj(cfg, "verlet", 100, cells_oracle=True, chunks=(1, 99))
 
 
+def test_verlet_condensed_state_whole_warp_lists_on_every_block():
+    """config 2 with 1,000 particles condensed into a droplet (inputs.config2_condensed): ~730 lists of 50-80 entries, more
+    than the warps of the idle blocks (264-320 at this size), so the persistent kernel hands the rest to the warps of the
+    particle blocks after their own particles; ~300 more go to 4-lane groups.  Step 0 and a 60-step trajectory (several
+    prunes and a full rebuild in the droplet) against the oracle, then the profile path over another list event."""
+    cfg = I.config2_condensed()
+    assert cfg["n_droplet"] == 1000
+    check_step0(cfg, "verlet")
+    check_traj(cfg, "verlet", 60, cells_oracle=True, chunks=(1, 22, 37))
+    sim = make_sim(cfg, "verlet")
+    k = sim.profile_step(60)
+    assert k["rebuilds"] + k["prunes"] >= 2
+    ref = O.run(cfg, 60, cells=True)
+    st = sim.get_state()
+    assert traj_error(st["pos"], ref["pos"], cfg["box_len"], cfg["bc"]) <= TRAJ_TOL
+    sim.close()
+
+
 def test_single_particle_and_no_walls():
     cfg = I.small_case(3, 1, (10.0, 10.0, 10.0), (0, 1, 0), seed=3)
     for algo in ALGOS:
