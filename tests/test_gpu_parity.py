@@ -157,6 +157,9 @@ def test_verlet_condensed_state_whole_warp_lists_on_every_block():
     st = sim.get_state()
     assert traj_error(st["pos"], ref["pos"], cfg["box_len"], cfg["bc"]) <= TRAJ_TOL
     sim.close()
+    # the same lists in fp32 mode (the whole-warp walk folds per pair there), against the oracle on the float-rounded input
+    c32 = _float_rounded(cfg)
+    check_step0(c32, "verlet", ref=O.forces(c32, cells=True), precision=32, ftol=1e-4, bracket=_cutoff_bracket(c32, cells=True))
 
 
 def test_single_particle_and_no_walls():
