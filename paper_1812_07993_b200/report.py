@@ -60,6 +60,10 @@ def main():
     ap.add_argument("--precisions", default="64,32", help="config 4 precisions to run (subset)")
     ap.add_argument("--steps", type=int, default=0, help="override the number of timed steps of every row (0: per-config defaults)")
     ap.add_argument("--json", default="")
+    ap.add_argument("--split", default="", help="instead of the table: the persistent kernel's own timers (md_profile_step) for "
+                    "these workloads, comma separated: cfg0, cfg1, cfg2, cfg3, 2pK (config 4 at 2^K); --steps per launch "
+                    "(default 2000) after --split-warmup steps (default 500)")
+    ap.add_argument("--split-warmup", type=int, default=500)
     args = ap.parse_args()
     import torch
 
@@ -68,6 +72,27 @@ def main():
 
     if not torch.cuda.is_available():
         raise SystemExit("report: no CUDA device; the CUDA path has no fallback")
+    if args.split:
+        print("| workload | us per step: total = phase + barrier wait + list events | full rebuilds (us each: bin / scan / scatter / build) "
+              "| prunes (us each) |\n|---|---|---|---|")
+        for name in args.split.split(","):
+            cfg = {"cfg0": I.config0, "cfg1": I.config1, "cfg2": I.config2, "cfg3": lambda: I.config3("cone")}.get(
+                name, lambda: I.config4(int(name[2:])))()
+            sim = md.Simulation(cfg, algo="verlet")
+            done = 0
+            while done < args.split_warmup:                      # long warm-ups (the film on the pore wall) in 20,000-step launches
+                n = min(20000, args.split_warmup - done)
+                sim.step(n)
+                done += n
+            n = args.steps or 2000
+            k = sim.profile_step(n)
+            us = [x * 1e3 / n for x in k["ms"]]
+            print("| %s after %d steps | %.2f = %.2f + %.2f + %.2f | %d (%s) | %d (%.1f) |" % (
+                name, args.split_warmup, k["total_ms"] * 1e3 / n, us[0], us[1], us[2], k["rebuilds"],
+                " / ".join("%.1f" % (x * 1e3 / max(k["rebuilds"], 1)) for x in k["rebuild_ms"]), k["prunes"],
+                k["prune_ms"] * 1e3 / max(k["prunes"], 1)), flush=True)
+            sim.close()
+        return
     peaks = md.measure_peaks()
     want = {int(x) for x in args.configs.split(",")}
     rows = []
