@@ -114,7 +114,10 @@ __device__ __forceinline__ int vl_face(int raw) { return (raw >> VL_FACE_SHIFT) 
 #define MD_VL_GROUP 4
 #endif
 constexpr int VL_GROUP = MD_VL_GROUP;   // lanes sharing one heavy particle's list
-constexpr int VL_WARP_T = 48;           // lists longer than this (inside an adsorbed film: up to ~100 entries) get a whole warp
+#ifndef MD_VL_WARP_T
+#define MD_VL_WARP_T 48
+#endif
+constexpr int VL_WARP_T = MD_VL_WARP_T;   // lists longer than this (inside an adsorbed film: up to ~100 entries) get a whole warp
 #ifndef MD_VL_WARP_ROUNDS
 #define MD_VL_WARP_ROUNDS 1
 #endif
