@@ -481,15 +481,20 @@ __device__ __forceinline__ void phase_step(const Params<T>& p, const Verlet<T>& 
         const int b = blockIdx.x, q = (lane / VL_GROUP) * (VL_THREADS / 32) + (threadIdx.x >> 5);
         // Lists longer than VL_WARP_T (a particle inside an adsorbed film has ~100 neighbours within r_c + skin): one
         // per WARP, lane l takes entries l, l + 32, l + 64, l + 96 -- one batch, a butterfly sum, and lane 0 integrates.
-        // Walked by four lanes such a list would take 7 batches while the grid waits.  The warps of the idle blocks take
-        // VL_WARP_ROUNDS each first; the rest goes to the warps of the particle blocks, one each after their own
-        // particles (a film that covers the wall has ~1,500 such lists at N = 65,536, the idle blocks 320 warps).
+        // Walked by four lanes such a list would take 7 batches while the grid waits.  The warps of the idle blocks that
+        // hold no lane group take VL_WARP_ROUNDS each first (the group slots below fill every idle block's warps from
+        // warp 0 up, these lists from its last warp down: a warp with eight groups AND such a list was the slowest of
+        // the grid, 6.2 us against 4.8, once a film covers the wall); the rest goes to the warps of the particle blocks,
+        // one each after their own particles (the film has ~1,500 such lists at N = 65,536, the idle blocks 320 warps).
         if (n32 > 0) {
-            const int icap = nsp * (VL_THREADS / 32) * VL_WARP_ROUNDS;
+            constexpr int WPB = VL_THREADS / 32;
+            const int wi = threadIdx.x >> 5, back = WPB - 1 - wi;
+            const int nfree = nsp > 0 ? max(WPB - (nh + nsp * GPW - 1) / (nsp * GPW), 0) : 0;   // idle warps per block without groups
+            const int icap = nsp * nfree * VL_WARP_ROUNDS;
             const bool idle = b >= nbl;
-            // particle blocks: one block after the other, last warp first (spilled lane groups start at warp 0)
-            const int h0 = idle ? (b - nbl) + nsp * (threadIdx.x >> 5) : icap + (VL_THREADS / 32 - 1 - (threadIdx.x >> 5)) * nbl + b;
-            const int hlim = idle ? min(n32, icap) : n32, nw32 = (idle ? nsp : nbl) * (VL_THREADS / 32);
+            // idle blocks: block after block, last warp first; particle blocks likewise (spilled lane groups start at warp 0)
+            const int h0 = idle ? (back < nfree ? (b - nbl) + nsp * back : n32) : icap + back * nbl + b;
+            const int hlim = idle ? min(n32, icap) : n32, nw32 = idle ? nsp * nfree : nbl * WPB;
             const PairCoef<T> qv = coef_vv(p), qw = coef_vw(p);
             const bool fpx = sizeof(T) == 4 && p.bc[0] == BC_PERIODIC, fpy = sizeof(T) == 4 && p.bc[1] == BC_PERIODIC,
                        fpz = sizeof(T) == 4 && p.bc[2] == BC_PERIODIC;
