@@ -229,13 +229,13 @@ def config2(seed=BASE_SEED + 2):
     return cylinder_config(65536, seed, "cfg2_cyl3d_64k", steps=10000, box=110.0, length=40)
 
 
-def config2_condensed(seed=BASE_SEED + 2, side=12.0, density=0.6, corner=(14.0, 14.0, 14.0)):
-    """config 2 with part of the vapor condensed: the vapor particles inside a cube of `side` at `corner` (far from the pore)
-    are replaced, one for one, by a jittered simple-cubic lattice at liquid `density` filling the cube (the rest of the
-    replaced particles come from the end of the array).  About 1,000 particles then have 60-90 neighbours within
-    r_c + skin -- the state a long run of config 2 reaches on the pore wall -- while N_v stays 65,536.  Velocities unchanged."""
-    cfg = config2(seed)
-    rng = SplitMix64(seed + 77)
+def condense(cfg, side=12.0, density=0.6, corner=(14.0, 14.0, 14.0), name=None):
+    """A 3D configuration with part of its vapor condensed: the vapor particles inside a cube of `side` at `corner` (far
+    from the pore) are replaced, one for one, by a jittered simple-cubic lattice at liquid `density` filling the cube (the
+    rest of the replaced particles come from the end of the array).  About 1,000 particles then have 60-90 neighbours within
+    r_c + skin -- the state a long run reaches on the pore wall -- while N_v stays the same.  Velocities unchanged."""
+    cfg = dict(cfg)
+    rng = SplitMix64(cfg["seed"] + 77)
     a = density ** (-1.0 / 3.0)
     m = int(math.floor(side / a))
     grid = np.array([(i, j, k) for i in range(m) for j in range(m) for k in range(m)], dtype=np.float64)
@@ -245,11 +245,17 @@ def config2_condensed(seed=BASE_SEED + 2, side=12.0, density=0.6, corner=(14.0, 
     inside = np.nonzero(np.all((pos > lo) & (pos < hi), axis=1))[0]
     n = len(drop)
     assert len(inside) <= n < len(pos)
-    outside_tail = [i for i in range(len(pos) - 1, -1, -1) if i not in set(inside.tolist())][: n - len(inside)]
+    taken = set(inside.tolist())
+    outside_tail = [i for i in range(len(pos) - 1, -1, -1) if i not in taken][: n - len(inside)]
     idx = np.concatenate([inside, np.array(outside_tail, dtype=np.int64)])
     pos[idx] = drop
-    cfg.update(name="cfg2_condensed", pos=np.ascontiguousarray(pos), n_droplet=n)
+    cfg.update(name=name or cfg["name"] + "_condensed", pos=np.ascontiguousarray(pos), n_droplet=n)
     return cfg
+
+
+def config2_condensed(seed=BASE_SEED + 2):
+    """config 2 with 1,000 of its 65,536 vapor particles condensed into a droplet (see condense)."""
+    return condense(config2(seed), name="cfg2_condensed")
 
 
 def config3(shape, seed=None, n_vapor=262144):

@@ -162,6 +162,16 @@ def test_verlet_condensed_state_whole_warp_lists_on_every_block():
     check_step0(c32, "verlet", ref=O.forces(c32, cells=True), precision=32, ftol=1e-4, bracket=_cutoff_bracket(c32, cells=True))
 
 
+def test_verlet_condensed_state_three_blocks_per_sm_variant():
+    """The same droplet in a 100,000-particle box: the 80-register build of the persistent kernel (several particles per
+    thread, no idle blocks), where every whole-warp list is taken by a particle-block warp after its own particles and the
+    lists of 13-48 entries stay with their own threads.  Step 0 and a 60-step trajectory against the oracle."""
+    cfg = I.condense(I.cylinder_config(100000, 4321, "cyl3d_100k"))
+    assert cfg["n_droplet"] == 1000 and cfg["n_vapor"] == 100000
+    check_step0(cfg, "verlet")
+    check_traj(cfg, "verlet", 60, cells_oracle=True, chunks=(1, 22, 37))
+
+
 def test_single_particle_and_no_walls():
     cfg = I.small_case(3, 1, (10.0, 10.0, 10.0), (0, 1, 0), seed=3)
     for algo in ALGOS:
