@@ -955,33 +955,41 @@ int create_t(md_sim** out, const md_box& box, const md_pore* pore, const md_lj& 
     if (algo == MD_FORCE_ALLPAIRS) {
         // dot-product kernel: needs at most one periodic image per dimension inside r_c + margin of a face
         bool ok = true;
-        double smax = 0.0;
-        for (int a = 0; a < box.dim; ++a) {
+        for (int a = 0; a < box.dim; ++a)
             if (box.bc[a] == MD_BC_PERIODIC && box.len[a] < 2.2 * lj.r_cut) ok = false;
-            // largest |coordinate| of an entry, ghosts included: x runs from r_c + 1 (see org below), y and z are centred
-            const double h = (a == 0 ? box.len[a] + lj.r_cut + 1.0 : 0.5 * box.len[a]) + 1.1 * lj.r_cut;
-            smax += 2.0 * h * h;
-        }
         if (ok) {
             md::AllPairsDot& a = s->ad;
             s->dot = true;
             if constexpr (std::is_same<T, double>::value) { a.jv = s->l.jv; a.jw = s->l.jw; }
             a.ghost_count = s->l.ghost_count; a.nwg = 0;
-            // origin: x' = x + r_c + 1 >= r_c + 1 makes |r_i|^2 - r_c^2 - bound > 0 for every particle in the box (the
-            // filter compares positive doubles through their high words, md_allpairs.cuh); y, z: box centre
+            // Origin: x' = x + shift with shift^2 > thr makes |r_i|^2 - thr > 0 for every particle in the box (the filter
+            // compares positive numbers through their bits, md_allpairs.cuh); y, z: box centre.  thr = r_c^2 plus a bound
+            // on the rounding of the dot-product form and of |r_i|^2 - thr, which grows with the largest |coordinate| of
+            // an entry (ghosts included) and so with the shift itself: r_c + 1 unless the box is thousands of sigma wide
+            // in fp32 mode (~6 eps32 |r|^2 terms; fp64: 64 x 2.3e-16 |r|^2).
+            constexpr bool F32 = std::is_same<T, float>::value;
+            double shift = lj.r_cut + 1.0, thr = 0.0;
+            for (int it = 0; it < 8; ++it) {
+                double smax = 0.0;
+                for (int k = 0; k < box.dim; ++k) {
+                    const double h = (k == 0 ? box.len[k] + shift : 0.5 * box.len[k]) + 1.1 * lj.r_cut;
+                    smax += 2.0 * h * h;
+                }
+                thr = lj.r_cut * lj.r_cut + (F32 ? 1e-6 * smax + 1e-3 : 64.0 * 2.3e-16 * smax + 1e-12);
+                if (shift * shift > 1.05 * thr) break;
+                shift = std::sqrt(1.05 * thr) + 1.0;
+            }
             for (int k = 0; k < 3; ++k) a.org[k] = k < box.dim ? 0.5 * box.len[k] : 0.0;
-            a.org[0] = -(lj.r_cut + 1.0);
+            a.org[0] = -shift;
             a.edge = lj.r_cut * (1.0 + 1e-9) + 1e-9;
-            // filter threshold: r_c^2 plus a bound on the rounding of the dot-product form and of |r_i|^2 - thr
-            a.thr = lj.r_cut * lj.r_cut + 64.0 * 2.3e-16 * smax + 1e-12;
-            if constexpr (std::is_same<T, float>::value) {
+            a.thr = thr;
+            if constexpr (F32) {
                 md::AllPairsDotF& g = s->adf;
                 g.jv = s->l.jv; g.jw = s->l.jw; g.jv_id = s->l.jv_id; g.jw_id = s->l.jw_id; g.wr = s->l.wtr;
                 g.ghost_count = s->l.ghost_count; g.nwg = 0;
                 for (int k = 0; k < 3; ++k) g.org[k] = (float)a.org[k];
                 g.edge = (float)(lj.r_cut * (1.0 + 1e-5) + 1e-4);
-                // fp32 filter: rounding of the dot-product form (~6 eps32 |r|^2 terms), of |r_i|^2 - thr and of the shift
-                g.thr = (float)(lj.r_cut * lj.r_cut + 1e-6 * smax + 1e-3);
+                g.thr = (float)thr;
             }
         }
     }

@@ -172,6 +172,24 @@ def test_verlet_condensed_state_three_blocks_per_sm_variant():
     check_traj(cfg, "verlet", 60, cells_oracle=True, chunks=(1, 22, 37))
 
 
+def test_allpairs_filter_in_a_huge_sparse_box():
+    """The all-pairs filter compares t = |r_i|^2 - r^2 with |r_i|^2 - (r_c^2 + rounding bound) through the bits of positive
+    numbers; the bound grows with the box (fp32: 1e-6 |r|^2), so in a box thousands of sigma wide the origin has to move out
+    further than r_c + 1 or the threshold of a particle near x = 0 at the y, z centre turns negative.  Three dense clusters in a
+    3000 sigma periodic box -- at that spot, in the far corner and in the middle -- against the oracle, fp64 and fp32."""
+    L = 3000.0
+    base = I.small_case(3, 240, (9.0, 9.0, 9.0), (1, 1, 1), n_wall=12, seed=31, min_sep=0.9)
+    spots = np.array([[0.3, 0.5 * L - 4.0, 0.5 * L - 4.0], [L - 9.5, 0.4, 0.6], [0.5 * L, 0.5 * L, 0.5 * L]])
+    pos = np.concatenate([base["pos"][k::3] + spots[k] for k in range(3)])
+    vel = np.concatenate([base["vel"][k::3] for k in range(3)])
+    cfg = dict(base, pos=np.ascontiguousarray(pos), vel=np.ascontiguousarray(vel), wall=base["wall"] + spots[0], box_len=[L, L, L], bc=[0, 0, 0])
+    ref = O.forces(cfg)
+    assert ref["pairs_vv"] > 400 and ref["pairs_vw"] > 20
+    check_step0(cfg, "allpairs", ref=ref)
+    c32 = _float_rounded(cfg)
+    check_step0(c32, "allpairs", ref=O.forces(c32), precision=32, ftol=1e-4, bracket=_cutoff_bracket(c32, cells=False))
+
+
 def test_single_particle_and_no_walls():
     cfg = I.small_case(3, 1, (10.0, 10.0, 10.0), (0, 1, 0), seed=3)
     for algo in ALGOS:
